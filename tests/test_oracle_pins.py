@@ -1,0 +1,331 @@
+"""Pins for the float64 oracle: what physics and mathematics fix, independent of any code of ours.
+
+Each test names the pin of DESIGN.md section 6 (after SURVEY.md section 8(c) C.7) it implements and
+the mistake it is meant to catch.  None of these re-types the oracle's formula as its own check:
+the expectations are an analytic solution (Hankel function via SciPy), conservation laws, symmetry
+(reciprocity), the adjoint identity against complex-step derivatives of the forward code, finite
+differences of the misfit, closed-form special cases and brute force on tiny inputs.
+"""
+import numpy as np
+import pytest
+from scipy.special import hankel2
+
+import gpr_inputs as gi
+import oracle
+from helpers import problem, rel_l2
+
+C0, MU0, EPS0 = gi.C0, gi.MU0, gi.EPS0
+
+
+# ------------------------------------------------------------------------------------------------
+# Pin 1: analytic 2-D line source  (forward scheme, source scale and sign, time alignment, CPML)
+# ------------------------------------------------------------------------------------------------
+def _analytic_trace(w, dt, rho, eps_r, sigma):
+    """Ez(rho, t_n = n dt) for a z-directed line current I(t) sampled as w[n] = I((n+1/2) dt) in a
+    homogeneous medium: Ez(w) = -(w mu0 / 4) I(w) H0^(2)(k rho), k = w sqrt(mu0 eps (1 - j s/(w eps)))
+    (Harrington, Time-Harmonic EM Fields, eq. 5-84), e^{+jwt} convention."""
+    nt = len(w)
+    nfft = 8 * nt
+    W = np.fft.rfft(w, nfft)
+    om = 2.0 * np.pi * np.fft.rfftfreq(nfft, dt)
+    E = np.zeros_like(W)
+    o = om[1:]
+    eps = EPS0 * eps_r
+    k = o * np.sqrt(MU0 * eps * (1.0 - 1j * sigma / (o * eps)))
+    k = np.where(k.imag > 0, -k, k)              # decaying branch for e^{+jwt}
+    E[1:] = -(o * MU0 / 4.0) * W[1:] * np.exp(-1j * o * dt / 2.0) * hankel2(0, k * rho)
+    return np.fft.irfft(E, nfft)[:nt]
+
+
+def _line_source_error(dx, eps_r, sigma, offsets_m):
+    f = 400e6
+    dt = 2e-11 * dx / 0.01
+    nt = int(round(12e-9 / dt))
+    npml = int(round(0.2 / dx))
+    n = int(round(1.4 / dx)) + 2 * npml + 1
+    c = n // 2
+    order, smax, kmax, amax = gi.cpml_defaults(dx, f, eps_r)
+    w = gi.ricker(nt, dt, f).astype(np.float64)
+    recs = []
+    for off in offsets_m:
+        k = int(round(off / dx))
+        recs.append((c, c + k))                    # on-axis
+        kd = int(round(off / dx / np.sqrt(2)))
+        recs.append((c + kd, c + kd))              # diagonal
+    pb = oracle.Problem(nz=n, nx=n, dx=dx, dt=dt, nt=nt, npml=npml, pml_order=order, pml_sigma_max=smax,
+                        pml_kappa_max=kmax, pml_alpha_max=amax, src_zx=np.array([[c, c]]),
+                        rec_zx=np.array([recs]), wavelet=w)
+    tr = oracle.forward(pb, np.full((n, n), eps_r), np.full((n, n), sigma))["traces"][0]
+    errs = []
+    for r, (z, x) in enumerate(recs):
+        rho = dx * np.hypot(z - c, x - c)
+        errs.append(rel_l2(tr[:, r], _analytic_trace(w, dt, rho, eps_r, sigma)))
+    return np.array(errs)
+
+
+@pytest.mark.parametrize("eps_r,sigma", [(1.0, 0.0), (4.0, 5e-3)])
+def test_pin1_line_source_green_function_second_order(eps_r, sigma):
+    """A wrong source scale/sign, a half-step time misalignment, a missing Cb factor or a reflecting
+    CPML all give O(1) or O(dt) errors here; the correct scheme converges with order 2."""
+    offs = (0.2, 0.4, 0.6)
+    e1 = _line_source_error(0.01, eps_r, sigma, offs)
+    e2 = _line_source_error(0.005, eps_r, sigma, offs)
+    bound = 5e-3 if eps_r == 1.0 else 4e-2      # grid dispersion grows with sqrt(eps_r) at fixed dx
+    assert np.all(e1 < bound), e1
+    ratio = e1 / e2
+    assert np.all(ratio > 3.0) and np.all(ratio < 5.0), (e1, e2, ratio)
+
+
+# ------------------------------------------------------------------------------------------------
+# Pin 2: discrete energy conservation in a lossless PEC box (signs, staggering, ring)
+# ------------------------------------------------------------------------------------------------
+def test_pin2_energy_conserved_lossless_pec_box():
+    wl = gi.small_random(nz=40, nx=46, nt=600, npml=0, nshots=1, nrec=1, lossy=False, seed=7)
+    w = wl.wavelet.astype(np.float64).copy()
+    nsrc_on = 380
+    w[nsrc_on:] = 0.0                              # source switched off after step nsrc_on - 1
+    pb = problem(wl, wavelet=w)
+    out = oracle.forward(pb, wl.eps_r, wl.sigma, want_h_hist=True)
+    ez, hx, hy = out["ez_hist"][0], out["hx_hist"][0], out["hy_hist"][0]
+    eps = EPS0 * wl.eps_r.astype(np.float64)
+    dx2 = wl.dx ** 2
+    ns = np.arange(nsrc_on + 1, wl.nt)             # hx[n] = Hx^{n-1/2}, hx[n+1] = Hx^{n+1/2}
+    W = np.array([0.5 * np.sum(eps * ez[n] ** 2) * dx2
+                  + 0.5 * MU0 * (np.sum(hx[n + 1] * hx[n]) + np.sum(hy[n + 1] * hy[n])) * dx2 for n in ns])
+    assert W[0] > 0
+    assert np.max(np.abs(W / W[0] - 1.0)) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# Pin 3: reciprocity (Cb source factor, collocated materials, H-located CPML tables)
+# ------------------------------------------------------------------------------------------------
+def test_pin3_reciprocity_heterogeneous_lossy_cpml():
+    wl = gi.small_random(nz=60, nx=70, nt=400, npml=10, nshots=1, nrec=1, seed=11)
+    a, b = (14, 17), (41, 55)                      # both interior, one close to the CPML
+    tr = []
+    for s, r in ((a, b), (b, a)):
+        pb = problem(wl, src_zx=np.array([s]), rec_zx=np.array([[r]]))
+        tr.append(oracle.forward(pb, wl.eps_r, wl.sigma)["traces"][0, :, 0])
+    assert np.linalg.norm(tr[0]) > 0
+    assert rel_l2(tr[0], tr[1]) < 1e-12
+
+
+
+# ------------------------------------------------------------------------------------------------
+# Pin 4: adjoint identity <J dm, y> = <dm, J^T y> with J dm from a complex step of the forward code
+# ------------------------------------------------------------------------------------------------
+def test_pin4_adjoint_identity_complex_step():
+    wl = gi.small_random(nz=44, nx=52, nt=160, npml=8, nshots=2, nrec=6, seed=21)
+    pb = problem(wl)
+    rng = np.random.default_rng(5)
+    de = rng.standard_normal((wl.nz, wl.nx))
+    ds = rng.standard_normal((wl.nz, wl.nx)) * 1e-2
+    y = rng.standard_normal((wl.nshots, wl.nt, wl.nrec))
+    h = 1e-30
+    trz = oracle.forward(pb, wl.eps_r + 1j * h * de, wl.sigma + 1j * h * ds)["traces"]
+    Jdm = trz.imag / h
+    ge, gs = oracle.gradient(pb, wl.eps_r, wl.sigma, y)
+    lhs = float(np.sum(Jdm * y))
+    rhs = float(np.sum(ge * de) + np.sum(gs * ds))
+    assert abs(lhs) > 0
+    assert abs(lhs - rhs) / abs(lhs) < 1e-10
+    # each parameter separately (a swapped chain-rule term would cancel only in the sum by accident)
+    Je = oracle.forward(pb, wl.eps_r + 1j * h * de, wl.sigma.astype(np.complex128))["traces"].imag / h
+    Js = oracle.forward(pb, wl.eps_r.astype(np.complex128), wl.sigma + 1j * h * ds)["traces"].imag / h
+    assert abs(np.sum(Je * y) - np.sum(ge * de)) / abs(np.sum(Je * y)) < 1e-10
+    assert abs(np.sum(Js * y) - np.sum(gs * ds)) / abs(np.sum(Js * y)) < 1e-10
+
+
+# ------------------------------------------------------------------------------------------------
+# Pin 5: central finite differences of the misfit (independent of complex arithmetic)
+# ------------------------------------------------------------------------------------------------
+def test_pin5_finite_differences_of_misfit():
+    wl = gi.small_random(nz=44, nx=52, nt=200, npml=8, nshots=1, nrec=6, seed=33)
+    pb = problem(wl)
+    eps = wl.eps_r.astype(np.float64)
+    sig = wl.sigma.astype(np.float64)
+    rng = np.random.default_rng(9)
+    d_obs = oracle.forward(pb, eps * (1 + 0.05 * rng.standard_normal(eps.shape)), sig * 1.1)["traces"]
+
+    def misfit(e, s):
+        return 0.5 * np.sum((oracle.forward(pb, e, s)["traces"] - d_obs) ** 2)
+
+    res = oracle.forward(pb, eps, sig)["traces"] - d_obs
+    ge, gs = oracle.gradient(pb, eps, sig, res)
+    sz, sx = map(int, wl.src_zx[0])
+    cells = [(20, 25), (sz, sx), (3, 30), (22, 2), (30, 40)]     # interior, source, CPML z, CPML x
+    for (j, i) in cells:
+        for which, g, h in (("eps", ge, 1e-4), ("sig", gs, 1e-6)):
+            ep, em, sp, sm = eps.copy(), eps.copy(), sig.copy(), sig.copy()
+            if which == "eps":
+                ep[j, i] += h; em[j, i] -= h
+            else:
+                sp[j, i] += h; sm[j, i] -= h
+            fd = (misfit(ep, sp) - misfit(em, sm)) / (2 * h)
+            assert abs(fd - g[j, i]) <= 2e-6 * max(abs(fd), np.max(np.abs(g)) * 1e-3), (j, i, which, fd, g[j, i])
+    # ring cells are never updated: gradient exactly zero there
+    for g in (ge, gs):
+        assert np.all(g[0, :] == 0) and np.all(g[-1, :] == 0) and np.all(g[:, 0] == 0) and np.all(g[:, -1] == 0)
+    # random direction
+    de = rng.standard_normal(eps.shape)
+    ds = rng.standard_normal(eps.shape) * 1e-3
+    h = 1e-5
+    fd = (misfit(eps + h * de, sig + h * ds) - misfit(eps - h * de, sig - h * ds)) / (2 * h)
+    an = np.sum(ge * de) + np.sum(gs * ds)
+    assert abs(fd - an) / abs(an) < 1e-7
+
+
+# ------------------------------------------------------------------------------------------------
+# Pin 6: special cases of the coefficient build and of the CPML tables
+# ------------------------------------------------------------------------------------------------
+def test_pin6_coefficients_special_cases():
+    dt = 2e-11
+    er = np.array([1.0, 4.0, 9.5, 20.0])
+    # sigma = 0: exactly Eq. (3)'s coefficients: 1 and dt/eps
+    ca, cb = oracle.coefficients(er, np.zeros(4), dt)
+    assert np.all(ca == 1.0)
+    np.testing.assert_allclose(cb, dt / (EPS0 * er), rtol=1e-15)
+    # lossy: Ca = (2 eps - sigma dt)/(2 eps + sigma dt), Cb = 2 dt/(2 eps + sigma dt)  (Taflove 3.31)
+    sg = np.array([1e-3, 5e-3, 2e-2, 30e-3])
+    ca, cb = oracle.coefficients(er, sg, dt)
+    e = EPS0 * er
+    np.testing.assert_allclose(ca, (2 * e - sg * dt) / (2 * e + sg * dt), rtol=1e-14)
+    np.testing.assert_allclose(cb, 2 * dt / (2 * e + sg * dt), rtol=1e-14)
+    # first-order agreement with Eq. (3)'s explicit form: Ca = 1 - sigma dt/eps + O((sigma dt/eps)^2)
+    x = sg * dt / e
+    assert np.all(np.abs(ca - (1 - x)) < x ** 2)
+    # sigma > 100 S/m: PEC
+    ca, cb = oracle.coefficients(np.array([4.0, 4.0]), np.array([100.0, 100.5]), dt)
+    assert ca[1] == 0 and cb[1] == 0 and ca[0] != 0 and cb[0] != 0
+
+
+def test_pin6_cpml_tables():
+    n, P, m, dt = 64, 10, 3, 2e-11
+    smax, kmax, amax = 5.0, 3.0, 0.02
+    b, c, ik = oracle.cpml_profile(n, P, m, smax, kmax, amax, dt, 0)
+    # interior and interface: trivial; symmetric; graded monotonically; ring has rho = 1
+    assert np.all(b[P:n - P] == 0) and np.all(c[P:n - P] == 0) and np.all(ik[P:n - P] == 1)
+    np.testing.assert_allclose(b, b[::-1], rtol=1e-14)
+    np.testing.assert_allclose(c, c[::-1], rtol=1e-14)
+    assert np.all(np.diff(ik[:P + 1]) > 0) and abs(ik[0] - 1 / kmax) < 1e-15
+    assert abs(b[0] - np.exp(-(smax / kmax) * dt / EPS0)) < 1e-15       # alpha(rho=1) = 0
+    assert np.all(c[:P] < 0) and np.all((b[:P] > 0) & (b[:P] < 1))
+    bh, ch, ikh = oracle.cpml_profile(n, P, m, smax, kmax, amax, dt, 1)
+    assert len(bh) == n - 1
+    np.testing.assert_allclose(bh, bh[::-1], rtol=1e-14)
+    assert np.all(bh[P:n - 1 - P] == 0) and bh[P - 1] > 0 and bh[n - 1 - P] > 0
+    rho = 0.5 / P                                                        # innermost H node
+    sp, kap, al = smax * rho ** m, 1 + (kmax - 1) * rho ** m, amax * (1 - rho)
+    assert abs(bh[P - 1] - np.exp(-(sp / kap + al) * dt / EPS0)) < 1e-15
+    assert abs(ch[P - 1] - sp * (bh[P - 1] - 1) / (kap * (sp + kap * al))) < 1e-18
+    # P = 0: all trivial
+    b0, c0, ik0 = oracle.cpml_profile(n, 0, m, smax, kmax, amax, dt, 0)
+    assert np.all(b0 == 0) and np.all(c0 == 0) and np.all(ik0 == 1)
+
+
+def test_pin6_npml0_matches_plain_numpy_yee():
+    """With no CPML the oracle must equal a psi-free vectorised Yee loop written directly from
+    Eqs. (3)-(5) in the Ca/Cb form."""
+    wl = gi.small_random(nz=30, nx=36, nt=150, npml=0, nshots=1, nrec=4, seed=3)
+    pb = problem(wl)
+    tr = oracle.forward(pb, wl.eps_r, wl.sigma)["traces"][0]
+    eps = EPS0 * wl.eps_r.astype(np.float64)
+    sg = wl.sigma.astype(np.float64)
+    dt, dx = wl.dt, wl.dx
+    ca = (2 * eps - sg * dt) / (2 * eps + sg * dt)
+    cb = 2 * dt / (2 * eps + sg * dt)
+    ez = np.zeros((wl.nz, wl.nx)); hx = np.zeros((wl.nz - 1, wl.nx)); hy = np.zeros((wl.nz, wl.nx - 1))
+    ref = np.zeros((wl.nt, wl.nrec))
+    sz, sx = wl.src_zx[0]
+    for n in range(wl.nt):
+        ref[n] = ez[wl.rec_zx[0, :, 0], wl.rec_zx[0, :, 1]]
+        hx -= dt / MU0 * (ez[1:, :] - ez[:-1, :]) / dx
+        hy += dt / MU0 * (ez[:, 1:] - ez[:, :-1]) / dx
+        ez[1:-1, 1:-1] = ca[1:-1, 1:-1] * ez[1:-1, 1:-1] + cb[1:-1, 1:-1] * (
+            (hy[1:-1, 1:] - hy[1:-1, :-1]) / dx - (hx[1:, 1:-1] - hx[:-1, 1:-1]) / dx)
+        ez[sz, sx] -= cb[sz, sx] * float(wl.wavelet[n]) / dx ** 2
+    assert np.linalg.norm(ref) > 0
+    assert rel_l2(tr, ref) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# Pin 7: CPML quality against a box so large that no reflection can return
+# ------------------------------------------------------------------------------------------------
+def test_pin7_cpml_vs_big_box():
+    wl = gi.config1(nt=500)
+    pb = problem(wl)
+    tr = oracle.forward(pb, wl.eps_r, wl.sigma)["traces"]
+    # slowest medium eps_r = 4 -> c/2; round trip to the new wall must exceed nt*dt
+    pad = int(np.ceil(0.5 * (C0 / 2.0) * wl.nt * wl.dt / wl.dx)) + 5
+    eps_b = np.pad(wl.eps_r, pad, mode="edge")
+    sig_b = np.pad(wl.sigma, pad, mode="edge")
+    pbb = problem(wl, nz=wl.nz + 2 * pad, nx=wl.nx + 2 * pad, npml=0, src_zx=wl.src_zx + pad,
+                  rec_zx=wl.rec_zx + pad)
+    trb = oracle.forward(pbb, eps_b, sig_b)["traces"]
+    err = rel_l2(tr, trb)
+    assert err < 5e-4, err            # a sign error in any psi gives growth or >> 1e-2
+    # without CPML the same small box reflects strongly: the layer is what makes the difference
+    tr0 = oracle.forward(problem(wl, npml=0), wl.eps_r, wl.sigma)["traces"]
+    assert rel_l2(tr0, trb) > 50 * err
+
+
+# ------------------------------------------------------------------------------------------------
+# Pin 8: linearity in the wavelet, shot independence, additivity of the gradient over shots
+# ------------------------------------------------------------------------------------------------
+def test_pin8_linearity_and_shot_independence():
+    wl = gi.small_random(nz=40, nx=48, nt=140, npml=8, nshots=3, nrec=5, seed=41)
+    rng = np.random.default_rng(2)
+    w1 = rng.standard_normal((3, wl.nt))
+    w2 = rng.standard_normal((3, wl.nt))
+    f = lambda w: oracle.forward(problem(wl, wavelet=w), wl.eps_r, wl.sigma)["traces"]
+    assert rel_l2(f(2.0 * w1 - 3.0 * w2), 2.0 * f(w1) - 3.0 * f(w2)) < 1e-13
+    full = f(w1)
+    res = rng.standard_normal(full.shape)
+    ge, gs = oracle.gradient(problem(wl, wavelet=w1), wl.eps_r, wl.sigma, res)
+    ge_sum = np.zeros_like(ge); gs_sum = np.zeros_like(gs)
+    for s in range(3):
+        pbs = problem(wl, wavelet=w1[s], src_zx=wl.src_zx[s:s + 1], rec_zx=wl.rec_zx[s:s + 1])
+        assert rel_l2(oracle.forward(pbs, wl.eps_r, wl.sigma)["traces"][0], full[s]) < 1e-15
+        a, b = oracle.gradient(pbs, wl.eps_r, wl.sigma, res[s:s + 1])
+        ge_sum += a; gs_sum += b
+    assert rel_l2(ge_sum, ge) < 1e-13 and rel_l2(gs_sum, gs) < 1e-13
+
+
+def test_pin8_coincident_receivers_sum():
+    wl = gi.small_random(nz=36, nx=40, nt=100, npml=6, nshots=1, nrec=3, seed=43)
+    rec = wl.rec_zx.copy()
+    rec[0, 2] = rec[0, 0]                           # receivers 0 and 2 on the same node
+    rng = np.random.default_rng(3)
+    res = rng.standard_normal((1, wl.nt, 3))
+    ge, gs = oracle.gradient(problem(wl, rec_zx=rec), wl.eps_r, wl.sigma, res)
+    res2 = res[:, :, :2].copy()
+    res2[:, :, 0] += res[:, :, 2]
+    ge2, gs2 = oracle.gradient(problem(wl, rec_zx=rec[:, :2]), wl.eps_r, wl.sigma, res2)
+    assert rel_l2(ge, ge2) < 1e-13 and rel_l2(gs, gs2) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# Pin 9: checkpoint-and-recompute == stored history
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("K", [1, 7, 50, 149, 150, 400])
+def test_pin9_checkpointed_gradient_equals_stored_history(K):
+    wl = gi.small_random(nz=40, nx=44, nt=150, npml=8, nshots=2, nrec=4, seed=51)
+    pb = problem(wl)
+    rng = np.random.default_rng(4)
+    res = rng.standard_normal((wl.nshots, wl.nt, wl.nrec))
+    ge0, gs0, tr0 = oracle.gradient(pb, wl.eps_r, wl.sigma, res, 0, want_traces=True)
+    ge, gs, tr = oracle.gradient(pb, wl.eps_r, wl.sigma, res, K, want_traces=True)
+    assert np.array_equal(tr, tr0)
+    assert rel_l2(ge, ge0) < 1e-14 and rel_l2(gs, gs0) < 1e-14
+    assert rel_l2(tr0, oracle.forward(pb, wl.eps_r, wl.sigma)["traces"]) == 0.0
+
+
+# ------------------------------------------------------------------------------------------------
+# argument checking
+# ------------------------------------------------------------------------------------------------
+def test_geometry_on_ring_rejected():
+    wl = gi.small_random(nz=30, nx=30, nt=10, npml=4, nshots=1, nrec=1)
+    with pytest.raises(ValueError):
+        oracle.forward(problem(wl, src_zx=np.array([[0, 5]])), wl.eps_r, wl.sigma)
+    with pytest.raises(ValueError):
+        oracle.forward(problem(wl, rec_zx=np.array([[[5, wl.nx - 1]]])), wl.eps_r, wl.sigma)
