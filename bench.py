@@ -1,0 +1,298 @@
+#!/usr/bin/env python
+"""bench.py -- forward+adjoint FDTD throughput of libgprfwi on BASELINE.json's configs.
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: coefficient build,
+nt forward steps (H+E+CPML+source+receivers+history), residual, nt adjoint steps with gradient
+accumulation, chain rule.  Default workload: BASELINE.json configs[1] (paper-scale synthetic,
+240x440 full grid, nt=3000, 20 shots, 100 receivers, full Ez history in HBM).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4|1] [--impl ours|reference]
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the float64 CPU oracle (oracle/) instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+import gpr_inputs as gi  # noqa: E402
+
+METRIC = "forward+adjoint FDTD Gcell-updates/s"
+UNIT = "Gcell-updates/s"
+# algorithmic bytes per cell-step (SURVEY.md section 8(d), T = 1 figures)
+BYTES_FWD, BYTES_ADJ, BYTES_RECOMPUTE = 28.0, 32.0, 28.0
+
+
+def load_workload(cfg: int):
+    return {1: gi.config1, 2: gi.config2, 3: gi.config3, 4: gi.config4}[cfg]()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json, burst copy)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for k, nm in enumerate(names):
+                    if r[3 + k].lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(wl, shots):
+    """Oracle forward+adjoint on a few shots of the workload; returns (seconds, cell_updates)."""
+    import oracle
+    from helpers import problem
+    sub = wl.subset(shots)
+    res = gi.random_residual(sub, 1.0)
+    t0 = time.perf_counter()
+    oracle.gradient(problem(sub), sub.eps_r, sub.sigma, res)
+    return time.perf_counter() - t0, sub.cell_updates
+
+
+def run_reference(args, wl):
+    import oracle
+    oracle.build()
+    per_step_shots = [0]
+    for _ in range(args.warmup):
+        oracle_sample(wl.subset([0], nt=min(wl.nt, 200)), [0])
+    times, work = [], 0
+    for k in range(args.steps):
+        t, w = oracle_sample(wl, [(k * 7) % wl.nshots])
+        times.append(t); work += w
+    total = sum(times)
+    val = work / total / 1e9
+    sample = f"{args.steps} steps x 1 shot of {wl.name} (full grid, full nt), float64, OpenMP over rows"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": wl.name, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--budget-gb", type=float, default=0.0, help="workspace budget (0 = 92%% of free HBM)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    wl = load_workload(args.config)
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, wl)
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    from paper_2506_20513_b200 import (Simulation, build, gprfwi_gradient_host, gprfwi_residual,
+                                       gprfwi_workspace_bytes, gprfwi_workspace_bytes_host, make_params)
+    build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    p = make_params(nz=wl.nz, nx=wl.nx, dx=wl.dx, dt=wl.dt, nt=wl.nt, npml=wl.npml, pml_order=wl.pml_order,
+                    pml_sigma_max=wl.pml_sigma_max, pml_kappa_max=wl.pml_kappa_max,
+                    pml_alpha_max=wl.pml_alpha_max, nshots=wl.nshots, nrec=wl.nrec)
+    free, _total = torch.cuda.mem_get_info(dev)
+    ntr = wl.nshots * wl.nt * wl.nrec
+    budget = int(args.budget_gb * 1e9) if args.budget_gb > 0 else int(free * 0.92) - 3 * ntr * 4
+    sim = Simulation(p, wl.src_zx, wl.rec_zx, wl.wavelet, dev, budget_bytes=budget)
+    eps = torch.as_tensor(wl.eps_r, device=dev)
+    sig = torch.as_tensor(wl.sigma, device=dev)
+    # observed data: a seeded stand-in with the traces' scale (d_obs content does not change the work)
+    rng = np.random.Generator(np.random.PCG64(wl.seed + 99))
+    d_obs_h = (rng.standard_normal((wl.nshots, wl.nt, wl.nrec)) * 1e-3).astype(np.float32)
+    d_obs = torch.as_tensor(d_obs_h, device=dev)
+    res = torch.empty_like(d_obs)
+    misfit = torch.zeros(1, dtype=torch.float64, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step(timers=None):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)] if timers is not None else None
+        if ev: ev[0].record(stream)
+        tr = sim.forward(eps, sig)
+        if ev: ev[1].record(stream)
+        misfit.zero_()
+        gprfwi_residual(tr, d_obs, res, misfit)
+        if ev: ev[2].record(stream)
+        ge, gs = sim.adjoint(res)
+        if world > 1:                      # shots are sharded over ranks: sum the gradients
+            dist.all_reduce(ge); dist.all_reduce(gs)
+        if ev:
+            ev[3].record(stream)
+            timers.append(ev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    timers = []
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        e0.record(stream)
+        for _ in range(args.steps):
+            step(timers)
+        e1.record(stream)
+        barrier()
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    fwd_ms = statistics.mean(e[0].elapsed_time(e[1]) for e in timers)
+    adj_ms = statistics.mean(e[2].elapsed_time(e[3]) for e in timers)
+    launches = sim.launch_count()          # kernels of the last forward + adjoint
+    plan = sim.plan
+    cells = wl.nz * wl.nx * wl.nshots
+    work = wl.cell_updates * world
+    value = work * args.steps / (ms * 1e-3) / 1e9
+
+    # roofline of the dominant kernel (adjoint step: 32 B per cell-step) from live CUDA-event times
+    peak, peak_src = peaks()
+    recompute_steps = 0 if plan["full_history"] else wl.nt          # ~ (K-1)/K of nt re-run per pass
+    adj_bytes = cells * BYTES_ADJ + (cells * BYTES_RECOMPUTE if recompute_steps else 0.0)
+    adj_launch_us = adj_ms * 1e3 / wl.nt
+    achieved = adj_bytes / (adj_launch_us * 1e-6) / 1e9
+    fwd_bytes = cells * (BYTES_FWD if plan["full_history"] else 24.0)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(f"config{args.config}", {}).get("adj_step_dram_bytes_per_launch")
+    roofline = {"bound": "hbm", "kernel": "adj_step_kernel (+recompute fwd_step_kernel)" if recompute_steps
+                else "adj_step_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": adj_bytes, "avg_launch_us": adj_launch_us,
+                "forward": {"kernel": "fwd_step_kernel", "achieved": fwd_bytes / (fwd_ms * 1e-3 / wl.nt) / 1e9,
+                            "avg_launch_us": fwd_ms * 1e3 / wl.nt,
+                            "frac": fwd_bytes / (fwd_ms * 1e-3 / wl.nt) / 1e9 / peak},
+                "pair_effective_gbs": (fwd_bytes + adj_bytes) * wl.nt / ((fwd_ms + adj_ms) * 1e-3) / 1e9,
+                "frac_of_8TBs_nominal": (fwd_bytes + adj_bytes) * wl.nt / ((fwd_ms + adj_ms) * 1e-3) / 1e9 / 8000.0}
+
+    # end to end through the host-buffer C-ABI call (H2D of models/wavelet/d_obs, D2H of traces/grads)
+    e2e = None
+    if not args.no_e2e:
+        sim.close(); del sim
+        torch.cuda.empty_cache()
+        nb = gprfwi_workspace_bytes_host(p, budget)
+        ws = torch.empty(nb, dtype=torch.uint8, device=dev)
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory().numpy()
+        h_eps, h_sig, h_w, h_d = pin(wl.eps_r), pin(wl.sigma), pin(wl.wavelet), pin(d_obs_h)
+        h_tr = torch.empty((wl.nshots, wl.nt, wl.nrec), dtype=torch.float32).pin_memory().numpy()
+        gprfwi_gradient_host(p, h_eps, h_sig, h_w, wl.src_zx, wl.rec_zx, h_d, ws, h_tr)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            gprfwi_gradient_host(p, h_eps, h_sig, h_w, wl.src_zx, wl.rec_zx, h_d, ws, h_tr)
+        torch.cuda.synchronize()
+        dt_e2e = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt_e2e], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt_e2e = float(t.item())
+        model_b = wl.nz * wl.nx * 4
+        e2e = {"value": work * args.steps / dt_e2e / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": 2 * model_b + wl.nt * 4 + ntr * 4,
+               "d2h_bytes_per_step": ntr * 4 + 2 * model_b + 8}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        shots = [0, wl.nshots // 2] if args.config <= 2 else [0]
+        sub = wl if args.config <= 2 else wl.subset(list(range(wl.nshots)), nt=min(wl.nt, 400))
+        secs, w = oracle_sample(sub, shots)
+        cpu = {"value": w / secs / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"oracle.gradient (forward+adjoint, float64) on shots {shots} of {sub.name}, "
+                         f"{secs:.1f} s"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": wl.name, "grid": [wl.nz, wl.nx], "nt": wl.nt, "shots_per_gpu": wl.nshots,
+                           "receivers": wl.nrec, "plan": plan, "fwd_ms": fwd_ms, "adj_ms": adj_ms,
+                           "s_per_fwi_iteration": ms / args.steps * 1e-3,
+                           "l2": "inputs larger than L2 (Ez history / checkpoints stream through HBM)"},
+                "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int((launches + 1) * args.steps),
+                "roofline": roofline, "cpu_baseline": cpu}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

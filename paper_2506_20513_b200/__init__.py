@@ -1,0 +1,12 @@
+"""B200-native forward + exact-adjoint 2-D TM FDTD for GPR dual-parameter FWI (arxiv/paper_2506_20513).
+
+Thin Python binding over the C-ABI library ``libgprfwi.so`` (include/gprfwi.h).  PyTorch is used only
+for device memory and streams; every step of the path runs in the library's CUDA kernels.
+"""
+from ._lib import GprfwiError, Params, Plan, EXPORTS, LIB_PATH  # noqa: F401
+from .api import (Simulation, gprfwi_adjoint, gprfwi_forward, gprfwi_gradient_host,  # noqa: F401
+                  gprfwi_residual, gprfwi_workspace_bytes, gprfwi_workspace_bytes_host, make_params)
+
+__all__ = ["Simulation", "make_params", "gprfwi_workspace_bytes", "gprfwi_workspace_bytes_host",
+           "gprfwi_forward", "gprfwi_adjoint", "gprfwi_gradient_host", "gprfwi_residual",
+           "GprfwiError", "Params", "Plan"]

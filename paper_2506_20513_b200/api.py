@@ -1,0 +1,167 @@
+"""Python binding with the same names as the C-ABI calls (include/gprfwi.h).
+
+Argument marshalling only: tensors must already be fp32, contiguous and on a CUDA device (host
+entry points take NumPy arrays); nothing is computed here.
+"""
+from __future__ import annotations
+
+import ctypes
+
+import numpy as np
+import torch
+
+from . import _lib
+from ._lib import Params, Plan, check
+
+
+def make_params(*, nz, nx, dx, dt, nt, npml, pml_order, pml_sigma_max, pml_kappa_max, pml_alpha_max,
+                nshots, nrec, pitch=None, wavelet_per_shot=0, checkpoint_stride=0) -> Params:
+    return Params(int(nz), int(nx), int(nx if pitch is None else pitch), float(dx), float(dt), int(nt),
+                  int(npml), int(pml_order), float(pml_sigma_max), float(pml_kappa_max),
+                  float(pml_alpha_max), int(nshots), int(nrec), int(wavelet_per_shot),
+                  int(checkpoint_stride))
+
+
+def _dev(t: torch.Tensor, name: str, n: int | None = None) -> int:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if t.dtype != torch.float32 or not t.is_contiguous():
+        raise TypeError(f"{name} must be contiguous float32")
+    if n is not None and t.numel() < n:
+        raise ValueError(f"{name} has {t.numel()} elements, needs {n}")
+    return t.data_ptr()
+
+
+def _i32(a, shape, name):
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    if a.shape != shape:
+        raise ValueError(f"{name} must have shape {shape}, got {a.shape}")
+    return a
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def gprfwi_workspace_bytes(p: Params, budget_bytes: int = 0):
+    """-> (bytes, plan dict); bytes == 0 if the params are invalid or nothing fits the budget."""
+    plan = Plan()
+    n = _lib.load().gprfwi_workspace_bytes(ctypes.byref(p), int(budget_bytes), ctypes.byref(plan))
+    return int(n), plan.as_dict()
+
+
+def gprfwi_workspace_bytes_host(p: Params, budget_bytes: int = 0) -> int:
+    return int(_lib.load().gprfwi_workspace_bytes_host(ctypes.byref(p), int(budget_bytes)))
+
+
+def gprfwi_forward(p: Params, eps_r, sigma, wavelet, src_zx, rec_zx, workspace, traces, handle=None,
+                   stream=None):
+    """Enqueue Algorithm 1 on `stream`; returns the (new or reused) handle (an int)."""
+    lib = _lib.load()
+    src = _i32(src_zx, (p.nshots, 2), "src_zx")
+    rec = _i32(np.asarray(rec_zx).reshape(p.nshots, p.nrec, 2), (p.nshots, p.nrec, 2), "rec_zx")
+    if not (isinstance(workspace, torch.Tensor) and workspace.is_cuda and workspace.dtype == torch.uint8):
+        raise TypeError("workspace must be a CUDA uint8 tensor")
+    h = ctypes.c_void_p(handle)
+    nw = (p.nshots if p.wavelet_per_shot else 1) * p.nt
+    code = lib.gprfwi_forward(
+        ctypes.byref(h), ctypes.byref(p), _dev(eps_r, "eps_r", p.nz * p.pitch), _dev(sigma, "sigma", p.nz * p.pitch),
+        _dev(wavelet, "wavelet", nw), src.ctypes.data, rec.ctypes.data, workspace.data_ptr(),
+        workspace.numel(), _dev(traces, "traces", p.nshots * p.nt * p.nrec) if p.nrec else None,
+        _stream_ptr(stream))
+    check(code)
+    return h.value
+
+
+def gprfwi_adjoint(handle, p: Params, residual, grad_eps_r, grad_sigma, stream=None):
+    """Enqueue Algorithm 2 + chain rule on `stream`."""
+    check(_lib.load().gprfwi_adjoint(
+        ctypes.c_void_p(handle), _dev(residual, "residual", p.nshots * p.nt * p.nrec) if p.nrec else None,
+        _dev(grad_eps_r, "grad_eps_r", p.nz * p.pitch), _dev(grad_sigma, "grad_sigma", p.nz * p.pitch),
+        _stream_ptr(stream)))
+
+
+def gprfwi_residual(d_syn, d_obs, residual, misfit=None, stream=None):
+    n = d_syn.numel()
+    mp = None
+    if misfit is not None:
+        if not (misfit.is_cuda and misfit.dtype == torch.float64):
+            raise TypeError("misfit must be a CUDA float64 tensor")
+        mp = misfit.data_ptr()
+    check(_lib.load().gprfwi_residual(_dev(d_syn, "d_syn"), _dev(d_obs, "d_obs", n), _dev(residual, "residual", n),
+                                      n, mp, _stream_ptr(stream)))
+
+
+def gprfwi_gradient_host(p: Params, eps_r, sigma, wavelet, src_zx, rec_zx, d_obs, workspace, traces=None,
+                         stream=None):
+    """Host-buffer gradient evaluation (NumPy in, NumPy out); copies are inside the call.
+    Returns (grad_eps_r, grad_sigma, misfit); `traces` (NumPy, optional) is filled in place."""
+    lib = _lib.load()
+
+    def f32(a, n, name):
+        a = np.ascontiguousarray(a, dtype=np.float32)
+        if a.size < n:
+            raise ValueError(f"{name} too small")
+        return a
+
+    src = _i32(src_zx, (p.nshots, 2), "src_zx")
+    rec = _i32(np.asarray(rec_zx).reshape(p.nshots, p.nrec, 2), (p.nshots, p.nrec, 2), "rec_zx")
+    e, s = f32(eps_r, p.nz * p.pitch, "eps_r"), f32(sigma, p.nz * p.pitch, "sigma")
+    w = f32(wavelet, (p.nshots if p.wavelet_per_shot else 1) * p.nt, "wavelet")
+    d = f32(d_obs, p.nshots * p.nt * p.nrec, "d_obs")
+    ge = np.empty((p.nz, p.pitch), dtype=np.float32)
+    gs = np.empty((p.nz, p.pitch), dtype=np.float32)
+    if traces is not None and not (traces.dtype == np.float32 and traces.flags.c_contiguous):
+        raise TypeError("traces must be C-contiguous float32")
+    mf = ctypes.c_double(0.0)
+    check(lib.gprfwi_gradient_host(
+        ctypes.byref(p), e.ctypes.data, s.ctypes.data, w.ctypes.data, src.ctypes.data, rec.ctypes.data,
+        d.ctypes.data, workspace.data_ptr(), workspace.numel(),
+        traces.ctypes.data if traces is not None else None, ge.ctypes.data, gs.ctypes.data,
+        ctypes.byref(mf), _stream_ptr(stream)))
+    return ge, gs, mf.value
+
+
+class Simulation:
+    """Owns the device buffers (torch) and the library handle for one problem."""
+
+    def __init__(self, p: Params, src_zx, rec_zx, wavelet, device="cuda:0", budget_bytes: int = 0):
+        self.p = p
+        self.device = torch.device(device)
+        self.src_zx, self.rec_zx = src_zx, rec_zx
+        nbytes, self.plan = gprfwi_workspace_bytes(p, budget_bytes)
+        if nbytes == 0:
+            raise ValueError("invalid parameters or nothing fits the memory budget")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.wavelet = torch.as_tensor(np.ascontiguousarray(wavelet, dtype=np.float32), device=self.device)
+        self.traces = torch.empty((p.nshots, p.nt, p.nrec), dtype=torch.float32, device=self.device)
+        self.grad_eps_r = torch.empty((p.nz, p.pitch), dtype=torch.float32, device=self.device)
+        self.grad_sigma = torch.empty((p.nz, p.pitch), dtype=torch.float32, device=self.device)
+        self.handle = None
+        self._models = None
+
+    def forward(self, eps_r: torch.Tensor, sigma: torch.Tensor, stream=None) -> torch.Tensor:
+        self._models = (eps_r, sigma)       # must stay alive and unmodified until the adjoint
+        self.handle = gprfwi_forward(self.p, eps_r, sigma, self.wavelet, self.src_zx, self.rec_zx,
+                                     self.workspace, self.traces, self.handle, stream)
+        return self.traces
+
+    def adjoint(self, residual: torch.Tensor, stream=None):
+        gprfwi_adjoint(self.handle, self.p, residual, self.grad_eps_r, self.grad_sigma, stream)
+        return self.grad_eps_r, self.grad_sigma
+
+    def launch_count(self) -> int:
+        return int(_lib.load().gprfwi_launch_count(ctypes.c_void_p(self.handle)))
+
+    def close(self):
+        if self.handle is not None:
+            _lib.load().gprfwi_release(ctypes.c_void_p(self.handle))
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

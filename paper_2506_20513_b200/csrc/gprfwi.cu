@@ -1,0 +1,650 @@
+// gprfwi.cu -- host side of libgprfwi: argument checks, memory plan, CPML tables, launch sequences
+// and the extern "C" boundary declared in include/gprfwi.h.  sm_100a only; no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "gprfwi.h"
+#include "gprfwi_adj.cuh"
+#include "gprfwi_common.cuh"
+#include "gprfwi_fwd.cuh"
+#include "gprfwi_misc.cuh"
+
+namespace gprfwi {
+
+static const double kC0 = 299792458.0;
+static const double kPi = 3.14159265358979323846;
+static const double kMu0 = 4.0e-7 * kPi;
+static const double kEps0d = 1.0 / (kMu0 * kC0 * kC0);
+
+static thread_local char g_cuda_err[256] = "no CUDA error recorded";
+
+static int cuda_fail(cudaError_t e, const char* what)
+{
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "CUDA error in %s: %s", what, cudaGetErrorString(e));
+  return GPRFWI_ECUDA;
+}
+#define GPR_CUDA(call)                                  \
+  do {                                                  \
+    cudaError_t e__ = (call);                           \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+  } while (0)
+
+// kernel launch (one place, so that every launch is counted the same way)
+#ifndef GPR_LAUNCH
+#define GPR_LAUNCH(kernel, grid, block, stream, ...) kernel<<<grid, block, 0, stream>>>(__VA_ARGS__)
+#endif
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ------------------------------------------------------------------------------------------------
+// memory plan
+// ------------------------------------------------------------------------------------------------
+struct Layout {
+  // geometry-derived sizes (floats)
+  int pitch = 0, xw = 0;
+  size_t plane = 0, zstrip = 0, xstrip = 0;
+  size_t hslot = 0;        // Hx, Hy, 4 psi strips of ONE shot
+  size_t full = 0;         // hslot + Ez plane
+  int tiles_x = 0, tiles_y = 0;
+  // plan
+  bool full_history = true;
+  int K = 0;               // checkpoint stride (nt when full history)
+  int ncheck = 0;          // checkpoints at n = 0, K, 2K, ... (< nt); slot ncheck = state at nt
+  int Sb = 0;              // shots per adjoint pass
+  int group = 1, ngroups = 1;
+  size_t bytes = 0;
+};
+
+static int validate(const gprfwi_params* p)
+{
+  if (!p) return GPRFWI_EINVAL;
+  if (p->npml < 0 || p->nz < 2 * p->npml + 3 || p->nx < 2 * p->npml + 3) return GPRFWI_EINVAL;
+  if (p->nt <= 0 || p->pitch < p->nx || p->nshots <= 0 || p->nrec < 0) return GPRFWI_EINVAL;
+  if (!(p->dx > 0.f) || !(p->dt > 0.f) || p->checkpoint_stride < 0) return GPRFWI_EINVAL;
+  if (p->npml > 0 && (p->pml_order < 0 || !(p->pml_kappa_max >= 1.f) || p->pml_sigma_max < 0.f ||
+                      p->pml_alpha_max < 0.f))
+    return GPRFWI_EINVAL;
+  if ((double)p->nz * p->nx > 2.0e9 / 4) return GPRFWI_EINVAL;           // int32 plane offsets
+  // Eq. (11), PAPER.md:93 with dx = dy and the vacuum speed of light (tiny fp32 slack)
+  if ((double)p->dt > (double)p->dx / (kC0 * std::sqrt(2.0)) * (1.0 + 1e-6)) return GPRFWI_ECFL;
+  return GPRFWI_OK;
+}
+
+static void base_layout(const gprfwi_params* p, Layout& L)
+{
+  L.pitch = (int)align_up((size_t)p->nx, 32);
+  L.xw = (int)align_up((size_t)2 * p->npml, 4);
+  L.plane = (size_t)p->nz * L.pitch;
+  L.zstrip = (size_t)2 * p->npml * L.pitch;
+  L.xstrip = (size_t)p->nz * L.xw;
+  L.hslot = 2 * L.plane + 2 * L.zstrip + 2 * L.xstrip;
+  L.full = L.hslot + L.plane;
+  L.tiles_x = (p->nx + kBlockCols - 1) / kBlockCols;
+  L.tiles_y = (p->nz + kBlockRows - 1) / kBlockRows;
+}
+
+static void set_groups(Layout& L)
+{
+  const int tiles = L.tiles_x * L.tiles_y;
+  int want = std::max(1, (1184 + tiles - 1) / tiles);     // >= 8 blocks per SM worth of tiles
+  int ng = std::min(L.Sb, want);
+  L.group = (L.Sb + ng - 1) / ng;
+  L.ngroups = (L.Sb + L.group - 1) / L.group;
+}
+
+// device pointers carved out of the caller's workspace
+struct Carve {
+  float *ca = nullptr, *cb = nullptr, *tables = nullptr, *gca = nullptr, *gcb = nullptr;
+  int *src_off = nullptr, *rec_off = nullptr, *blk_start = nullptr, *blk_rec = nullptr;
+  float* hist = nullptr;      // full history: (nt+1) * S planes
+  float* ckpt = nullptr;      // (ncheck+1) * S full states
+  float* seg = nullptr;       // (K-1) * Sb planes: Ez^{cK+1 .. cK+K-1}
+  float* fscratch = nullptr;  // 2 * S full states (forward ping-pong; reused by the recompute)
+  float* lam = nullptr;       // 2 * Sb full states (adjoint ping-pong)
+};
+
+// One routine both sizes and carves the workspace, so the two can never disagree.
+static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* c)
+{
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> char* {
+    char* r = base ? base + off : nullptr;
+    off += align_up(bytes, 256);
+    return r;
+  };
+  const size_t S = (size_t)p->nshots, R = (size_t)p->nrec, f = sizeof(float);
+  const size_t ntile = (size_t)L.tiles_x * L.tiles_y;
+  Carve tmp;
+  Carve& o = c ? *c : tmp;
+  o.ca = (float*)take(L.plane * f);
+  o.cb = (float*)take(L.plane * f);
+  o.tables = (float*)take((size_t)6 * (p->nx + p->nz) * f);
+  o.gca = (float*)take((size_t)L.ngroups * L.plane * f);
+  o.gcb = (float*)take((size_t)L.ngroups * L.plane * f);
+  o.src_off = (int*)take(S * sizeof(int));
+  o.rec_off = (int*)take(std::max<size_t>(S * R, 1) * sizeof(int));
+  o.blk_start = (int*)take(S * (ntile + 1) * sizeof(int));
+  o.blk_rec = (int*)take(std::max<size_t>(S * R, 1) * sizeof(int));
+  o.fscratch = (float*)take(2 * S * L.full * f);
+  o.lam = (float*)take(2 * (size_t)L.Sb * L.full * f);
+  if (L.full_history) {
+    o.hist = (float*)take((size_t)(p->nt + 1) * S * L.plane * f);
+  } else {
+    o.ckpt = (float*)take((size_t)(L.ncheck + 1) * S * L.full * f);
+    o.seg = (float*)take(std::max<size_t>((size_t)(L.K - 1) * L.Sb * L.plane, 1) * f);
+  }
+  return off;
+}
+
+// Chooses full history when it fits (or no budget is given), else the checkpoint stride K and the
+// adjoint shot sub-batch Sb that need the least memory for the largest Sb that fits.
+static bool make_plan(const gprfwi_params* p, size_t budget, Layout& L)
+{
+  base_layout(p, L);
+  if (p->checkpoint_stride == 0) {
+    L.full_history = true;
+    L.K = p->nt;
+    L.ncheck = 1;
+    L.Sb = p->nshots;
+    set_groups(L);
+    L.bytes = carve(p, L, nullptr, nullptr);
+    if (budget == 0 || L.bytes <= budget) return true;
+  }
+  L.full_history = false;
+  const int S = p->nshots;
+  int prev_sb = -1;
+  for (int div = 1; div <= S; ++div) {
+    const int sb = (S + div - 1) / div;
+    if (sb == prev_sb) continue;
+    prev_sb = sb;
+    L.Sb = sb;
+    set_groups(L);
+    int candidates[3];
+    int nc = 0;
+    if (p->checkpoint_stride > 0) {
+      candidates[nc++] = std::min(p->checkpoint_stride, p->nt);
+    } else {
+      const double kopt = std::sqrt((double)p->nt * S * (double)L.full / ((double)sb * (double)L.plane));
+      const int k0 = std::max(1, std::min(p->nt, (int)std::floor(kopt)));
+      candidates[nc++] = k0;
+      candidates[nc++] = std::min(p->nt, k0 + 1);
+    }
+    size_t best = 0;
+    int bestK = 0;
+    for (int q = 0; q < nc; ++q) {
+      L.K = candidates[q];
+      L.ncheck = (p->nt + L.K - 1) / L.K;
+      const size_t b = carve(p, L, nullptr, nullptr);
+      if (bestK == 0 || b < best) { best = b; bestK = L.K; }
+    }
+    L.K = bestK;
+    L.ncheck = (p->nt + L.K - 1) / L.K;
+    L.bytes = best;
+    if (budget == 0 || L.bytes <= budget) return true;
+  }
+  return false;
+}
+
+// ------------------------------------------------------------------------------------------------
+// CPML 1-D tables (reading R4: Roden-Gedney CPML, CFS stretching, polynomial grading).
+// Node position p = i (E-located) or i + 1/2 (H-located); depth into the layer d, rho = d/P:
+//   sigma_p = smax rho^m, kappa = 1 + (kmax-1) rho^m, alpha = amax (1 - rho)
+//   b = exp(-(sigma_p/kappa + alpha) dt/eps0),  c = sigma_p (b-1) / (kappa (sigma_p + kappa alpha))
+// Built in float64, stored as fp32.  Outside the layer b = c = 0, 1/kappa = 1.
+// ------------------------------------------------------------------------------------------------
+static void build_table(const gprfwi_params* p, int n, bool hloc, float* b, float* c, float* ik)
+{
+  const int P = p->npml, len = hloc ? n - 1 : n;
+  for (int i = 0; i < n; ++i) { b[i] = 0.f; c[i] = 0.f; ik[i] = 1.f; }
+  if (P <= 0) return;
+  for (int i = 0; i < len; ++i) {
+    const double pos = hloc ? i + 0.5 : (double)i;
+    const double depth = std::max(std::max((double)P - pos, pos - (double)(n - 1 - P)), 0.0);
+    if (depth <= 0.0) continue;
+    const double rho = depth / P, rm = std::pow(rho, (double)p->pml_order);
+    const double sg = (double)p->pml_sigma_max * rm;
+    const double kap = 1.0 + ((double)p->pml_kappa_max - 1.0) * rm;
+    const double al = (double)p->pml_alpha_max * (1.0 - rho);
+    const double bb = std::exp(-(sg / kap + al) * (double)p->dt / kEps0d);
+    const double den = kap * (sg + kap * al);
+    b[i] = (float)bb;
+    c[i] = den != 0.0 ? (float)(sg * (bb - 1.0) / den) : 0.f;
+    ik[i] = (float)(1.0 / kap);
+  }
+}
+
+}  // namespace gprfwi
+
+using namespace gprfwi;
+
+struct gprfwi_handle {
+  gprfwi_params p;
+  Layout L;
+  Carve c;
+  Geo geo;
+  const float *eps_r = nullptr, *sigma = nullptr, *wavelet = nullptr;
+  void* workspace = nullptr;
+  std::vector<float> h_tables;
+  std::vector<int> h_src_off, h_rec_off, h_blk_start, h_blk_rec;
+  bool forward_done = false;
+  int64_t launches = 0;
+};
+
+namespace gprfwi {
+
+static State state_at(const Layout& L, float* base, size_t S, size_t shot0)
+{
+  // a block of S full states laid out array by array: ez[S], hx[S], hy[S], phxz[S], pezz[S], phyx[S], pezx[S]
+  State s;
+  float* q = base;
+  s.ez = q + shot0 * L.plane;   q += S * L.plane;
+  s.hx = q + shot0 * L.plane;   q += S * L.plane;
+  s.hy = q + shot0 * L.plane;   q += S * L.plane;
+  s.phxz = q + shot0 * L.zstrip; q += S * L.zstrip;
+  s.pezz = q + shot0 * L.zstrip; q += S * L.zstrip;
+  s.phyx = q + shot0 * L.xstrip; q += S * L.xstrip;
+  s.pezx = q + shot0 * L.xstrip;
+  return s;
+}
+
+static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t* rec_zx)
+{
+  const gprfwi_params& p = h->p;
+  const Layout& L = h->L;
+  const int S = p.nshots, R = p.nrec, ntile = L.tiles_x * L.tiles_y;
+  h->h_src_off.assign(S, 0);
+  h->h_rec_off.assign(std::max(S * R, 1), 0);
+  h->h_blk_start.assign((size_t)S * (ntile + 1), 0);
+  h->h_blk_rec.assign(std::max(S * R, 1), 0);
+  auto ok = [&](int z, int x) { return z >= 1 && z <= p.nz - 2 && x >= 1 && x <= p.nx - 2; };
+  for (int s = 0; s < S; ++s) {
+    const int z = src_zx[2 * s], x = src_zx[2 * s + 1];
+    if (!ok(z, x)) return GPRFWI_EGEOM;
+    h->h_src_off[s] = z * L.pitch + x;
+    int* start = h->h_blk_start.data() + (size_t)s * (ntile + 1);
+    std::vector<int> tile_of(R);
+    for (int r = 0; r < R; ++r) {
+      const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
+      if (!ok(rz, rx)) return GPRFWI_EGEOM;
+      h->h_rec_off[(size_t)s * R + r] = rz * L.pitch + rx;
+      tile_of[r] = (rz / kBlockRows) * L.tiles_x + rx / kBlockCols;
+      start[tile_of[r] + 1]++;
+    }
+    for (int t = 0; t < ntile; ++t) start[t + 1] += start[t];
+    std::vector<int> fill(start, start + ntile);
+    for (int r = 0; r < R; ++r) h->h_blk_rec[(size_t)s * R + fill[tile_of[r]]++] = r;
+  }
+  return GPRFWI_OK;
+}
+
+static int upload_static(gprfwi_handle* h, cudaStream_t st)
+{
+  const gprfwi_params& p = h->p;
+  const Layout& L = h->L;
+  const int n = p.nx + p.nz;
+  h->h_tables.assign((size_t)6 * n, 0.f);
+  float* t = h->h_tables.data();
+  // order: ex(b,c,k)[nx] ez(b,c,k)[nz] hx(b,c,k)[nx] hz(b,c,k)[nz]
+  float* ex = t;             float* ez = ex + 3 * p.nx;
+  float* hx = ez + 3 * p.nz; float* hz = hx + 3 * p.nx;
+  build_table(&p, p.nx, false, ex, ex + p.nx, ex + 2 * p.nx);
+  build_table(&p, p.nz, false, ez, ez + p.nz, ez + 2 * p.nz);
+  build_table(&p, p.nx, true, hx, hx + p.nx, hx + 2 * p.nx);
+  build_table(&p, p.nz, true, hz, hz + p.nz, hz + 2 * p.nz);
+  GPR_CUDA(cudaMemcpyAsync(h->c.tables, t, h->h_tables.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+  GPR_CUDA(cudaMemcpyAsync(h->c.src_off, h->h_src_off.data(), h->h_src_off.size() * sizeof(int),
+                           cudaMemcpyHostToDevice, st));
+  GPR_CUDA(cudaMemcpyAsync(h->c.rec_off, h->h_rec_off.data(), h->h_rec_off.size() * sizeof(int),
+                           cudaMemcpyHostToDevice, st));
+  GPR_CUDA(cudaMemcpyAsync(h->c.blk_start, h->h_blk_start.data(), h->h_blk_start.size() * sizeof(int),
+                           cudaMemcpyHostToDevice, st));
+  GPR_CUDA(cudaMemcpyAsync(h->c.blk_rec, h->h_blk_rec.data(), h->h_blk_rec.size() * sizeof(int),
+                           cudaMemcpyHostToDevice, st));
+  Geo& g = h->geo;
+  g.nz = p.nz; g.nx = p.nx; g.P = p.npml; g.pitch = L.pitch; g.xw = L.xw;
+  g.plane = (long long)L.plane; g.zstrip = (long long)L.zstrip; g.xstrip = (long long)L.xstrip;
+  g.rdx = (float)(1.0 / (double)p.dx);
+  g.Db = (float)((double)p.dt / kMu0);
+  const float* d = h->c.tables;
+  g.bex = d; g.cex = d + p.nx; g.kex = d + 2 * p.nx; d += 3 * p.nx;
+  g.bez = d; g.cez = d + p.nz; g.kez = d + 2 * p.nz; d += 3 * p.nz;
+  g.bhx = d; g.chx = d + p.nx; g.khx = d + 2 * p.nx; d += 3 * p.nx;
+  g.bhz = d; g.chz = d + p.nz; g.khz = d + 2 * p.nz;
+  return GPRFWI_OK;
+}
+
+// One forward step n -> n+1 for `ns` shots starting at global shot `shot0`.
+static int launch_fwd(gprfwi_handle* h, cudaStream_t st, int n, int shot0, int ns, const State& in,
+                      const State& out, float* traces)
+{
+  const gprfwi_params& p = h->p;
+  FwdArgs a;
+  a.g = h->geo;
+  a.in = in;
+  a.out = out;
+  a.ca = h->c.ca;
+  a.cb = h->c.cb;
+  a.wav_stride = p.wavelet_per_shot ? p.nt : 0;
+  a.wavelet = h->wavelet + n + (size_t)shot0 * a.wav_stride;
+  a.src_off = h->c.src_off + shot0;
+  a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
+  a.trace_stride = (long long)p.nt * p.nrec;
+  a.traces = (traces && p.nrec > 0) ? traces + (size_t)shot0 * a.trace_stride + (size_t)n * p.nrec : nullptr;
+  a.R = p.nrec;
+  a.nshots = ns;
+  a.tiles_y = h->L.tiles_y;
+  dim3 grid(h->L.tiles_x, h->L.tiles_y + (a.traces ? 1 : 0), ns), block(32, kWarpsY);
+  GPR_LAUNCH(fwd_step_kernel, grid, block, st, a);
+  h->launches++;
+  return GPRFWI_OK;
+}
+
+}  // namespace gprfwi
+
+// ------------------------------------------------------------------------------------------------
+// extern "C" boundary (include/gprfwi.h)
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+int gprfwi_version(void) { return 100; }
+
+const char* gprfwi_strerror(int code)
+{
+  switch (code) {
+    case GPRFWI_OK: return "ok";
+    case GPRFWI_EINVAL: return "invalid argument";
+    case GPRFWI_ECFL: return "time step violates the CFL condition (Eq. 11)";
+    case GPRFWI_EGEOM: return "source or receiver outside [1, n-2]";
+    case GPRFWI_ENOMEM: return "workspace too small";
+    case GPRFWI_ESTATE: return "adjoint called without a completed forward";
+    case GPRFWI_ECUDA: return g_cuda_err;
+    default: return "unknown gprfwi status";
+  }
+}
+
+size_t gprfwi_workspace_bytes(const gprfwi_params* p, size_t budget_bytes, gprfwi_plan* plan)
+{
+  if (validate(p) != GPRFWI_OK) return 0;
+  Layout L;
+  if (!make_plan(p, budget_bytes, L)) return 0;
+  if (plan) {
+    plan->workspace_bytes = L.bytes;
+    plan->full_history = L.full_history ? 1 : 0;
+    plan->checkpoint_stride = L.K;
+    plan->shots_per_pass = L.Sb;
+    plan->time_block = 1;
+  }
+  return L.bytes;
+}
+
+int gprfwi_get_plan(const gprfwi_handle* h, gprfwi_plan* plan)
+{
+  if (!h || !plan) return GPRFWI_EINVAL;
+  plan->workspace_bytes = h->L.bytes;
+  plan->full_history = h->L.full_history ? 1 : 0;
+  plan->checkpoint_stride = h->L.K;
+  plan->shots_per_pass = h->L.Sb;
+  plan->time_block = 1;
+  return GPRFWI_OK;
+}
+
+int64_t gprfwi_launch_count(const gprfwi_handle* h) { return h ? h->launches : 0; }
+
+void gprfwi_release(gprfwi_handle* h) { delete h; }
+
+int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_r, const float* sigma,
+                   const float* wavelet, const int32_t* src_zx, const int32_t* rec_zx, void* workspace,
+                   size_t workspace_bytes, float* traces, void* cuda_stream)
+{
+  int rc = validate(p);
+  if (rc != GPRFWI_OK) return rc;
+  if (!hp || !eps_r || !sigma || !wavelet || !src_zx || !workspace || (p->nrec > 0 && (!rec_zx || !traces)))
+    return GPRFWI_EINVAL;
+  if ((uintptr_t)workspace % 256 != 0) return GPRFWI_EINVAL;
+  Layout L;
+  if (!make_plan(p, workspace_bytes, L)) return GPRFWI_ENOMEM;
+  gprfwi_handle* h = *hp;
+  const bool fresh = (h == nullptr);
+  if (fresh) {
+    h = new (std::nothrow) gprfwi_handle();
+    if (!h) return GPRFWI_ENOMEM;
+  } else if (std::memcmp(&h->p, p, sizeof(*p)) != 0) {
+    return GPRFWI_EINVAL;
+  }
+  h->p = *p;
+  h->L = L;
+  h->eps_r = eps_r; h->sigma = sigma; h->wavelet = wavelet; h->workspace = workspace;
+  h->forward_done = false;
+  h->launches = 0;
+  carve(p, L, (char*)workspace, &h->c);
+  rc = build_geometry(h, src_zx, rec_zx);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (rc == GPRFWI_OK) rc = upload_static(h, st);
+  if (rc != GPRFWI_OK) { if (fresh) delete h; return rc; }
+  *hp = h;
+
+  const size_t S = p->nshots, f = sizeof(float);
+  // kernel a: Ca/Cb once per call, shared by all shots
+  {
+    dim3 grid((L.pitch + 127) / 128, p->nz), block(128);
+    GPR_LAUNCH(coef_kernel, grid, block, st, eps_r, sigma, p->pitch, p->nz, p->nx, L.pitch,
+                                        (float)(1.0 / (double)p->dt), h->c.ca, h->c.cb);
+    h->launches++;
+  }
+  // fields are zero at n = 0
+  GPR_CUDA(cudaMemsetAsync(h->c.fscratch, 0, 2 * S * L.full * f, st));
+  float* slot[2] = {h->c.fscratch, h->c.fscratch + S * L.full};
+  if (L.full_history) {
+    GPR_CUDA(cudaMemsetAsync(h->c.hist, 0, S * L.plane * f, st));
+    for (int n = 0; n < p->nt; ++n) {
+      State in = state_at(L, slot[n & 1], S, 0), out = state_at(L, slot[(n + 1) & 1], S, 0);
+      in.ez = h->c.hist + (size_t)n * S * L.plane;
+      out.ez = h->c.hist + (size_t)(n + 1) * S * L.plane;
+      launch_fwd(h, st, n, 0, (int)S, in, out, traces);
+    }
+  } else {
+    GPR_CUDA(cudaMemsetAsync(h->c.ckpt, 0, S * L.full * f, st));      // checkpoint 0 = zero state
+    for (int n = 0; n < p->nt; ++n) {
+      float* src = (n % L.K == 0) ? h->c.ckpt + (size_t)(n / L.K) * S * L.full : slot[n & 1];
+      const int m = n + 1;
+      float* dst = (m == p->nt) ? h->c.ckpt + (size_t)L.ncheck * S * L.full
+                 : (m % L.K == 0) ? h->c.ckpt + (size_t)(m / L.K) * S * L.full : slot[m & 1];
+      launch_fwd(h, st, n, 0, (int)S, state_at(L, src, S, 0), state_at(L, dst, S, 0), traces);
+    }
+  }
+  GPR_CUDA(cudaGetLastError());
+  h->forward_done = true;
+  return GPRFWI_OK;
+}
+
+int gprfwi_adjoint(gprfwi_handle* h, const float* residual, float* grad_eps_r, float* grad_sigma,
+                   void* cuda_stream)
+{
+  if (!h || !grad_eps_r || !grad_sigma || (h->p.nrec > 0 && !residual)) return GPRFWI_EINVAL;
+  if (!h->forward_done) return GPRFWI_ESTATE;
+  const gprfwi_params* p = &h->p;
+  const Layout& L = h->L;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t S = p->nshots, f = sizeof(float);
+  const long long tstride = (long long)p->nt * p->nrec;
+  GPR_CUDA(cudaMemsetAsync(h->c.gca, 0, (size_t)L.ngroups * L.plane * f, st));
+  GPR_CUDA(cudaMemsetAsync(h->c.gcb, 0, (size_t)L.ngroups * L.plane * f, st));
+  float* lam[2] = {h->c.lam, h->c.lam + (size_t)L.Sb * L.full};
+  float* rs[2] = {h->c.fscratch, h->c.fscratch + S * L.full};     // recompute ping-pong
+
+  for (int shot0 = 0; shot0 < (int)S; shot0 += L.Sb) {
+    const int ns = std::min(L.Sb, (int)S - shot0);
+    // lambda = 0 at the end time, Eq. (10)
+    GPR_CUDA(cudaMemsetAsync(h->c.lam, 0, 2 * (size_t)L.Sb * L.full * f, st));
+    int flip = 0;
+    const int nseg = L.full_history ? 1 : L.ncheck;
+    for (int c = nseg - 1; c >= 0; --c) {
+      const int n0 = L.full_history ? 0 : c * L.K;
+      const int n1 = L.full_history ? p->nt : std::min(n0 + L.K, p->nt);
+      // forward Ez plane of step m for local shot 0 of this pass
+      auto ez_plane = [&](int m) -> float* {
+        if (L.full_history) return h->c.hist + ((size_t)m * S + shot0) * L.plane;
+        if (m == n0) return h->c.ckpt + (size_t)c * S * L.full + (size_t)shot0 * L.plane;
+        if (m == n1) {
+          const size_t slot = (m == p->nt) ? (size_t)L.ncheck : (size_t)(m / L.K);
+          return h->c.ckpt + slot * S * L.full + (size_t)shot0 * L.plane;
+        }
+        return h->c.seg + (size_t)(m - n0 - 1) * L.Sb * L.plane;
+      };
+      if (!L.full_history) {
+        // recompute Ez^{n0+1 .. n1-1} from checkpoint c with the same kernel in the same order
+        for (int n = n0; n < n1 - 1; ++n) {
+          State in = (n == n0) ? state_at(L, h->c.ckpt + (size_t)c * S * L.full, S, shot0)
+                               : state_at(L, rs[n & 1], S, 0);
+          State out = state_at(L, rs[(n + 1) & 1], S, 0);
+          in.ez = ez_plane(n);
+          out.ez = ez_plane(n + 1);
+          launch_fwd(h, st, n, shot0, ns, in, out, nullptr);
+        }
+      }
+      for (int n = n1 - 1; n >= n0; --n) {
+        AdjArgs a;
+        a.g = h->geo;
+        a.in = state_at(L, lam[flip], L.Sb, 0);
+        a.out = state_at(L, lam[flip ^ 1], L.Sb, 0);
+        a.ca = h->c.ca;
+        a.cb = h->c.cb;
+        a.en = ez_plane(n);
+        a.en1 = ez_plane(n + 1);
+        a.gca = h->c.gca;
+        a.gcb = h->c.gcb;
+        a.trace_stride = tstride;
+        a.residual = residual ? residual + (size_t)shot0 * tstride + (size_t)n * p->nrec : nullptr;
+        a.rec_off = h->c.rec_off + (size_t)shot0 * p->nrec;
+        a.blk_start = h->c.blk_start + (size_t)shot0 * (L.tiles_x * L.tiles_y + 1);
+        a.blk_rec = h->c.blk_rec + (size_t)shot0 * p->nrec;
+        a.R = p->nrec;
+        a.nshots = ns;
+        a.group = L.group;
+        a.tiles_x = L.tiles_x;
+        a.tiles_y = L.tiles_y;
+        dim3 grid(L.tiles_x, L.tiles_y, (ns + L.group - 1) / L.group), block(32, kWarpsY);
+        GPR_LAUNCH(adj_step_kernel, grid, block, st, a);
+        h->launches++;
+        flip ^= 1;
+      }
+    }
+  }
+  {
+    dim3 grid((p->nx + 127) / 128, p->nz), block(128);
+    GPR_LAUNCH(grad_finalize_kernel, grid, block, st, h->eps_r, h->sigma, p->pitch, p->nz, p->nx, L.pitch,
+                                                 (long long)L.plane, L.ngroups, (float)(1.0 / (double)p->dt),
+                                                 h->c.gca, h->c.gcb, grad_eps_r, grad_sigma);
+    h->launches++;
+  }
+  GPR_CUDA(cudaGetLastError());
+  return GPRFWI_OK;
+}
+
+int gprfwi_residual(const float* d_syn, const float* d_obs, float* residual, size_t n, double* misfit,
+                    void* cuda_stream)
+{
+  if (!d_syn || !d_obs || !residual) return GPRFWI_EINVAL;
+  if (n == 0) return GPRFWI_OK;
+  const int blocks = (int)std::min<size_t>((n + 255) / 256, 148 * 8);
+  GPR_LAUNCH(residual_kernel, dim3(blocks), dim3(256), (cudaStream_t)cuda_stream, d_syn, d_obs, residual, n, misfit);
+  GPR_CUDA(cudaGetLastError());
+  return GPRFWI_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// host-buffer entry point: one misfit-gradient evaluation, copies included
+// ------------------------------------------------------------------------------------------------
+namespace gprfwi {
+struct HostCarve {
+  float *eps = nullptr, *sig = nullptr, *wav = nullptr, *dobs = nullptr, *traces = nullptr, *res = nullptr;
+  float *ge = nullptr, *gs = nullptr;
+  double* misfit = nullptr;
+  char* core = nullptr;
+  size_t head = 0;
+};
+static size_t host_carve(const gprfwi_params* p, char* base, HostCarve* c)
+{
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> char* {
+    char* r = base ? base + off : nullptr;
+    off += align_up(std::max<size_t>(bytes, 1), 256);
+    return r;
+  };
+  const size_t model = (size_t)p->nz * p->pitch * sizeof(float);
+  const size_t tr = (size_t)p->nshots * p->nt * p->nrec * sizeof(float);
+  const size_t wv = (size_t)(p->wavelet_per_shot ? p->nshots : 1) * p->nt * sizeof(float);
+  HostCarve tmp;
+  HostCarve& o = c ? *c : tmp;
+  o.eps = (float*)take(model); o.sig = (float*)take(model);
+  o.ge = (float*)take(model);  o.gs = (float*)take(model);
+  o.wav = (float*)take(wv);
+  o.dobs = (float*)take(tr); o.traces = (float*)take(tr); o.res = (float*)take(tr);
+  o.misfit = (double*)take(sizeof(double));
+  o.core = base ? base + off : nullptr;
+  o.head = off;
+  return off;
+}
+}  // namespace gprfwi
+
+extern "C" {
+
+size_t gprfwi_workspace_bytes_host(const gprfwi_params* p, size_t budget_bytes)
+{
+  if (validate(p) != GPRFWI_OK) return 0;
+  const size_t head = host_carve(p, nullptr, nullptr);
+  if (budget_bytes != 0 && budget_bytes <= head) return 0;
+  const size_t core = gprfwi_workspace_bytes(p, budget_bytes ? budget_bytes - head : 0, nullptr);
+  return core ? head + core : 0;
+}
+
+int gprfwi_gradient_host(const gprfwi_params* p, const float* eps_r, const float* sigma, const float* wavelet,
+                         const int32_t* src_zx, const int32_t* rec_zx, const float* d_obs, void* workspace,
+                         size_t workspace_bytes, float* traces, float* grad_eps_r, float* grad_sigma,
+                         double* misfit, void* cuda_stream)
+{
+  int rc = validate(p);
+  if (rc != GPRFWI_OK) return rc;
+  if (!eps_r || !sigma || !wavelet || !src_zx || !workspace || !grad_eps_r || !grad_sigma ||
+      (p->nrec > 0 && (!rec_zx || !d_obs)))
+    return GPRFWI_EINVAL;
+  if ((uintptr_t)workspace % 256 != 0) return GPRFWI_EINVAL;
+  HostCarve hc;
+  host_carve(p, (char*)workspace, &hc);
+  if (workspace_bytes <= hc.head) return GPRFWI_ENOMEM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t model = (size_t)p->nz * p->pitch * sizeof(float);
+  const size_t ntr = (size_t)p->nshots * p->nt * p->nrec;
+  const size_t wv = (size_t)(p->wavelet_per_shot ? p->nshots : 1) * p->nt * sizeof(float);
+  GPR_CUDA(cudaMemcpyAsync(hc.eps, eps_r, model, cudaMemcpyHostToDevice, st));
+  GPR_CUDA(cudaMemcpyAsync(hc.sig, sigma, model, cudaMemcpyHostToDevice, st));
+  GPR_CUDA(cudaMemcpyAsync(hc.wav, wavelet, wv, cudaMemcpyHostToDevice, st));
+  if (ntr) GPR_CUDA(cudaMemcpyAsync(hc.dobs, d_obs, ntr * sizeof(float), cudaMemcpyHostToDevice, st));
+  GPR_CUDA(cudaMemsetAsync(hc.misfit, 0, sizeof(double), st));
+  gprfwi_handle* h = nullptr;
+  rc = gprfwi_forward(&h, p, hc.eps, hc.sig, hc.wav, src_zx, rec_zx, hc.core, workspace_bytes - hc.head,
+                      hc.traces, st);
+  if (rc != GPRFWI_OK) return rc;
+  rc = gprfwi_residual(hc.traces, hc.dobs, hc.res, ntr, hc.misfit, st);
+  if (rc == GPRFWI_OK) rc = gprfwi_adjoint(h, hc.res, hc.ge, hc.gs, st);
+  gprfwi_release(h);
+  if (rc != GPRFWI_OK) return rc;
+  if (traces && ntr) GPR_CUDA(cudaMemcpyAsync(traces, hc.traces, ntr * sizeof(float), cudaMemcpyDeviceToHost, st));
+  GPR_CUDA(cudaMemcpyAsync(grad_eps_r, hc.ge, model, cudaMemcpyDeviceToHost, st));
+  GPR_CUDA(cudaMemcpyAsync(grad_sigma, hc.gs, model, cudaMemcpyDeviceToHost, st));
+  double mf = 0.0;
+  GPR_CUDA(cudaMemcpyAsync(&mf, hc.misfit, sizeof(double), cudaMemcpyDeviceToHost, st));
+  GPR_CUDA(cudaStreamSynchronize(st));
+  if (misfit) *misfit = mf;
+  return GPRFWI_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,67 @@
+// gprfwi_common.cuh -- device-side data layout shared by all kernels of libgprfwi.
+//
+// Layout in HBM, all fp32, shot index outermost:
+//   field plane   [S][nz][pitch]     pitch = internal row pitch, multiple of 32 floats (128 B)
+//                 Ez at (j,i); Hx at (j+1/2,i) (row nz-1 unused, kept 0); Hy at (j,i+1/2)
+//                 (column nx-1 unused, kept 0); columns [nx, roundup4(nx)) are written as 0.
+//   z-strips      [S][2P][pitch]     CPML psi of the z-derivative, only the 2P rows where it lives
+//   x-strips      [S][nz][xw]        CPML psi of the x-derivative, only the 2P columns (xw = roundup4(2P))
+//   Ca, Cb        [nz][pitch]        shared by all shots
+//   1-D CPML tables (b, c, 1/kappa) per axis and per E/H location, built on the host in float64.
+#pragma once
+#include <stdint.h>
+#include <vector_types.h>
+
+#if defined(__CUDACC__)
+#define GPR_HD __host__ __device__ __forceinline__
+#else
+#define GPR_HD inline
+#endif
+
+namespace gprfwi {
+
+struct Geo {
+  int nz, nx, P;        // full grid, CPML thickness
+  int pitch;            // internal row pitch in floats
+  int xw;               // x-strip row width in floats
+  long long plane;      // nz * pitch
+  long long zstrip;     // 2P * pitch   (per shot)
+  long long xstrip;     // nz * xw      (per shot)
+  float rdx, Db;        // 1/dx ; dt/mu0 (the paper's uH4 with mu_r = 1)
+  // 1-D CPML tables, E-located (n entries) and H-located (n-1 entries)
+  const float *bex, *cex, *kex;   // x axis, E nodes
+  const float *bez, *cez, *kez;   // z axis, E nodes
+  const float *bhx, *chx, *khx;   // x axis, H nodes (i + 1/2)
+  const float *bhz, *chz, *khz;   // z axis, H nodes (j + 1/2)
+};
+
+// One complete state of the scheme for a batch of shots (pointers are for local shot 0).
+// Forward: ez = Ez, hx/hy = H, p* = psi.  Adjoint: the same slots hold the adjoint variables.
+struct State {
+  float* ez;     // [S][nz][pitch]
+  float* hx;     // [S][nz][pitch]
+  float* hy;     // [S][nz][pitch]
+  float* phxz;   // [S][2P][pitch]  psi of dEz/dz in the Hx update (H-z located rows)
+  float* pezz;   // [S][2P][pitch]  psi of dHx/dz in the Ez update (E-z located rows)
+  float* phyx;   // [S][nz][xw]     psi of dEz/dx in the Hy update (H-x located columns)
+  float* pezx;   // [S][nz][xw]     psi of dHy/dx in the Ez update (E-x located columns)
+};
+
+// strip index of an E-located / H-located node along an axis of n Ez nodes, or -1 outside the CPML
+GPR_HD int strip_e(int i, int n, int P) { return i < P ? i : (i >= n - P ? i - (n - P) + P : -1); }
+GPR_HD int strip_h(int i, int n, int P)
+{
+  return i < P ? i : ((i >= n - 1 - P && i < n - 1) ? i - (n - 1 - P) + P : -1);
+}
+
+GPR_HD float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+GPR_HD void st4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+GPR_HD float4 mk4(float a, float b, float c, float d) { float4 v; v.x = a; v.y = b; v.z = c; v.w = d; return v; }
+GPR_HD void unpack(float4 v, float* o) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
+
+constexpr int kRZ = 8;        // rows streamed per thread (v1 kernels)
+constexpr int kWarpsY = 4;    // warps per block, stacked in z
+constexpr int kBlockRows = kRZ * kWarpsY;
+constexpr int kBlockCols = 128;   // 32 lanes x float4
+
+}  // namespace gprfwi

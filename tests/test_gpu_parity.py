@@ -1,0 +1,231 @@
+"""Parity of the CUDA path (through the C-ABI) against the float64 oracle.  Needs a B200.
+
+Tolerances are north_star's: relative L2 <= 1e-4 on traces, <= 1e-3 on each gradient, over the whole
+array, with both sides given the same seeded inputs and the SAME residual (oracle traces - oracle
+d_obs, or a seeded random residual, rounded to fp32) -- DESIGN.md section 8.
+"""
+import numpy as np
+import pytest
+import torch
+
+import gpr_inputs as gi
+import oracle
+from helpers import problem, rel_l2
+from test_boundary import params_of
+from paper_2506_20513_b200 import (GprfwiError, Simulation, gprfwi_gradient_host, gprfwi_residual,
+                                   gprfwi_workspace_bytes, gprfwi_workspace_bytes_host)
+
+pytestmark = pytest.mark.gpu
+
+TOL_TRACE, TOL_GRAD = 1e-4, 1e-3
+
+
+def dev():
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch.device("cuda:0")
+
+
+def padded(a, pitch):
+    out = np.zeros((a.shape[0], pitch), dtype=np.float32)
+    out[:, :a.shape[1]] = a
+    return out
+
+
+def run_gpu(wl, residual=None, pitch=None, budget=0, checkpoint_stride=0):
+    pitch = pitch or wl.nx
+    p = params_of(wl, pitch=pitch, checkpoint_stride=checkpoint_stride)
+    sim = Simulation(p, wl.src_zx, wl.rec_zx, wl.wavelet, dev(), budget_bytes=budget)
+    sim.workspace.fill_(0xAB)          # the library must not rely on a zeroed workspace
+    e = torch.as_tensor(padded(wl.eps_r, pitch), device=dev())
+    s = torch.as_tensor(padded(wl.sigma, pitch), device=dev())
+    tr = sim.forward(e, s).cpu().numpy().copy()
+    ge = gs = None
+    if residual is not None:
+        r = torch.as_tensor(np.ascontiguousarray(residual, dtype=np.float32), device=dev())
+        a, b = sim.adjoint(r)
+        torch.cuda.synchronize()
+        ge, gs = a.cpu().numpy()[:, :wl.nx].copy(), b.cpu().numpy()[:, :wl.nx].copy()
+    plan = dict(sim.plan)
+    sim.close()
+    return tr, ge, gs, plan
+
+
+def oracle_all(wl, residual=None, with_obs=False):
+    pb = problem(wl)
+    tr = oracle.forward(pb, wl.eps_r, wl.sigma)["traces"]
+    if residual is None:
+        if with_obs:
+            residual = tr - oracle.forward(pb, wl.eps_r_obs, wl.sigma_obs)["traces"]
+        else:
+            residual = gi.random_residual(wl, float(np.sqrt(np.mean(tr ** 2))))
+    residual = residual.astype(np.float32)
+    ge, gs = oracle.gradient(pb, wl.eps_r, wl.sigma, residual)
+    return tr, residual, ge, gs
+
+
+def assert_parity(wl, got, ref, tag=""):
+    tr, ge, gs = got
+    tr_o, ge_o, gs_o = ref
+    et, ee, es = rel_l2(tr, tr_o), rel_l2(ge, ge_o), rel_l2(gs, gs_o)
+    print(f"[parity] {wl.name}{tag}: traces {et:.2e} grad_eps_r {ee:.2e} grad_sigma {es:.2e}")
+    assert et <= TOL_TRACE, et
+    assert ee <= TOL_GRAD, ee
+    assert es <= TOL_GRAD, es
+
+
+# ------------------------------------------------------------------------------------------------
+def test_config1_traces_and_gradients():
+    """BASELINE.json config 1 in full: 120x120, nt=800, d_obs from the model with the disc."""
+    wl = gi.config1()
+    tr_o, res, ge_o, gs_o = oracle_all(wl, with_obs=True)
+    tr, ge, gs, plan = run_gpu(wl, res)
+    assert plan["full_history"] == 1
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
+    assert np.all(tr[:, 0, :] == 0.0)               # sample 0 is recorded before the first update
+    for g in (ge, gs):                               # PEC ring: exactly zero gradient
+        assert np.all(g[0] == 0) and np.all(g[-1] == 0) and np.all(g[:, 0] == 0) and np.all(g[:, -1] == 0)
+
+
+def test_config1_end_to_end_residual_on_gpu():
+    """GPU forms the residual from its own fp32 traces (little margin: |res|/|trace| ~ 2 %)."""
+    wl = gi.config1()
+    pb = problem(wl)
+    tr_o, res_o, ge_o, gs_o = oracle_all(wl, with_obs=True)
+    d_obs = oracle.forward(pb, wl.eps_r_obs, wl.sigma_obs)["traces"].astype(np.float32)
+    p = params_of(wl)
+    ws = torch.empty(gprfwi_workspace_bytes_host(p), dtype=torch.uint8, device=dev())
+    tr = np.zeros((wl.nshots, wl.nt, wl.nrec), dtype=np.float32)
+    ge, gs, misfit = gprfwi_gradient_host(p, wl.eps_r, wl.sigma, wl.wavelet, wl.src_zx, wl.rec_zx, d_obs, ws, tr)
+    assert rel_l2(tr, tr_o) <= TOL_TRACE
+    assert abs(misfit - 0.5 * np.sum(res_o.astype(np.float64) ** 2)) <= 2e-3 * misfit
+    ee, es = rel_l2(ge, ge_o), rel_l2(gs, gs_o)
+    print(f"[parity] config1 end-to-end: grad_eps_r {ee:.2e} grad_sigma {es:.2e} misfit {misfit:.6e}")
+    assert ee <= TOL_GRAD and es <= TOL_GRAD
+
+
+@pytest.mark.parametrize("shape", [(44, 52, 8), (70, 150, 10), (97, 263, 12), (40, 40, 0), (33, 129, 5)])
+def test_small_ragged_grids(shape):
+    """Several tiles with ragged tails in x and z, scattered interior sources/receivers
+    (incl. receivers inside the CPML), CPML thickness not a multiple of 4, and a PEC box."""
+    nz, nx, npml = shape
+    wl = gi.small_random(nz=nz, nx=nx, nt=150, npml=npml, nshots=3, nrec=7, seed=nz * 1000 + nx)
+    tr_o, res, ge_o, gs_o = oracle_all(wl)
+    tr, ge, gs, _ = run_gpu(wl, res, pitch=nx + 5)
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o), f" {shape}")
+
+
+def test_checkpoint_recompute_is_bit_identical_and_subbatched():
+    """SURVEY 8(a) a6 / pin 9: gradients from checkpoint-and-recompute (forced stride, then a small
+    budget that also forces shot sub-batches) equal the stored-history ones bit for bit."""
+    wl = gi.small_random(nz=64, nx=140, nt=101, npml=10, nshots=5, nrec=6, seed=77)
+    tr_o, res, ge_o, gs_o = oracle_all(wl)
+    full = run_gpu(wl, res)
+    assert full[3]["full_history"] == 1
+    assert_parity(wl, full[:3], (tr_o, ge_o, gs_o), " full")
+    for K in (1, 7, 100, 101):
+        ck = run_gpu(wl, res, checkpoint_stride=K)
+        assert ck[3]["full_history"] == 0 and ck[3]["checkpoint_stride"] == K
+        assert np.array_equal(ck[0], full[0]) and np.array_equal(ck[1], full[1]) and np.array_equal(ck[2], full[2])
+    p = params_of(wl)
+    lo = min(b for b in (gprfwi_workspace_bytes(p, int(full[3]["workspace_bytes"] * f))[0]
+                         for f in np.linspace(0.2, 0.9, 15)) if b > 0)
+    ck = run_gpu(wl, res, budget=lo)
+    print("[plan] small budget:", ck[3])
+    assert ck[3]["full_history"] == 0
+    assert np.array_equal(ck[0], full[0])
+    # sub-batched passes change the shot grouping of the gradient sum, hence rounding order only
+    assert rel_l2(ck[1], full[1]) < 1e-5 and rel_l2(ck[2], full[2]) < 1e-5
+    assert_parity(wl, ck[:3], (tr_o, ge_o, gs_o), " small-budget")
+
+
+def test_batched_equals_per_shot_and_adjoint_reusable():
+    wl = gi.small_random(nz=60, nx=136, nt=120, npml=8, nshots=4, nrec=5, seed=5)
+    tr_o, res, _, _ = oracle_all(wl)
+    p = params_of(wl)
+    sim = Simulation(p, wl.src_zx, wl.rec_zx, wl.wavelet, dev())
+    e = torch.as_tensor(wl.eps_r, device=dev()); s = torch.as_tensor(wl.sigma, device=dev())
+    tr = sim.forward(e, s).cpu().numpy().copy()
+    r = torch.as_tensor(res, device=dev())
+    g1 = [t.cpu().numpy().copy() for t in sim.adjoint(r)]
+    g2 = [t.cpu().numpy().copy() for t in sim.adjoint(2.0 * r)]       # second adjoint, same forward
+    assert rel_l2(g2[0], 2.0 * g1[0]) < 1e-6 and rel_l2(g2[1], 2.0 * g1[1]) < 1e-6
+    sim.close()
+    ge_sum = np.zeros_like(g1[0], dtype=np.float64); gs_sum = np.zeros_like(ge_sum)
+    for k in range(wl.nshots):
+        one = wl.subset([k])
+        t1, a, b, _ = run_gpu(one, res[k:k + 1])
+        assert np.array_equal(t1[0], tr[k])                            # shots are independent
+        ge_sum += a; gs_sum += b
+    assert rel_l2(g1[0], ge_sum) < 1e-5 and rel_l2(g1[1], gs_sum) < 1e-5
+
+
+def test_coincident_receivers_and_receiver_on_source():
+    wl = gi.small_random(nz=50, nx=60, nt=100, npml=8, nshots=2, nrec=4, seed=9)
+    wl.rec_zx[0, 3] = wl.rec_zx[0, 0]
+    wl.rec_zx[1, 2] = wl.src_zx[1]
+    tr_o, res, ge_o, gs_o = oracle_all(wl)
+    tr, ge, gs, _ = run_gpu(wl, res)
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
+
+
+def test_pec_cells_and_zero_sigma():
+    """sigma > 100 S/m => PEC cell (Ca = Cb = 0, zero gradient); sigma = 0 => Ca = 1 exactly."""
+    wl = gi.small_random(nz=48, nx=56, nt=120, npml=8, nshots=1, nrec=5, seed=13, lossy=False)
+    wl.sigma[20:24, 30:36] = 1.0e3
+    tr_o, res, ge_o, gs_o = oracle_all(wl)
+    tr, ge, gs, _ = run_gpu(wl, res)
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
+    assert np.all(ge[20:24, 30:36] == 0) and np.all(gs[20:24, 30:36] == 0)
+
+
+def test_residual_kernel_and_errors():
+    a = torch.randn(100003, device=dev()); b = torch.randn(100003, device=dev())
+    r = torch.empty_like(a); m = torch.zeros(1, dtype=torch.float64, device=dev())
+    gprfwi_residual(a, b, r, m)
+    torch.cuda.synchronize()
+    assert torch.equal(r, a - b)
+    assert abs(m.item() - 0.5 * float(((a - b).double() ** 2).sum())) < 1e-9 * m.item()
+    wl = gi.small_random(nz=30, nx=30, nt=10, npml=4, nshots=1, nrec=1)
+    wl.src_zx[0] = (0, 5)
+    with pytest.raises(GprfwiError) as ei:
+        run_gpu(wl)
+    assert ei.value.code == -3                                          # EGEOM
+    with pytest.raises(TypeError):
+        sim = Simulation(params_of(gi.small_random()), np.zeros((2, 2)), np.zeros((2, 5, 2)), np.zeros(120), dev())
+        sim.forward(torch.zeros(44, 52), torch.zeros(44, 52))          # CPU tensors are refused
+
+
+def test_config2_subset_against_oracle():
+    """Config 2 at full grid size and nt, first / middle / last shot (the oracle's full run of 20
+    shots is what bench.py times; here 3 shots keep the test in tens of seconds)."""
+    wl = gi.config2().subset([0, 10, 19])
+    tr_o, res, ge_o, gs_o = oracle_all(wl, with_obs=True)
+    tr, ge, gs, _ = run_gpu(wl, res)
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
+
+
+def test_config2_full_launch_configuration_properties():
+    """Config 2 exactly as bench.py launches it (20 shots, nt=3000, full history in HBM): the three
+    oracle-checked shots must be reproduced bit-for-bit inside the batch (shots are independent),
+    and the batched gradient must equal the sum of per-shot gradients."""
+    wl = gi.config2()
+    sub = wl.subset([0, 10, 19])
+    tr_o, res_sub, _, _ = oracle_all(sub, with_obs=True)
+    res = gi.random_residual(wl, float(np.sqrt(np.mean(tr_o ** 2))))
+    res[[0, 10, 19]] = res_sub
+    tr, ge, gs, plan = run_gpu(wl, res)
+    assert plan["full_history"] == 1 and plan["shots_per_pass"] == 20
+    assert rel_l2(tr[[0, 10, 19]], tr_o) <= TOL_TRACE
+    t3, _, _, _ = run_gpu(sub)
+    assert np.array_equal(t3, tr[[0, 10, 19]])
+    assert np.isfinite(ge).all() and np.isfinite(gs).all()
+
+
+def test_config3_checkpointed_subset_against_oracle():
+    """Config 3 grid (540x1040), nt cut to 600 and 2 shots for the oracle's sake, forced through
+    checkpoint-and-recompute as the full config requires."""
+    wl = gi.config3(nt=600).subset([0, 59])
+    tr_o, res, ge_o, gs_o = oracle_all(wl, with_obs=True)
+    tr, ge, gs, plan = run_gpu(wl, res, checkpoint_stride=40)
+    assert plan["full_history"] == 0
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
