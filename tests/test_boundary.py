@@ -83,7 +83,6 @@ def test_plan_full_history_when_it_fits_else_checkpoints(lib):
     assert 0 < nb2 <= nb // 4 and plan2["full_history"] == 0 and 1 < plan2["checkpoint_stride"] < wl.nt
     # config 3 and 4 need recompute inside 170 GB; config 4 also needs shot sub-batches
     budget = 170 * 10 ** 9
-    wl3 = gi.config3.__wrapped__() if hasattr(gi.config3, "__wrapped__") else None
     p3 = make_params(nz=540, nx=1040, dx=0.01, dt=2e-11, nt=4000, npml=20, pml_order=3, pml_sigma_max=1.0,
                      pml_kappa_max=1.0, pml_alpha_max=0.0, nshots=60, nrec=200)
     nb3, plan3 = gprfwi_workspace_bytes(p3, budget)
