@@ -5,14 +5,17 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
 
 #include "gprfwi.h"
 #include "gprfwi_adj.cuh"
+#include "gprfwi_adj_tile.cuh"
 #include "gprfwi_common.cuh"
 #include "gprfwi_fwd.cuh"
+#include "gprfwi_fwd_tile.cuh"
 #include "gprfwi_misc.cuh"
 
 namespace gprfwi {
@@ -51,6 +54,10 @@ struct Layout {
   size_t plane = 0, zstrip = 0, xstrip = 0;
   size_t hslot = 0;        // Hx, Hy, 4 psi strips of ONE shot
   size_t full = 0;         // hslot + Ez plane
+  int T = 1;               // time steps fused per launch (1: v1 streaming kernels)
+  int tz = kBlockRows, tx = kBlockCols;   // tile owned by one CTA
+  int hz = 0, hx = 0;      // halo staged around it
+  int zcap = 0, xcap = 0;  // psi strip rows / columns staged per CTA (max over tiles)
   int tiles_x = 0, tiles_y = 0;
   // plan
   bool full_history = true;
@@ -85,14 +92,34 @@ static void base_layout(const gprfwi_params* p, Layout& L)
   L.xstrip = (size_t)p->nz * L.xw;
   L.hslot = 2 * L.plane + 2 * L.zstrip + 2 * L.xstrip;
   L.full = L.hslot + L.plane;
-  L.tiles_x = (p->nx + kBlockCols - 1) / kBlockCols;
-  L.tiles_y = (p->nz + kBlockRows - 1) / kBlockRows;
+  // time blocking: GPRFWI_TIME_BLOCK=1 selects the one-step-per-launch kernels (debug / comparison)
+  L.T = 4;
+  if (const char* e = std::getenv("GPRFWI_TIME_BLOCK")) L.T = std::max(1, std::min(4, std::atoi(e)));
+  if (L.T > 1) { L.tz = 32; L.tx = 64; L.hz = L.T; L.hx = 4; }
+  L.tiles_x = (p->nx + L.tx - 1) / L.tx;
+  L.tiles_y = (p->nz + L.tz - 1) / L.tz;
+  // strip rows / columns a region can hold: count of strip indices met by [lo, lo + len)
+  auto span = [&](int lo, int len, int n, bool hloc) {
+    int first = -1, last = -1;
+    for (int q = std::max(lo, 0); q < std::min(lo + len, n); ++q) {
+      const int sidx = hloc ? strip_h(q, n, p->npml) : strip_e(q, n, p->npml);
+      if (sidx >= 0) { if (first < 0) first = sidx; last = sidx; }
+    }
+    return first < 0 ? 0 : last - first + 1;
+  };
+  L.zcap = L.xcap = 0;
+  for (int t = 0; t < L.tiles_y; ++t)
+    for (int hl = 0; hl < 2; ++hl) L.zcap = std::max(L.zcap, span(t * L.tz - L.hz, L.tz + 2 * L.hz, p->nz, hl));
+  for (int t = 0; t < L.tiles_x; ++t)
+    for (int hl = 0; hl < 2; ++hl) L.xcap = std::max(L.xcap, span(t * L.tx - L.hx, L.tx + 2 * L.hx, p->nx, hl));
+  L.zcap = std::max(L.zcap, 1);
+  L.xcap = std::max(L.xcap, 1);
 }
 
 static void set_groups(Layout& L)
 {
   const int tiles = L.tiles_x * L.tiles_y;
-  int want = std::max(1, (1184 + tiles - 1) / tiles);     // >= 8 blocks per SM worth of tiles
+  int want = std::max(1, ((L.T > 1 ? 888 : 1184) + tiles - 1) / tiles);   // CTAs to fill 148 SMs a few times
   int ng = std::min(L.Sb, want);
   L.group = (L.Sb + ng - 1) / ng;
   L.ngroups = (L.Sb + L.group - 1) / L.group;
@@ -102,6 +129,7 @@ static void set_groups(Layout& L)
 struct Carve {
   float *ca = nullptr, *cb = nullptr, *tables = nullptr, *gca = nullptr, *gcb = nullptr;
   int *src_off = nullptr, *rec_off = nullptr, *blk_start = nullptr, *blk_rec = nullptr;
+  int *reg_start = nullptr, *reg_rec = nullptr;   // receivers by region (tile + halo), global CSR
   float* hist = nullptr;      // full history: (nt+1) * S planes
   float* ckpt = nullptr;      // (ncheck+1) * S full states
   float* seg = nullptr;       // (K-1) * Sb planes: Ez^{cK+1 .. cK+K-1}
@@ -131,6 +159,8 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
   o.rec_off = (int*)take(std::max<size_t>(S * R, 1) * sizeof(int));
   o.blk_start = (int*)take(S * (ntile + 1) * sizeof(int));
   o.blk_rec = (int*)take(std::max<size_t>(S * R, 1) * sizeof(int));
+  o.reg_start = (int*)take((S * ntile + 1) * sizeof(int));
+  o.reg_rec = (int*)take(std::max<size_t>(4 * S * R, 1) * sizeof(int));
   o.fscratch = (float*)take(2 * S * L.full * f);
   o.lam = (float*)take(2 * (size_t)L.Sb * L.full * f);
   if (L.full_history) {
@@ -171,9 +201,9 @@ static bool make_plan(const gprfwi_params* p, size_t budget, Layout& L)
       candidates[nc++] = std::min(p->checkpoint_stride, p->nt);
     } else {
       const double kopt = std::sqrt((double)p->nt * S * (double)L.full / ((double)sb * (double)L.plane));
-      const int k0 = std::max(1, std::min(p->nt, (int)std::floor(kopt)));
+      const int k0 = std::max(L.T, std::min(p->nt, (int)std::floor(kopt) / L.T * L.T));   // multiples of T
       candidates[nc++] = k0;
-      candidates[nc++] = std::min(p->nt, k0 + 1);
+      candidates[nc++] = std::min(p->nt, k0 + L.T);
     }
     size_t best = 0;
     int bestK = 0;
@@ -231,7 +261,7 @@ struct gprfwi_handle {
   const float *eps_r = nullptr, *sigma = nullptr, *wavelet = nullptr;
   void* workspace = nullptr;
   std::vector<float> h_tables;
-  std::vector<int> h_src_off, h_rec_off, h_blk_start, h_blk_rec;
+  std::vector<int> h_src_off, h_rec_off, h_blk_start, h_blk_rec, h_reg_start, h_reg_rec;
   bool forward_done = false;
   int64_t launches = 0;
 };
@@ -273,13 +303,29 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
       const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
       if (!ok(rz, rx)) return GPRFWI_EGEOM;
       h->h_rec_off[(size_t)s * R + r] = rz * L.pitch + rx;
-      tile_of[r] = (rz / kBlockRows) * L.tiles_x + rx / kBlockCols;
+      tile_of[r] = (rz / L.tz) * L.tiles_x + rx / L.tx;
       start[tile_of[r] + 1]++;
     }
     for (int t = 0; t < ntile; ++t) start[t + 1] += start[t];
     std::vector<int> fill(start, start + ntile);
     for (int r = 0; r < R; ++r) h->h_blk_rec[(size_t)s * R + fill[tile_of[r]]++] = r;
   }
+  // receivers by region: a receiver within the halo of a tile is injected there too
+  h->h_reg_start.assign((size_t)S * ntile + 1, 0);
+  h->h_reg_rec.clear();
+  for (int s = 0; s < S; ++s)
+    for (int ty = 0; ty < L.tiles_y; ++ty)
+      for (int tx = 0; tx < L.tiles_x; ++tx) {
+        const int z0 = ty * L.tz - L.hz, z1 = ty * L.tz + L.tz + L.hz;
+        const int x0 = tx * L.tx - L.hx, x1 = tx * L.tx + L.tx + L.hx;
+        for (int r = 0; r < R; ++r) {
+          const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
+          if (rz >= z0 && rz < z1 && rx >= x0 && rx < x1) h->h_reg_rec.push_back(r);
+        }
+        h->h_reg_start[(size_t)s * ntile + ty * L.tiles_x + tx + 1] = (int)h->h_reg_rec.size();
+      }
+  if (h->h_reg_rec.size() > (size_t)std::max(4 * S * R, 1)) return GPRFWI_EINVAL;
+  if (h->h_reg_rec.empty()) h->h_reg_rec.push_back(0);
   return GPRFWI_OK;
 }
 
@@ -305,6 +351,10 @@ static int upload_static(gprfwi_handle* h, cudaStream_t st)
   GPR_CUDA(cudaMemcpyAsync(h->c.blk_start, h->h_blk_start.data(), h->h_blk_start.size() * sizeof(int),
                            cudaMemcpyHostToDevice, st));
   GPR_CUDA(cudaMemcpyAsync(h->c.blk_rec, h->h_blk_rec.data(), h->h_blk_rec.size() * sizeof(int),
+                           cudaMemcpyHostToDevice, st));
+  GPR_CUDA(cudaMemcpyAsync(h->c.reg_start, h->h_reg_start.data(), h->h_reg_start.size() * sizeof(int),
+                           cudaMemcpyHostToDevice, st));
+  GPR_CUDA(cudaMemcpyAsync(h->c.reg_rec, h->h_reg_rec.data(), h->h_reg_rec.size() * sizeof(int),
                            cudaMemcpyHostToDevice, st));
   Geo& g = h->geo;
   g.nz = p.nz; g.nx = p.nx; g.P = p.npml; g.pitch = L.pitch; g.xw = L.xw;
@@ -345,6 +395,132 @@ static int launch_fwd(gprfwi_handle* h, cudaStream_t st, int n, int shot0, int n
   return GPRFWI_OK;
 }
 
+
+// ---- temporally blocked kernels: tile variants and their launchers ------------------------------
+#ifndef GPR_LAUNCH_SMEM
+#define GPR_LAUNCH_SMEM(kernel, grid, block, smem, stream, ...) kernel<<<grid, block, smem, stream>>>(__VA_ARGS__)
+#endif
+#define GPR_TILE_VARIANT 32, 64, 4
+using FwdTileV = FwdTile<GPR_TILE_VARIANT>;
+using AdjTileV = AdjTile<GPR_TILE_VARIANT>;
+
+static int tile_kernels_init(const Layout& L)
+{
+#if defined(__CUDACC__) && !defined(GPRFWI_EMU)
+  GPR_CUDA(cudaFuncSetAttribute(fwd_tile_kernel<GPR_TILE_VARIANT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)(FwdTileV::smem_floats(L.zcap, L.xcap) * sizeof(float))));
+  GPR_CUDA(cudaFuncSetAttribute(adj_tile_kernel<GPR_TILE_VARIANT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)(AdjTileV::smem_floats(L.zcap, L.xcap) * sizeof(float))));
+#endif
+  (void)L;
+  return GPRFWI_OK;
+}
+
+// Forward block: steps n .. n+nsub-1 for `ns` shots from global shot `shot0`.  ez_of(m) gives the
+// plane that must receive Ez^m (local shot 0) or NULL; in.ez / out.ez are already set by the caller.
+template <class EzOf>
+static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, int shot0, int ns,
+                            const State& in, const State& out, float* traces, EzOf ez_of)
+{
+  const gprfwi_params& p = h->p;
+  const Layout& L = h->L;
+  if (L.T == 1) return launch_fwd(h, st, n, shot0, ns, in, out, traces);
+  FwdTileArgs a;
+  a.g = h->geo;
+  a.in = in;
+  a.out = out;
+  a.ca = h->c.ca;
+  a.cb = h->c.cb;
+  for (int t = 0; t < kMaxT; ++t) a.ez_hist[t] = (t >= 1 && t < nsub) ? ez_of(n + t) : nullptr;
+  a.wav_stride = p.wavelet_per_shot ? p.nt : 0;
+  a.wavelet = h->wavelet + n + (size_t)shot0 * a.wav_stride;
+  a.src_off = h->c.src_off + shot0;
+  a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
+  a.blk_start = h->c.blk_start + (size_t)shot0 * (L.tiles_x * L.tiles_y + 1);
+  a.blk_rec = h->c.blk_rec + (size_t)shot0 * p.nrec;
+  a.trace_stride = (long long)p.nt * p.nrec;
+  a.traces = (traces && p.nrec > 0) ? traces + (size_t)shot0 * a.trace_stride + (size_t)n * p.nrec : nullptr;
+  a.R = p.nrec;
+  a.nsub = nsub;
+  a.tiles_x = L.tiles_x;
+  a.tiles_y = L.tiles_y;
+  a.zcap = L.zcap;
+  a.xcap = L.xcap;
+  dim3 grid(L.tiles_x, L.tiles_y, ns), block(kTileThreads);
+  GPR_LAUNCH_SMEM(fwd_tile_kernel<GPR_TILE_VARIANT>, grid, block,
+                  FwdTileV::smem_floats(L.zcap, L.xcap) * sizeof(float), st, a);
+  h->launches++;
+  return GPRFWI_OK;
+}
+
+// Adjoint block: reverse steps n_hi-1 .. n_hi-nsub for `ns` shots from global shot `shot0`.
+template <class EzOf>
+static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsub, int shot0, int ns,
+                            const State& in, const State& out, const float* residual, EzOf ez_of)
+{
+  const gprfwi_params& p = h->p;
+  const Layout& L = h->L;
+  const long long tstride = (long long)p.nt * p.nrec;
+  const int ngrp = (ns + L.group - 1) / L.group;
+  if (L.T == 1) {
+    const int n = n_hi - 1;
+    AdjArgs a;
+    a.g = h->geo;
+    a.in = in;
+    a.out = out;
+    a.ca = h->c.ca;
+    a.cb = h->c.cb;
+    a.en = ez_of(n);
+    a.en1 = ez_of(n + 1);
+    a.gca = h->c.gca;
+    a.gcb = h->c.gcb;
+    a.trace_stride = tstride;
+    a.residual = residual ? residual + (size_t)shot0 * tstride + (size_t)n * p.nrec : nullptr;
+    a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
+    a.blk_start = h->c.blk_start + (size_t)shot0 * (L.tiles_x * L.tiles_y + 1);
+    a.blk_rec = h->c.blk_rec + (size_t)shot0 * p.nrec;
+    a.R = p.nrec;
+    a.nshots = ns;
+    a.group = L.group;
+    a.tiles_x = L.tiles_x;
+    a.tiles_y = L.tiles_y;
+    dim3 grid(L.tiles_x, L.tiles_y, ngrp), block(32, kWarpsY);
+    GPR_LAUNCH(adj_step_kernel, grid, block, st, a);
+    h->launches++;
+    return GPRFWI_OK;
+  }
+  AdjTileArgs a;
+  a.g = h->geo;
+  a.in = in;
+  a.out = out;
+  a.ca = h->c.ca;
+  a.cb = h->c.cb;
+  for (int t = 0; t <= kMaxT; ++t) a.ez_planes[t] = t <= nsub ? ez_of(n_hi - t) : nullptr;
+  a.gca = h->c.gca;
+  a.gcb = h->c.gcb;
+  a.trace_stride = tstride;
+  a.residual = residual ? residual + (size_t)shot0 * tstride + (long long)n_hi * p.nrec : nullptr;
+  a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
+  a.reg_start = h->c.reg_start;
+  a.reg_rec = h->c.reg_rec;
+  a.R = p.nrec;
+  a.nsub = nsub;
+  a.n_hi = n_hi;
+  a.nt = p.nt;
+  a.nshots = ns;
+  a.group = L.group;
+  a.tiles_x = L.tiles_x;
+  a.tiles_y = L.tiles_y;
+  a.zcap = L.zcap;
+  a.xcap = L.xcap;
+  a.shot_base = shot0;
+  dim3 grid(L.tiles_x, L.tiles_y, ngrp), block(kTileThreads);
+  GPR_LAUNCH_SMEM(adj_tile_kernel<GPR_TILE_VARIANT>, grid, block,
+                  AdjTileV::smem_floats(L.zcap, L.xcap) * sizeof(float), st, a);
+  h->launches++;
+  return GPRFWI_OK;
+}
+
 }  // namespace gprfwi
 
 // ------------------------------------------------------------------------------------------------
@@ -378,7 +554,7 @@ size_t gprfwi_workspace_bytes(const gprfwi_params* p, size_t budget_bytes, gprfw
     plan->full_history = L.full_history ? 1 : 0;
     plan->checkpoint_stride = L.K;
     plan->shots_per_pass = L.Sb;
-    plan->time_block = 1;
+    plan->time_block = L.T;
   }
   return L.bytes;
 }
@@ -390,7 +566,7 @@ int gprfwi_get_plan(const gprfwi_handle* h, gprfwi_plan* plan)
   plan->full_history = h->L.full_history ? 1 : 0;
   plan->checkpoint_stride = h->L.K;
   plan->shots_per_pass = h->L.Sb;
-  plan->time_block = 1;
+  plan->time_block = h->L.T;
   return GPRFWI_OK;
 }
 
@@ -440,23 +616,31 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
   // fields are zero at n = 0
   GPR_CUDA(cudaMemsetAsync(h->c.fscratch, 0, 2 * S * L.full * f, st));
   float* slot[2] = {h->c.fscratch, h->c.fscratch + S * L.full};
-  if (L.full_history) {
-    GPR_CUDA(cudaMemsetAsync(h->c.hist, 0, S * L.plane * f, st));
-    for (int n = 0; n < p->nt; ++n) {
-      State in = state_at(L, slot[n & 1], S, 0), out = state_at(L, slot[(n + 1) & 1], S, 0);
+  rc = tile_kernels_init(L);
+  if (rc != GPRFWI_OK) return rc;
+  if (L.full_history) GPR_CUDA(cudaMemsetAsync(h->c.hist, 0, S * L.plane * f, st));
+  else GPR_CUDA(cudaMemsetAsync(h->c.ckpt, 0, S * L.full * f, st));       // checkpoint 0 = zero state
+  // blocks of up to T steps that never cross a checkpoint boundary
+  int idx = 0;
+  for (int n = 0; n < p->nt; ++idx) {
+    const int bound = L.full_history ? p->nt : std::min((n / L.K + 1) * L.K, p->nt);
+    const int nsub = std::min(L.T, bound - n), m = n + nsub;
+    State in, out;
+    if (L.full_history) {
+      in = state_at(L, slot[idx & 1], S, 0);
+      out = state_at(L, slot[(idx + 1) & 1], S, 0);
       in.ez = h->c.hist + (size_t)n * S * L.plane;
-      out.ez = h->c.hist + (size_t)(n + 1) * S * L.plane;
-      launch_fwd(h, st, n, 0, (int)S, in, out, traces);
-    }
-  } else {
-    GPR_CUDA(cudaMemsetAsync(h->c.ckpt, 0, S * L.full * f, st));      // checkpoint 0 = zero state
-    for (int n = 0; n < p->nt; ++n) {
-      float* src = (n % L.K == 0) ? h->c.ckpt + (size_t)(n / L.K) * S * L.full : slot[n & 1];
-      const int m = n + 1;
+      out.ez = h->c.hist + (size_t)m * S * L.plane;
+      launch_fwd_block(h, st, n, nsub, 0, (int)S, in, out, traces,
+                       [&](int q) { return h->c.hist + (size_t)q * S * L.plane; });
+    } else {
+      float* src = (n % L.K == 0) ? h->c.ckpt + (size_t)(n / L.K) * S * L.full : slot[idx & 1];
       float* dst = (m == p->nt) ? h->c.ckpt + (size_t)L.ncheck * S * L.full
-                 : (m % L.K == 0) ? h->c.ckpt + (size_t)(m / L.K) * S * L.full : slot[m & 1];
-      launch_fwd(h, st, n, 0, (int)S, state_at(L, src, S, 0), state_at(L, dst, S, 0), traces);
+                 : (m % L.K == 0) ? h->c.ckpt + (size_t)(m / L.K) * S * L.full : slot[(idx + 1) & 1];
+      launch_fwd_block(h, st, n, nsub, 0, (int)S, state_at(L, src, S, 0), state_at(L, dst, S, 0), traces,
+                       [](int) -> float* { return nullptr; });
     }
+    n = m;
   }
   GPR_CUDA(cudaGetLastError());
   h->forward_done = true;
@@ -498,41 +682,25 @@ int gprfwi_adjoint(gprfwi_handle* h, const float* residual, float* grad_eps_r, f
         return h->c.seg + (size_t)(m - n0 - 1) * L.Sb * L.plane;
       };
       if (!L.full_history) {
-        // recompute Ez^{n0+1 .. n1-1} from checkpoint c with the same kernel in the same order
-        for (int n = n0; n < n1 - 1; ++n) {
+        // recompute Ez^{n0+1 .. n1-1} from checkpoint c with the same kernel (Ez^{n1} is a checkpoint)
+        int idx = 0;
+        for (int n = n0; n < n1 - 1; ++idx) {
+          const int nsub = std::min(L.T, n1 - 1 - n);
           State in = (n == n0) ? state_at(L, h->c.ckpt + (size_t)c * S * L.full, S, shot0)
-                               : state_at(L, rs[n & 1], S, 0);
-          State out = state_at(L, rs[(n + 1) & 1], S, 0);
+                               : state_at(L, rs[idx & 1], S, 0);
+          State out = state_at(L, rs[(idx + 1) & 1], S, 0);
           in.ez = ez_plane(n);
-          out.ez = ez_plane(n + 1);
-          launch_fwd(h, st, n, shot0, ns, in, out, nullptr);
+          out.ez = ez_plane(n + nsub);
+          launch_fwd_block(h, st, n, nsub, shot0, ns, in, out, nullptr, ez_plane);
+          n += nsub;
         }
       }
-      for (int n = n1 - 1; n >= n0; --n) {
-        AdjArgs a;
-        a.g = h->geo;
-        a.in = state_at(L, lam[flip], L.Sb, 0);
-        a.out = state_at(L, lam[flip ^ 1], L.Sb, 0);
-        a.ca = h->c.ca;
-        a.cb = h->c.cb;
-        a.en = ez_plane(n);
-        a.en1 = ez_plane(n + 1);
-        a.gca = h->c.gca;
-        a.gcb = h->c.gcb;
-        a.trace_stride = tstride;
-        a.residual = residual ? residual + (size_t)shot0 * tstride + (size_t)n * p->nrec : nullptr;
-        a.rec_off = h->c.rec_off + (size_t)shot0 * p->nrec;
-        a.blk_start = h->c.blk_start + (size_t)shot0 * (L.tiles_x * L.tiles_y + 1);
-        a.blk_rec = h->c.blk_rec + (size_t)shot0 * p->nrec;
-        a.R = p->nrec;
-        a.nshots = ns;
-        a.group = L.group;
-        a.tiles_x = L.tiles_x;
-        a.tiles_y = L.tiles_y;
-        dim3 grid(L.tiles_x, L.tiles_y, (ns + L.group - 1) / L.group), block(32, kWarpsY);
-        GPR_LAUNCH(adj_step_kernel, grid, block, st, a);
-        h->launches++;
+      for (int n_hi = n1; n_hi > n0;) {
+        const int nsub = std::min(L.T, n_hi - n0);
+        launch_adj_block(h, st, n_hi, nsub, shot0, ns, state_at(L, lam[flip], L.Sb, 0),
+                         state_at(L, lam[flip ^ 1], L.Sb, 0), residual, ez_plane);
         flip ^= 1;
+        n_hi -= nsub;
       }
     }
   }

@@ -48,7 +48,7 @@ struct State {
 };
 
 // strip index of an E-located / H-located node along an axis of n Ez nodes, or -1 outside the CPML
-GPR_HD int strip_e(int i, int n, int P) { return i < P ? i : (i >= n - P ? i - (n - P) + P : -1); }
+GPR_HD int strip_e(int i, int n, int P) { return i < P ? i : ((i >= n - P && i < n) ? i - (n - P) + P : -1); }
 GPR_HD int strip_h(int i, int n, int P)
 {
   return i < P ? i : ((i >= n - 1 - P && i < n - 1) ? i - (n - 1 - P) + P : -1);
