@@ -42,8 +42,16 @@ template <int TZ, int TX, int T>
 struct AdjTile {
   using F = FwdTile<TZ, TX, T>;
   static constexpr int RH = F::RH, RW = F::RW, RW4 = F::RW4, NU = F::NU, KU = F::KU;
-  struct Regs { float ca[KU][4], ga[KU][4], gb[KU][4], e1[KU][4]; };
-  struct Smem { float *le, *hx, *hy, *cb, *pzh, *pze, *pxh, *pxe, *tz, *tx; };
+  // per-thread state: Ca, masked Cb (0 on the PEC ring) of the thread's cells, gradient partial
+  // sums, the carried forward plane E^{n+1}, and per unit the smem / global offsets and class mask
+  // (bit 0 in grid; 1 phase-B fast; 2 phase-C fast; 3 owned; 4 has H-CPML cells -> lazy psiH).
+  struct Regs {
+    float ca[KU][4], cb[KU][4], ga[KU][4], gb[KU][4], e1[KU][4];
+    int off[KU], goff[KU];
+    unsigned fl[KU];
+  };
+  static constexpr unsigned kIn = 1u, kBFast = 2u, kCFast = 4u, kOwn = 8u, kLazy = 16u;
+  struct Smem { float *le, *q, *hx, *hy, *pzh, *pze, *pxh, *pxe, *tz, *tx; };
   GPR_HD static size_t smem_floats(int zcap, int xcap)
   {
     return (size_t)4 * RH * RW + (size_t)2 * zcap * RW + (size_t)2 * RH * xcap + 6 * RH + 6 * RW;
@@ -56,8 +64,8 @@ struct AdjTile {
   {
     Ctx c;
     Smem& m = c.m;
-    m.le = base; m.hx = m.le + RH * RW; m.hy = m.hx + RH * RW; m.cb = m.hy + RH * RW;
-    m.pzh = m.cb + RH * RW; m.pze = m.pzh + a.zcap * RW;
+    m.le = base; m.q = m.le + RH * RW; m.hx = m.q + RH * RW; m.hy = m.hx + RH * RW;
+    m.pzh = m.hy + RH * RW; m.pze = m.pzh + a.zcap * RW;
     m.pxh = m.pze + a.zcap * RW; m.pxe = m.pxh + RH * a.xcap;
     m.tz = m.pxe + RH * a.xcap; m.tx = m.tz + 6 * RH;
     c.s = 0; c.gj0 = ty * TZ - T; c.gi0 = tx * TX - 4;
@@ -67,9 +75,8 @@ struct AdjTile {
     c.xmin_h = F::strip_min(c.gi0, a.g.nx, a.g.P, true);
     return c;
   }
-  GPR_HD static bool owned(int r, int lc) { return r >= T && r < T + TZ && lc >= 4 && lc < 4 + TX; }
 
-  // once per CTA: tables, Cb region, Ca registers, zeroed accumulators
+  // once per CTA: tables, Ca / masked Cb registers, unit classes, zeroed accumulators
   GPR_HD static void setup(const AdjTileArgs& a, const Ctx& c, int tid, Regs& rg)
   {
     const Geo& g = a.g;
@@ -92,25 +99,42 @@ struct AdjTile {
     for (int k = 0; k < KU; ++k) {
       const int u = tid + k * kTileThreads;
 #pragma unroll
-      for (int q = 0; q < 4; ++q) rg.ca[k][q] = rg.ga[k][q] = rg.gb[k][q] = rg.e1[k][q] = 0.f;
+      for (int q = 0; q < 4; ++q) rg.ca[k][q] = rg.cb[k][q] = rg.ga[k][q] = rg.gb[k][q] = rg.e1[k][q] = 0.f;
+      rg.off[k] = 0; rg.goff[k] = 0; rg.fl[k] = 0u;
       if (u >= NU) continue;
       const int r = u / RW4, lc = (u % RW4) * 4;
       const int gj = c.gj0 + r, gi = c.gi0 + lc;
-      float4 cb = mk4(0, 0, 0, 0);
-      if (gj >= 1 && gj <= g.nz - 2 && gi >= 0 && gi < g.nx) {      // Cb = 0 on ring rows: q = 0 there
-        cb = ld4(a.cb + (long long)gj * g.pitch + gi);
-        unpack(ld4(a.ca + (long long)gj * g.pitch + gi), rg.ca[k]);
-        if (gi == 0) cb.x = 0.f;                                    // ring columns
-        if (gi + 0 == g.nx - 1) cb.x = 0.f;
-        if (gi + 1 >= g.nx - 1) cb.y = 0.f;
-        if (gi + 2 >= g.nx - 1) cb.z = 0.f;
-        if (gi + 3 >= g.nx - 1) cb.w = 0.f;
+      if (!(gj >= 0 && gj < g.nz && gi >= 0 && gi < g.nx)) continue;
+      rg.off[k] = r * RW + lc;
+      rg.goff[k] = gj * g.pitch + gi;
+      if (gj >= 1 && gj <= g.nz - 2) {                   // Cb = 0 on the PEC ring: q = 0 there
+        unpack(ld4(a.cb + rg.goff[k]), rg.cb[k]);
+        unpack(ld4(a.ca + rg.goff[k]), rg.ca[k]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          if (gi + q < 1 || gi + q > g.nx - 2) rg.cb[k][q] = 0.f;
       }
-      st4(m.cb + r * RW + lc, cb);
+      const int P = g.P;
+      const bool noze0 = strip_e(gj, g.nz, P) < 0, noze1 = strip_e(gj + 1, g.nz, P) < 0;
+      const bool nozh0 = strip_h(gj, g.nz, P) < 0, nozhm = strip_h(gj - 1, g.nz, P) < 0;
+      const bool noxe4 = gi >= P && gi + 3 < g.nx - P;            // E-located columns gi..gi+3
+      const bool noxe5 = gi >= P && gi + 4 < g.nx - P;            // gi..gi+4
+      const bool noxh4 = gi >= P && gi + 3 < g.nx - 1 - P;        // H-located columns gi..gi+3
+      const bool noxh5 = gi - 1 >= P && gi + 3 < g.nx - 1 - P;    // gi-1..gi+3
+      unsigned f = kIn;
+      if (!(nozh0 && noxh4)) f |= kLazy;
+      if (r + 1 < RH && gj <= g.nz - 2 && lc + 4 < RW && gi + 3 <= g.nx - 2 && noze0 && noze1 && noxe5 &&
+          nozh0 && noxh4)
+        f |= kBFast;
+      if (r >= 1 && r <= RH - 2 && gj >= 1 && gj <= g.nz - 2 && lc >= 4 && lc + 3 <= RW - 2 && gi >= 1 &&
+          gi + 3 <= g.nx - 2 && noze0 && noxe4 && nozh0 && nozhm && noxh5)
+        f |= kCFast;
+      if (r >= T && r < T + TZ && lc >= 4 && lc < 4 + TX) f |= kOwn;
+      rg.fl[k] = f;
     }
   }
 
-  // per shot: stage the adjoint state of the region; first history plane into registers
+  // per shot: stage the adjoint state of the region, q = Cb*lamE; first history plane to registers
   GPR_HD static void load(const AdjTileArgs& a, const Ctx& c, int tid, Regs& rg)
   {
     const Geo& g = a.g;
@@ -120,29 +144,31 @@ struct AdjTile {
       const int u = tid + k * kTileThreads;
       if (u >= NU) continue;
       const int r = u / RW4, lc = (u % RW4) * 4;
-      const int gj = c.gj0 + r, gi = c.gi0 + lc;
-      const bool in = gj >= 0 && gj < g.nz && gi >= 0 && gi < g.nx;
       float4 e = mk4(0, 0, 0, 0), hx = e, hy = e;
-      if (in) {
-        const long long o = c.s * g.plane + (long long)gj * g.pitch + gi;
+      if (rg.fl[k] & kIn) {
+        const int gj = c.gj0 + r, gi = c.gi0 + lc;
+        const long long o = c.s * g.plane + rg.goff[k];
         e = ld4(a.in.ez + o); hx = ld4(a.in.hx + o); hy = ld4(a.in.hy + o);
         const int zh = strip_h(gj, g.nz, g.P), ze = strip_e(gj, g.nz, g.P);
         if (zh >= 0) st4(m.pzh + (zh - c.zmin_h) * RW + lc, ld4(a.in.phxz + c.s * g.zstrip + (long long)zh * g.pitch + gi));
         if (ze >= 0) st4(m.pze + (ze - c.zmin_e) * RW + lc, ld4(a.in.pezz + c.s * g.zstrip + (long long)ze * g.pitch + gi));
+        if (gi < g.P || gi + 3 >= g.nx - 1 - g.P) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const int xh = strip_h(gi + q, g.nx, g.P), xe = strip_e(gi + q, g.nx, g.P);
-          const long long po = c.s * g.xstrip + (long long)gj * g.xw;
-          if (xh >= 0) m.pxh[r * a.xcap + xh - c.xmin_h] = a.in.phyx[po + xh];
-          if (xe >= 0) m.pxe[r * a.xcap + xe - c.xmin_e] = a.in.pezx[po + xe];
+          for (int q = 0; q < 4; ++q) {
+            const int xh = strip_h(gi + q, g.nx, g.P), xe = strip_e(gi + q, g.nx, g.P);
+            const long long po = c.s * g.xstrip + (long long)gj * g.xw;
+            if (xh >= 0) m.pxh[r * a.xcap + xh - c.xmin_h] = a.in.phyx[po + xh];
+            if (xe >= 0) m.pxe[r * a.xcap + xe - c.xmin_e] = a.in.pezx[po + xe];
+          }
         }
-        if (owned(r, lc)) unpack(ld4(a.ez_planes[0] + o), rg.e1[k]);
+        if (rg.fl[k] & kOwn) unpack(ld4(a.ez_planes[0] + o), rg.e1[k]);
       }
       st4(m.le + r * RW + lc, e); st4(m.hx + r * RW + lc, hx); st4(m.hy + r * RW + lc, hy);
+      st4(m.q + r * RW + lc, mk4(rg.cb[k][0] * e.x, rg.cb[k][1] * e.y, rg.cb[k][2] * e.z, rg.cb[k][3] * e.w));
     }
   }
 
-  // transpose of recording: residual sample n+1 enters lamE at every receiver of the REGION
+  // transpose of recording: residual sample n+1 enters lamE (and q) at every receiver of the REGION
   GPR_HD static void inject(const AdjTileArgs& a, const Ctx& c, int tile, int tid, int t)
   {
     const int n1 = a.n_hi - t;                     // = n + 1 for reverse step n = n_hi - 1 - t
@@ -153,10 +179,13 @@ struct AdjTile {
       const int off = a.rec_off[(long long)c.s * a.R + r];
       const int lj = off / a.g.pitch - c.gj0, li = off % a.g.pitch - c.gi0;
       const float v = a.residual[c.s * a.trace_stride - (long long)t * a.R + r];
+      const float qv = a.cb[off] * v;              // receivers are never on the PEC ring
 #if defined(__CUDA_ARCH__)
       atomicAdd(c.m.le + lj * RW + li, v);         // coincident receivers sum
+      atomicAdd(c.m.q + lj * RW + li, qv);
 #else
       c.m.le[lj * RW + li] += v;
+      c.m.q[lj * RW + li] += qv;
 #endif
     }
   }
@@ -213,36 +242,39 @@ struct AdjTile {
   }
 
   // transpose of the E update + E CPML, applied to lamH
-  GPR_HD static void phase_b(const AdjTileArgs& a, const Ctx& c, int tid, int t)
+  GPR_HD static void phase_b(const AdjTileArgs& a, const Ctx& c, int tid, const Regs& rg, int t)
   {
     const Geo& g = a.g;
     const Smem& m = c.m;
 #pragma unroll
     for (int k = 0; k < KU; ++k) {
+      if (!(rg.fl[k] & kIn)) continue;
+      if (rg.fl[k] & kBFast) {                        // tz = -q, tx = q
+        const int o = rg.off[k];
+        const float4 q = ld4(m.q + o), qn = ld4(m.q + o + RW);
+        const float q5 = m.q[o + 4];
+        float4 hx = ld4(m.hx + o), hy = ld4(m.hy + o);
+        hx.x += (qn.x - q.x) * g.rdx; hx.y += (qn.y - q.y) * g.rdx;
+        hx.z += (qn.z - q.z) * g.rdx; hx.w += (qn.w - q.w) * g.rdx;
+        hy.x += (q.x - q.y) * g.rdx; hy.y += (q.y - q.z) * g.rdx;
+        hy.z += (q.z - q.w) * g.rdx; hy.w += (q.w - q5) * g.rdx;
+        st4(m.hx + o, hx); st4(m.hy + o, hy);
+        continue;
+      }
       const int u = tid + k * kTileThreads;
-      if (u >= NU) continue;
       const int r = u / RW4, lc = (u % RW4) * 4;
       const int gj = c.gj0 + r, gi = c.gi0 + lc;
-      if (gj < 0 || gj >= g.nz || gi < 0 || gi >= g.nx) continue;
-      if (t > 0) lazy_psih(a, c, r, lc, gj, gi);
+      if (t > 0 && (rg.fl[k] & kLazy)) lazy_psih(a, c, r, lc, gj, gi);
       float q[5];
-      {
-        float le[5], cb[5];
-        unpack(ld4(m.le + r * RW + lc), le);
-        unpack(ld4(m.cb + r * RW + lc), cb);
-        le[4] = lc + 4 < RW ? m.le[r * RW + lc + 4] : 0.f;
-        cb[4] = lc + 4 < RW ? m.cb[r * RW + lc + 4] : 0.f;
-#pragma unroll
-        for (int x = 0; x < 5; ++x) q[x] = cb[x] * le[x];
-      }
+      unpack(ld4(m.q + r * RW + lc), q);
+      q[4] = lc + 4 < RW ? m.q[r * RW + lc + 4] : 0.f;
       if (r + 1 < RH && gj <= g.nz - 2) {
-        float ln[4], cn[4], h[4];
-        unpack(ld4(m.le + (r + 1) * RW + lc), ln);
-        unpack(ld4(m.cb + (r + 1) * RW + lc), cn);
+        float qn[4], h[4];
+        unpack(ld4(m.q + (r + 1) * RW + lc), qn);
         unpack(ld4(m.hx + r * RW + lc), h);
 #pragma unroll
         for (int x = 0; x < 4; ++x)
-          h[x] += (tz_of(c, g, r, gj, lc + x, q[x]) - tz_of(c, g, r + 1, gj + 1, lc + x, cn[x] * ln[x])) * g.rdx;
+          h[x] += (tz_of(c, g, r, gj, lc + x, q[x]) - tz_of(c, g, r + 1, gj + 1, lc + x, qn[x])) * g.rdx;
         st4(m.hx + r * RW + lc, mk4(h[0], h[1], h[2], h[3]));
       }
       {
@@ -266,36 +298,45 @@ struct AdjTile {
   {
     const Geo& g = a.g;
     const Smem& m = c.m;
+    const float kap = g.Db * g.rdx;
 #pragma unroll
     for (int k = 0; k < KU; ++k) {
-      const int u = tid + k * kTileThreads;
-      if (u >= NU) continue;
-      const int r = u / RW4, lc = (u % RW4) * 4;
-      const int gj = c.gj0 + r, gi = c.gi0 + lc;
-      if (gj < 0 || gj >= g.nz || gi < 0 || gi >= g.nx) continue;
-      float mu[4], cb[4];
-      unpack(ld4(m.le + r * RW + lc), mu);
-      unpack(ld4(m.cb + r * RW + lc), cb);
-      const bool own = owned(r, lc);
-      if (own) {                                   // E^n of this step; E^{n+1} is carried in registers
+      if (!(rg.fl[k] & kIn)) continue;
+      const int o = rg.off[k];
+      float mu[4];
+      unpack(ld4(m.le + o), mu);
+      if (rg.fl[k] & kOwn) {                       // E^n of this step; E^{n+1} is carried in registers
         float e0[4];
-        unpack(ld4(a.ez_planes[t + 1] + c.s * g.plane + (long long)gj * g.pitch + gi), e0);
+        unpack(ld4(a.ez_planes[t + 1] + c.s * g.plane + rg.goff[k]), e0);
 #pragma unroll
-        for (int x = 0; x < 4; ++x) {
-          if (cb[x] != 0.f) {
-            rg.ga[k][x] += mu[x] * e0[x];
-            rg.gb[k][x] += mu[x] * ((rg.e1[k][x] - rg.ca[k][x] * e0[x]) / cb[x]);
-          }
+        for (int x = 0; x < 4; ++x) {              // gb holds sum mu*(E^{n+1} - Ca E^n); /Cb at the flush
+          rg.ga[k][x] += mu[x] * e0[x];
+          rg.gb[k][x] += mu[x] * (rg.e1[k][x] - rg.ca[k][x] * e0[x]);
           rg.e1[k][x] = e0[x];
         }
       }
+      if (rg.fl[k] & kCFast) {                     // sz = -Db*lamHx, sx = Db*lamHy
+        const float4 hy = ld4(m.hy + o), hxc = ld4(m.hx + o), hxm = ld4(m.hx + o - RW);
+        const float hy0 = m.hy[o - 1];
+        float4 le;
+        le.x = rg.ca[k][0] * mu[0] + kap * ((hxc.x - hxm.x) + (hy0 - hy.x));
+        le.y = rg.ca[k][1] * mu[1] + kap * ((hxc.y - hxm.y) + (hy.x - hy.y));
+        le.z = rg.ca[k][2] * mu[2] + kap * ((hxc.z - hxm.z) + (hy.y - hy.z));
+        le.w = rg.ca[k][3] * mu[3] + kap * ((hxc.w - hxm.w) + (hy.z - hy.w));
+        st4(m.le + o, le);
+        st4(m.q + o, mk4(rg.cb[k][0] * le.x, rg.cb[k][1] * le.y, rg.cb[k][2] * le.z, rg.cb[k][3] * le.w));
+        continue;
+      }
+      const int u = tid + k * kTileThreads;
+      const int r = u / RW4, lc = (u % RW4) * 4;
+      const int gj = c.gj0 + r, gi = c.gi0 + lc;
       if (!(r >= 1 && r <= RH - 2 && gj >= 1 && gj <= g.nz - 2)) continue;
       const int ze = strip_e(gj, g.nz, g.P);
       if (ze >= 0) {
         float* pp = m.pze + (ze - c.zmin_e) * RW + lc;
         const float b = m.tz[3 * RH + r];
 #pragma unroll
-        for (int x = 0; x < 4; ++x) pp[x] = b * (pp[x] - cb[x] * mu[x]);
+        for (int x = 0; x < 4; ++x) pp[x] = b * (pp[x] - rg.cb[k][x] * mu[x]);
       }
       const bool xpml_e = (gi < g.P) || (gi + 3 >= g.nx - g.P);
       const bool xpml_h = (gi - 1 < g.P) || (gi + 3 >= g.nx - 1 - g.P);
@@ -310,71 +351,76 @@ struct AdjTile {
           const int xe = strip_e(i, g.nx, g.P);
           if (xe >= 0) {
             float* pp = m.pxe + r * a.xcap + xe - c.xmin_e;
-            *pp = m.tx[3 * RW + lcol] * (*pp + cb[x] * mu[x]);
+            *pp = m.tx[3 * RW + lcol] * (*pp + rg.cb[k][x] * mu[x]);
           }
         }
-        const float szm = sz_of(c, g, r - 1, gj - 1, lcol), szc = gj <= g.nz - 2 ? sz_of(c, g, r, gj, lcol) : 0.f;
+        const float szm = sz_of(c, g, r - 1, gj - 1, lcol), szc = sz_of(c, g, r, gj, lcol);
         float sxm, sxc;
         if (xpml_h) {
           sxm = sx_of(a, c, r, i - 1, lcol - 1);
-          sxc = i <= g.nx - 2 ? sx_of(a, c, r, i, lcol) : 0.f;
+          sxc = sx_of(a, c, r, i, lcol);
         } else {
           sxm = g.Db * m.hy[r * RW + lcol - 1];
           sxc = g.Db * m.hy[r * RW + lcol];
         }
         le[x] = rg.ca[k][x] * mu[x] + (szm - szc) * g.rdx + (sxm - sxc) * g.rdx;
       }
-      st4(m.le + r * RW + lc, mk4(le[0], le[1], le[2], le[3]));
+      st4(m.le + o, mk4(le[0], le[1], le[2], le[3]));
+      st4(m.q + o, mk4(rg.cb[k][0] * le[0], rg.cb[k][1] * le[1], rg.cb[k][2] * le[2], rg.cb[k][3] * le[3]));
     }
   }
 
   // per shot: write back the owned part of the adjoint state (psiH with its pending recursion)
-  GPR_HD static void store(const AdjTileArgs& a, const Ctx& c, int tid)
+  GPR_HD static void store(const AdjTileArgs& a, const Ctx& c, int tid, const Regs& rg)
   {
     const Geo& g = a.g;
     const Smem& m = c.m;
 #pragma unroll
     for (int k = 0; k < KU; ++k) {
+      if ((rg.fl[k] & (kIn | kOwn)) != (kIn | kOwn)) continue;
       const int u = tid + k * kTileThreads;
-      if (u >= NU) continue;
       const int r = u / RW4, lc = (u % RW4) * 4;
       const int gj = c.gj0 + r, gi = c.gi0 + lc;
-      if (!owned(r, lc) || gj >= g.nz || gi >= g.nx) continue;
-      if (a.nsub > 0) lazy_psih(a, c, r, lc, gj, gi);
-      const long long o = c.s * g.plane + (long long)gj * g.pitch + gi;
+      if (a.nsub > 0 && (rg.fl[k] & kLazy)) lazy_psih(a, c, r, lc, gj, gi);
+      const long long o = c.s * g.plane + rg.goff[k];
       st4(a.out.ez + o, ld4(m.le + r * RW + lc));
       st4(a.out.hx + o, ld4(m.hx + r * RW + lc));
       st4(a.out.hy + o, ld4(m.hy + r * RW + lc));
       const int zh = strip_h(gj, g.nz, g.P), ze = strip_e(gj, g.nz, g.P);
       if (zh >= 0) st4(a.out.phxz + c.s * g.zstrip + (long long)zh * g.pitch + gi, ld4(m.pzh + (zh - c.zmin_h) * RW + lc));
       if (ze >= 0) st4(a.out.pezz + c.s * g.zstrip + (long long)ze * g.pitch + gi, ld4(m.pze + (ze - c.zmin_e) * RW + lc));
+      if (gi < g.P || gi + 3 >= g.nx - 1 - g.P) {
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const int xh = strip_h(gi + q, g.nx, g.P), xe = strip_e(gi + q, g.nx, g.P);
-        const long long po = c.s * g.xstrip + (long long)gj * g.xw;
-        if (xh >= 0) a.out.phyx[po + xh] = m.pxh[r * a.xcap + xh - c.xmin_h];
-        if (xe >= 0) a.out.pezx[po + xe] = m.pxe[r * a.xcap + xe - c.xmin_e];
+        for (int q = 0; q < 4; ++q) {
+          const int xh = strip_h(gi + q, g.nx, g.P), xe = strip_e(gi + q, g.nx, g.P);
+          const long long po = c.s * g.xstrip + (long long)gj * g.xw;
+          if (xh >= 0) a.out.phyx[po + xh] = m.pxh[r * a.xcap + xh - c.xmin_h];
+          if (xe >= 0) a.out.pezx[po + xe] = m.pxe[r * a.xcap + xe - c.xmin_e];
+        }
       }
     }
   }
 
-  // once per CTA: add the register accumulators to this group's gCa / gCb planes
+  // once per CTA: add the register partial sums to this group's gCa / gCb planes
   GPR_HD static void flush(const AdjTileArgs& a, const Ctx& c, int tid, int grp, const Regs& rg)
   {
     const Geo& g = a.g;
 #pragma unroll
     for (int k = 0; k < KU; ++k) {
-      const int u = tid + k * kTileThreads;
-      if (u >= NU) continue;
-      const int r = u / RW4, lc = (u % RW4) * 4;
-      const int gj = c.gj0 + r, gi = c.gi0 + lc;
-      if (!owned(r, lc) || gj >= g.nz || gi >= g.nx) continue;
-      float* pa = a.gca + grp * g.plane + (long long)gj * g.pitch + gi;
-      float* pb = a.gcb + grp * g.plane + (long long)gj * g.pitch + gi;
-      float4 va = ld4(pa), vb = ld4(pb);
-      va.x += rg.ga[k][0]; va.y += rg.ga[k][1]; va.z += rg.ga[k][2]; va.w += rg.ga[k][3];
-      vb.x += rg.gb[k][0]; vb.y += rg.gb[k][1]; vb.z += rg.gb[k][2]; vb.w += rg.gb[k][3];
-      st4(pa, va); st4(pb, vb);
+      if ((rg.fl[k] & (kIn | kOwn)) != (kIn | kOwn)) continue;
+      float* pa = a.gca + grp * g.plane + rg.goff[k];
+      float* pb = a.gcb + grp * g.plane + rg.goff[k];
+      float va[4], vb[4];
+      unpack(ld4(pa), va);
+      unpack(ld4(pb), vb);
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+        if (rg.cb[k][x] == 0.f) continue;          // PEC cells and the ring: no dependence on Ca, Cb
+        va[x] += rg.ga[k][x];
+        vb[x] += rg.gb[k][x] / rg.cb[k][x];
+      }
+      st4(pa, mk4(va[0], va[1], va[2], va[3]));
+      st4(pb, mk4(vb[0], vb[1], vb[2], vb[3]));
     }
   }
 };
@@ -399,12 +445,12 @@ __global__ void __launch_bounds__(kTileThreads) adj_tile_kernel(const AdjTileArg
     for (int t = 0; t < a.nsub; ++t) {
       K::inject(a, c, tile, tid, t);
       __syncthreads();
-      K::phase_b(a, c, tid, t);
+      K::phase_b(a, c, tid, rg, t);
       __syncthreads();
       K::phase_c(a, c, tid, rg, t);
       __syncthreads();
     }
-    K::store(a, c, tid);
+    K::store(a, c, tid, rg);
   }
   K::flush(a, c, tid, grp, rg);
 }

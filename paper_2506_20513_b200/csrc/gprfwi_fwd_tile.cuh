@@ -38,12 +38,26 @@ struct FwdTileArgs {
   int zcap, xcap;             // rows / columns of psi strips staged per CTA
 };
 
+// Update expressions off the CPML, written once with explicit fma so that the fast path, the general
+// path and every CTA that recomputes a halo cell round identically (results do not depend on the
+// time blocking or on which tile computed a cell).
+GPR_HD float fwd_h_minus(float h, float kap, float hi, float lo) { return fmaf(-kap, hi - lo, h); }
+GPR_HD float fwd_h_plus(float h, float kap, float hi, float lo) { return fmaf(kap, hi - lo, h); }
+GPR_HD float fwd_e_plain(float ca, float e, float cb, float hy1, float hy0, float hxc, float hxm, float rdx)
+{
+  return fmaf(cb, ((hy1 - hy0) - (hxc - hxm)) * rdx, ca * e);
+}
+
 template <int TZ, int TX, int T>
 struct FwdTile {
   static constexpr int RH = TZ + 2 * T, RW = TX + 8, RW4 = RW / 4;
   static constexpr int NU = RH * RW4;
   static constexpr int KU = (NU + kTileThreads - 1) / kTileThreads;
-  struct Regs { float ca[KU][4], cb[KU][4]; };
+  // per-thread state kept for the whole launch: Ca/Cb of the thread's cells and, per unit, the
+  // shared-memory offset and a class mask (bit 0: in the grid; 1: H fast path; 2: E fast path;
+  // 3: owned by this tile).  Fast path = no CPML, no grid or region edge, no source in the unit.
+  struct Regs { float ca[KU][4], cb[KU][4]; int off[KU], goff[KU]; unsigned fl[KU]; };
+  static constexpr unsigned kIn = 1u, kHFast = 2u, kEFast = 4u, kOwn = 8u;
 
   // shared-memory carve-up (floats)
   struct Smem {
@@ -112,10 +126,26 @@ struct FwdTile {
       const int u = tid + k * kTileThreads;
       rg.ca[k][0] = rg.ca[k][1] = rg.ca[k][2] = rg.ca[k][3] = 0.f;
       rg.cb[k][0] = rg.cb[k][1] = rg.cb[k][2] = rg.cb[k][3] = 0.f;
+      rg.off[k] = 0; rg.goff[k] = 0; rg.fl[k] = 0u;
       if (u >= NU) continue;
       const int r = u / RW4, lc = (u % RW4) * 4;
       const int gj = c.gj0 + r, gi = c.gi0 + lc;
       const bool in = gj >= 0 && gj < g.nz && gi >= 0 && gi < g.nx;
+      rg.off[k] = r * RW + lc;
+      rg.goff[k] = gj * g.pitch + gi;
+      if (in) {
+        const int src = a.src_off[c.s];
+        const int sj = src / g.pitch, si = src % g.pitch;
+        const bool nozh = strip_h(gj, g.nz, g.P) < 0, noze = strip_e(gj, g.nz, g.P) < 0;
+        const bool noxh = gi >= g.P && gi + 3 < g.nx - 1 - g.P, noxe = gi >= g.P && gi + 3 < g.nx - g.P;
+        unsigned f = kIn;
+        if (r + 1 < RH && gj <= g.nz - 2 && lc + 4 < RW && gi + 3 <= g.nx - 2 && nozh && noxh) f |= kHFast;
+        if (r >= 1 && r <= RH - 2 && gj >= 1 && gj <= g.nz - 2 && lc >= 4 && lc + 3 <= RW - 2 && gi >= 1 &&
+            gi + 3 <= g.nx - 2 && noze && noxe && !(gj == sj && si >= gi && si <= gi + 3))
+          f |= kEFast;
+        if (r >= T && r < T + TZ && lc >= 4 && lc < 4 + TX) f |= kOwn;
+        rg.fl[k] = f;
+      }
       float4 e = mk4(0, 0, 0, 0), hx = e, hy = e;
       if (in) {
         const long long o = c.s * g.plane + (long long)gj * g.pitch + gi;
@@ -152,17 +182,29 @@ struct FwdTile {
   }
 
   // ---- stages 2-3: H update + H CPML (Eqs. 4-5) ---------------------------------
-  GPR_HD static void phase_h(const FwdTileArgs& a, const Ctx& c, int tid)
+  GPR_HD static void phase_h(const FwdTileArgs& a, const Ctx& c, int tid, const Regs& rg)
   {
     const Geo& g = a.g;
     const Smem& m = c.m;
+    const float kap = g.Db * g.rdx;
 #pragma unroll
     for (int k = 0; k < KU; ++k) {
+      if (!(rg.fl[k] & kIn)) continue;
+      if (rg.fl[k] & kHFast) {
+        const int o = rg.off[k];
+        const float4 e4 = ld4(m.ez + o), en = ld4(m.ez + o + RW);
+        const float e5 = m.ez[o + 4];
+        float4 hx = ld4(m.hx + o), hy = ld4(m.hy + o);
+        hx.x = fwd_h_minus(hx.x, kap, en.x, e4.x); hx.y = fwd_h_minus(hx.y, kap, en.y, e4.y);
+        hx.z = fwd_h_minus(hx.z, kap, en.z, e4.z); hx.w = fwd_h_minus(hx.w, kap, en.w, e4.w);
+        hy.x = fwd_h_plus(hy.x, kap, e4.y, e4.x); hy.y = fwd_h_plus(hy.y, kap, e4.z, e4.y);
+        hy.z = fwd_h_plus(hy.z, kap, e4.w, e4.z); hy.w = fwd_h_plus(hy.w, kap, e5, e4.w);
+        st4(m.hx + o, hx); st4(m.hy + o, hy);
+        continue;
+      }
       const int u = tid + k * kTileThreads;
-      if (u >= NU) continue;
       const int r = u / RW4, lc = (u % RW4) * 4;
       const int gj = c.gj0 + r, gi = c.gi0 + lc;
-      if (gj < 0 || gj >= g.nz || gi < 0 || gi >= g.nx) continue;
       float e[5];
       unpack(ld4(m.ez + r * RW + lc), e);
       e[4] = lc + 4 < RW ? m.ez[r * RW + lc + 4] : 0.f;
@@ -185,7 +227,7 @@ struct FwdTile {
           st4(pp, mk4(p[0], p[1], p[2], p[3]));
         } else {
 #pragma unroll
-          for (int q = 0; q < 4; ++q) h[q] -= g.Db * ((en[q] - e[q]) * g.rdx);
+          for (int q = 0; q < 4; ++q) h[q] = fwd_h_minus(h[q], kap, en[q], e[q]);
         }
         st4(m.hx + r * RW + lc, mk4(h[0], h[1], h[2], h[3]));
       }
@@ -204,7 +246,7 @@ struct FwdTile {
             *pp = p;
             h[q] += g.Db * (d * m.tx[2 * RW + lc + q] + p);
           } else {
-            h[q] += g.Db * d;
+            h[q] = fwd_h_plus(h[q], kap, e[q + 1], e[q]);
           }
         }
         st4(m.hy + r * RW + lc, mk4(h[0], h[1], h[2], h[3]));
@@ -222,11 +264,23 @@ struct FwdTile {
     const float wn = a.wavelet[c.s * a.wav_stride + t] * (g.rdx * g.rdx);
 #pragma unroll
     for (int k = 0; k < KU; ++k) {
+      if (!(rg.fl[k] & kIn)) continue;
+      if (rg.fl[k] & kEFast) {
+        const int o = rg.off[k];
+        float4 ev = ld4(m.ez + o);
+        const float4 hy = ld4(m.hy + o), hxc = ld4(m.hx + o), hxm = ld4(m.hx + o - RW);
+        const float hy0 = m.hy[o - 1];
+        ev.x = fwd_e_plain(rg.ca[k][0], ev.x, rg.cb[k][0], hy.x, hy0, hxc.x, hxm.x, g.rdx);
+        ev.y = fwd_e_plain(rg.ca[k][1], ev.y, rg.cb[k][1], hy.y, hy.x, hxc.y, hxm.y, g.rdx);
+        ev.z = fwd_e_plain(rg.ca[k][2], ev.z, rg.cb[k][2], hy.z, hy.y, hxc.z, hxm.z, g.rdx);
+        ev.w = fwd_e_plain(rg.ca[k][3], ev.w, rg.cb[k][3], hy.w, hy.z, hxc.w, hxm.w, g.rdx);
+        st4(m.ez + o, ev);
+        if (ez_out && (rg.fl[k] & kOwn)) st4(ez_out + c.s * g.plane + rg.goff[k], ev);
+        continue;
+      }
       const int u = tid + k * kTileThreads;
-      if (u >= NU) continue;
       const int r = u / RW4, lc = (u % RW4) * 4;
       const int gj = c.gj0 + r, gi = c.gi0 + lc;
-      if (gj < 0 || gj >= g.nz || gi < 0 || gi >= g.nx) continue;
       float e[4];
       unpack(ld4(m.ez + r * RW + lc), e);
       if (r >= 1 && r <= RH - 2 && gj >= 1 && gj <= g.nz - 2) {
@@ -259,7 +313,8 @@ struct FwdTile {
             pz[q] = bz * pz[q] + cz * dzh;
             vz = dzh * kz + pz[q];
           }
-          e[q] = rg.ca[k][q] * e[q] + rg.cb[k][q] * (vx - vz);
+          if (xe < 0 && ze < 0) e[q] = fwd_e_plain(rg.ca[k][q], e[q], rg.cb[k][q], hy[q + 1], hy[q], hxc[q], hxm[q], g.rdx);
+          else e[q] = rg.ca[k][q] * e[q] + rg.cb[k][q] * (vx - vz);
           // stage 6: source; every CTA whose region holds the cell injects
           if (gj == sj && i == si) e[q] -= rg.cb[k][q] * wn;
         }
@@ -315,7 +370,7 @@ __global__ void __launch_bounds__(kTileThreads) fwd_tile_kernel(const FwdTileArg
   __syncthreads();
   for (int t = 0; t < a.nsub; ++t) {
     K::record(a, c, tile, tid, t);
-    K::phase_h(a, c, tid);
+    K::phase_h(a, c, tid, rg);
     __syncthreads();
     K::phase_e(a, c, tid, rg, t, t + 1 == a.nsub ? a.out.ez : a.ez_hist[t + 1]);
     __syncthreads();
