@@ -11,12 +11,11 @@
 #include <vector>
 
 #include "gprfwi.h"
-#include "gprfwi_adj.cuh"
-#include "gprfwi_adj_tile.cuh"
+#include "gprfwi_adj_kernel.cuh"
 #include "gprfwi_common.cuh"
-#include "gprfwi_fwd.cuh"
-#include "gprfwi_fwd_tile.cuh"
+#include "gprfwi_fwd_kernel.cuh"
 #include "gprfwi_misc.cuh"
+#include "gprfwi_tile.cuh"
 
 namespace gprfwi {
 
@@ -48,17 +47,25 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 // ------------------------------------------------------------------------------------------------
 // memory plan
 // ------------------------------------------------------------------------------------------------
+// register-tile shapes (rows per thread, warps per CTA, min CTAs per SM): gprfwi_tile.cuh
+#define GPR_FWD_TILE 4, 8, 2
+#define GPR_ADJ_TILE 3, 8, 2
+using FwdShape = RegTile<4, 8>;
+using AdjShape = RegTile<3, 8>;
+
+struct Tiling {
+  int oz = 0, tiles_x = 0, tiles_y = 0;   // owned rows per tile; tiles of kOwnW columns x oz rows
+  int tiles() const { return tiles_x * tiles_y; }
+};
+
 struct Layout {
   // geometry-derived sizes (floats)
   int pitch = 0, xw = 0;
   size_t plane = 0, zstrip = 0, xstrip = 0;
   size_t hslot = 0;        // Hx, Hy, 4 psi strips of ONE shot
   size_t full = 0;         // hslot + Ez plane
-  int T = 1;               // time steps fused per launch (1: v1 streaming kernels)
-  int tz = kBlockRows, tx = kBlockCols;   // tile owned by one CTA
-  int hz = 0, hx = 0;      // halo staged around it
-  int zcap = 0, xcap = 0;  // psi strip rows / columns staged per CTA (max over tiles)
-  int tiles_x = 0, tiles_y = 0;
+  int T = 4;               // time steps fused per launch = halo rows
+  Tiling f, a;             // forward / adjoint tilings
   // plan
   bool full_history = true;
   int K = 0;               // checkpoint stride (nt when full history)
@@ -92,34 +99,24 @@ static void base_layout(const gprfwi_params* p, Layout& L)
   L.xstrip = (size_t)p->nz * L.xw;
   L.hslot = 2 * L.plane + 2 * L.zstrip + 2 * L.xstrip;
   L.full = L.hslot + L.plane;
-  // time blocking: GPRFWI_TIME_BLOCK=1 selects the one-step-per-launch kernels (debug / comparison)
-  L.T = 4;
-  if (const char* e = std::getenv("GPRFWI_TIME_BLOCK")) L.T = std::max(1, std::min(4, std::atoi(e)));
-  if (L.T > 1) { L.tz = 32; L.tx = 64; L.hz = L.T; L.hx = 4; }
-  L.tiles_x = (p->nx + L.tx - 1) / L.tx;
-  L.tiles_y = (p->nz + L.tz - 1) / L.tz;
-  // strip rows / columns a region can hold: count of strip indices met by [lo, lo + len)
-  auto span = [&](int lo, int len, int n, bool hloc) {
-    int first = -1, last = -1;
-    for (int q = std::max(lo, 0); q < std::min(lo + len, n); ++q) {
-      const int sidx = hloc ? strip_h(q, n, p->npml) : strip_e(q, n, p->npml);
-      if (sidx >= 0) { if (first < 0) first = sidx; last = sidx; }
-    }
-    return first < 0 ? 0 : last - first + 1;
+  // time blocking: GPRFWI_TIME_BLOCK=1..4 (default 4) steps per launch; the z halo is as deep
+  L.T = kMaxT;
+  if (const char* e = std::getenv("GPRFWI_TIME_BLOCK")) L.T = std::max(1, std::min(kMaxT, std::atoi(e)));
+  auto tiling = [&](int rows, Tiling& t) {
+    t.oz = rows - 2 * L.T;
+    t.tiles_x = (p->nx + kOwnW - 1) / kOwnW;
+    t.tiles_y = (p->nz + t.oz - 1) / t.oz;
   };
-  L.zcap = L.xcap = 0;
-  for (int t = 0; t < L.tiles_y; ++t)
-    for (int hl = 0; hl < 2; ++hl) L.zcap = std::max(L.zcap, span(t * L.tz - L.hz, L.tz + 2 * L.hz, p->nz, hl));
-  for (int t = 0; t < L.tiles_x; ++t)
-    for (int hl = 0; hl < 2; ++hl) L.xcap = std::max(L.xcap, span(t * L.tx - L.hx, L.tx + 2 * L.hx, p->nx, hl));
-  L.zcap = std::max(L.zcap, 1);
-  L.xcap = std::max(L.xcap, 1);
+  tiling(FwdShape::ROWS, L.f);
+  tiling(AdjShape::ROWS, L.a);
 }
 
+// Shots of one adjoint pass are split into groups; a CTA sweeps the shots of its group one after the
+// other and keeps their gradient sum in registers.  Enough groups to fill the SMs a few times.
 static void set_groups(Layout& L)
 {
-  const int tiles = L.tiles_x * L.tiles_y;
-  int want = std::max(1, ((L.T > 1 ? 888 : 1184) + tiles - 1) / tiles);   // CTAs to fill 148 SMs a few times
+  const int tiles = L.a.tiles();
+  int want = std::max(1, (4 * 148 + tiles - 1) / tiles);
   int ng = std::min(L.Sb, want);
   L.group = (L.Sb + ng - 1) / ng;
   L.ngroups = (L.Sb + L.group - 1) / L.group;
@@ -147,7 +144,7 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
     return r;
   };
   const size_t S = (size_t)p->nshots, R = (size_t)p->nrec, f = sizeof(float);
-  const size_t ntile = (size_t)L.tiles_x * L.tiles_y;
+  const size_t ntile = (size_t)L.f.tiles(), natile = (size_t)L.a.tiles();
   Carve tmp;
   Carve& o = c ? *c : tmp;
   o.ca = (float*)take(L.plane * f);
@@ -159,8 +156,8 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
   o.rec_off = (int*)take(std::max<size_t>(S * R, 1) * sizeof(int));
   o.blk_start = (int*)take(S * (ntile + 1) * sizeof(int));
   o.blk_rec = (int*)take(std::max<size_t>(S * R, 1) * sizeof(int));
-  o.reg_start = (int*)take((S * ntile + 1) * sizeof(int));
-  o.reg_rec = (int*)take(std::max<size_t>(4 * S * R, 1) * sizeof(int));
+  o.reg_start = (int*)take((S * natile + 1) * sizeof(int));
+  o.reg_rec = (int*)take(std::max<size_t>(6 * S * R, 1) * sizeof(int));
   o.fscratch = (float*)take(2 * S * L.full * f);
   o.lam = (float*)take(2 * (size_t)L.Sb * L.full * f);
   if (L.full_history) {
@@ -287,7 +284,7 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
 {
   const gprfwi_params& p = h->p;
   const Layout& L = h->L;
-  const int S = p.nshots, R = p.nrec, ntile = L.tiles_x * L.tiles_y;
+  const int S = p.nshots, R = p.nrec, ntile = L.f.tiles(), natile = L.a.tiles();
   h->h_src_off.assign(S, 0);
   h->h_rec_off.assign(std::max(S * R, 1), 0);
   h->h_blk_start.assign((size_t)S * (ntile + 1), 0);
@@ -303,28 +300,28 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
       const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
       if (!ok(rz, rx)) return GPRFWI_EGEOM;
       h->h_rec_off[(size_t)s * R + r] = rz * L.pitch + rx;
-      tile_of[r] = (rz / L.tz) * L.tiles_x + rx / L.tx;
+      tile_of[r] = (rz / L.f.oz) * L.f.tiles_x + rx / kOwnW;
       start[tile_of[r] + 1]++;
     }
     for (int t = 0; t < ntile; ++t) start[t + 1] += start[t];
     std::vector<int> fill(start, start + ntile);
     for (int r = 0; r < R; ++r) h->h_blk_rec[(size_t)s * R + fill[tile_of[r]]++] = r;
   }
-  // receivers by region: a receiver within the halo of a tile is injected there too
-  h->h_reg_start.assign((size_t)S * ntile + 1, 0);
+  // receivers by region of the adjoint tiling: a receiver within the halo of a tile is injected there too
+  h->h_reg_start.assign((size_t)S * natile + 1, 0);
   h->h_reg_rec.clear();
   for (int s = 0; s < S; ++s)
-    for (int ty = 0; ty < L.tiles_y; ++ty)
-      for (int tx = 0; tx < L.tiles_x; ++tx) {
-        const int z0 = ty * L.tz - L.hz, z1 = ty * L.tz + L.tz + L.hz;
-        const int x0 = tx * L.tx - L.hx, x1 = tx * L.tx + L.tx + L.hx;
+    for (int ty = 0; ty < L.a.tiles_y; ++ty)
+      for (int tx = 0; tx < L.a.tiles_x; ++tx) {
+        const int z0 = ty * L.a.oz - L.T, z1 = z0 + AdjShape::ROWS;
+        const int x0 = tx * kOwnW - 4, x1 = x0 + kRegW;
         for (int r = 0; r < R; ++r) {
           const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
           if (rz >= z0 && rz < z1 && rx >= x0 && rx < x1) h->h_reg_rec.push_back(r);
         }
-        h->h_reg_start[(size_t)s * ntile + ty * L.tiles_x + tx + 1] = (int)h->h_reg_rec.size();
+        h->h_reg_start[(size_t)s * natile + ty * L.a.tiles_x + tx + 1] = (int)h->h_reg_rec.size();
       }
-  if (h->h_reg_rec.size() > (size_t)std::max(4 * S * R, 1)) return GPRFWI_EINVAL;
+  if (h->h_reg_rec.size() > (size_t)std::max(6 * S * R, 1)) return GPRFWI_EINVAL;
   if (h->h_reg_rec.empty()) h->h_reg_rec.push_back(0);
   return GPRFWI_OK;
 }
@@ -369,50 +366,17 @@ static int upload_static(gprfwi_handle* h, cudaStream_t st)
   return GPRFWI_OK;
 }
 
-// One forward step n -> n+1 for `ns` shots starting at global shot `shot0`.
-static int launch_fwd(gprfwi_handle* h, cudaStream_t st, int n, int shot0, int ns, const State& in,
-                      const State& out, float* traces)
-{
-  const gprfwi_params& p = h->p;
-  FwdArgs a;
-  a.g = h->geo;
-  a.in = in;
-  a.out = out;
-  a.ca = h->c.ca;
-  a.cb = h->c.cb;
-  a.wav_stride = p.wavelet_per_shot ? p.nt : 0;
-  a.wavelet = h->wavelet + n + (size_t)shot0 * a.wav_stride;
-  a.src_off = h->c.src_off + shot0;
-  a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
-  a.trace_stride = (long long)p.nt * p.nrec;
-  a.traces = (traces && p.nrec > 0) ? traces + (size_t)shot0 * a.trace_stride + (size_t)n * p.nrec : nullptr;
-  a.R = p.nrec;
-  a.nshots = ns;
-  a.tiles_y = h->L.tiles_y;
-  dim3 grid(h->L.tiles_x, h->L.tiles_y + (a.traces ? 1 : 0), ns), block(32, kWarpsY);
-  GPR_LAUNCH(fwd_step_kernel, grid, block, st, a);
-  h->launches++;
-  return GPRFWI_OK;
-}
-
-
-// ---- temporally blocked kernels: tile variants and their launchers ------------------------------
 #ifndef GPR_LAUNCH_SMEM
 #define GPR_LAUNCH_SMEM(kernel, grid, block, smem, stream, ...) kernel<<<grid, block, smem, stream>>>(__VA_ARGS__)
 #endif
-#define GPR_TILE_VARIANT 32, 64, 4
-using FwdTileV = FwdTile<GPR_TILE_VARIANT>;
-using AdjTileV = AdjTile<GPR_TILE_VARIANT>;
 
-static int tile_kernels_init(const Layout& L)
+static int kernels_init(const gprfwi_params* p)
 {
-#if defined(__CUDACC__) && !defined(GPRFWI_EMU)
-  GPR_CUDA(cudaFuncSetAttribute(fwd_tile_kernel<GPR_TILE_VARIANT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)(FwdTileV::smem_floats(L.zcap, L.xcap) * sizeof(float))));
-  GPR_CUDA(cudaFuncSetAttribute(adj_tile_kernel<GPR_TILE_VARIANT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)(AdjTileV::smem_floats(L.zcap, L.xcap) * sizeof(float))));
-#endif
-  (void)L;
+  const bool pml = p->npml > 0;
+  GPR_CUDA(cudaFuncSetAttribute(fwd_kernel<GPR_FWD_TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)FwdShape::smem_bytes(pml)));
+  GPR_CUDA(cudaFuncSetAttribute(adj_kernel<GPR_ADJ_TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)AdjShape::smem_bytes(pml)));
   return GPRFWI_OK;
 }
 
@@ -424,8 +388,7 @@ static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, 
 {
   const gprfwi_params& p = h->p;
   const Layout& L = h->L;
-  if (L.T == 1) return launch_fwd(h, st, n, shot0, ns, in, out, traces);
-  FwdTileArgs a;
+  FwdArgs a;
   a.g = h->geo;
   a.in = in;
   a.out = out;
@@ -436,19 +399,18 @@ static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, 
   a.wavelet = h->wavelet + n + (size_t)shot0 * a.wav_stride;
   a.src_off = h->c.src_off + shot0;
   a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
-  a.blk_start = h->c.blk_start + (size_t)shot0 * (L.tiles_x * L.tiles_y + 1);
+  a.blk_start = h->c.blk_start + (size_t)shot0 * (L.f.tiles() + 1);
   a.blk_rec = h->c.blk_rec + (size_t)shot0 * p.nrec;
   a.trace_stride = (long long)p.nt * p.nrec;
   a.traces = (traces && p.nrec > 0) ? traces + (size_t)shot0 * a.trace_stride + (size_t)n * p.nrec : nullptr;
-  a.R = p.nrec;
+  a.nrec = p.nrec;
   a.nsub = nsub;
-  a.tiles_x = L.tiles_x;
-  a.tiles_y = L.tiles_y;
-  a.zcap = L.zcap;
-  a.xcap = L.xcap;
-  dim3 grid(L.tiles_x, L.tiles_y, ns), block(kTileThreads);
-  GPR_LAUNCH_SMEM(fwd_tile_kernel<GPR_TILE_VARIANT>, grid, block,
-                  FwdTileV::smem_floats(L.zcap, L.xcap) * sizeof(float), st, a);
+  a.tiles_x = L.f.tiles_x;
+  a.tiles_y = L.f.tiles_y;
+  a.hz = L.T;
+  a.oz = L.f.oz;
+  dim3 grid(L.f.tiles_x, L.f.tiles_y, ns), block(FwdShape::THREADS);
+  GPR_LAUNCH_SMEM(fwd_kernel<GPR_FWD_TILE>, grid, block, FwdShape::smem_bytes(p.npml > 0), st, a);
   h->launches++;
   return GPRFWI_OK;
 }
@@ -462,34 +424,7 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   const Layout& L = h->L;
   const long long tstride = (long long)p.nt * p.nrec;
   const int ngrp = (ns + L.group - 1) / L.group;
-  if (L.T == 1) {
-    const int n = n_hi - 1;
-    AdjArgs a;
-    a.g = h->geo;
-    a.in = in;
-    a.out = out;
-    a.ca = h->c.ca;
-    a.cb = h->c.cb;
-    a.en = ez_of(n);
-    a.en1 = ez_of(n + 1);
-    a.gca = h->c.gca;
-    a.gcb = h->c.gcb;
-    a.trace_stride = tstride;
-    a.residual = residual ? residual + (size_t)shot0 * tstride + (size_t)n * p.nrec : nullptr;
-    a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
-    a.blk_start = h->c.blk_start + (size_t)shot0 * (L.tiles_x * L.tiles_y + 1);
-    a.blk_rec = h->c.blk_rec + (size_t)shot0 * p.nrec;
-    a.R = p.nrec;
-    a.nshots = ns;
-    a.group = L.group;
-    a.tiles_x = L.tiles_x;
-    a.tiles_y = L.tiles_y;
-    dim3 grid(L.tiles_x, L.tiles_y, ngrp), block(32, kWarpsY);
-    GPR_LAUNCH(adj_step_kernel, grid, block, st, a);
-    h->launches++;
-    return GPRFWI_OK;
-  }
-  AdjTileArgs a;
+  AdjArgs a;
   a.g = h->geo;
   a.in = in;
   a.out = out;
@@ -503,20 +438,19 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
   a.reg_start = h->c.reg_start;
   a.reg_rec = h->c.reg_rec;
-  a.R = p.nrec;
+  a.nrec = p.nrec;
   a.nsub = nsub;
   a.n_hi = n_hi;
   a.nt = p.nt;
   a.nshots = ns;
   a.group = L.group;
-  a.tiles_x = L.tiles_x;
-  a.tiles_y = L.tiles_y;
-  a.zcap = L.zcap;
-  a.xcap = L.xcap;
+  a.tiles_x = L.a.tiles_x;
+  a.tiles_y = L.a.tiles_y;
+  a.hz = L.T;
+  a.oz = L.a.oz;
   a.shot_base = shot0;
-  dim3 grid(L.tiles_x, L.tiles_y, ngrp), block(kTileThreads);
-  GPR_LAUNCH_SMEM(adj_tile_kernel<GPR_TILE_VARIANT>, grid, block,
-                  AdjTileV::smem_floats(L.zcap, L.xcap) * sizeof(float), st, a);
+  dim3 grid(L.a.tiles_x, L.a.tiles_y, ngrp), block(AdjShape::THREADS);
+  GPR_LAUNCH_SMEM(adj_kernel<GPR_ADJ_TILE>, grid, block, AdjShape::smem_bytes(p.npml > 0), st, a);
   h->launches++;
   return GPRFWI_OK;
 }
@@ -616,7 +550,7 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
   // fields are zero at n = 0
   GPR_CUDA(cudaMemsetAsync(h->c.fscratch, 0, 2 * S * L.full * f, st));
   float* slot[2] = {h->c.fscratch, h->c.fscratch + S * L.full};
-  rc = tile_kernels_init(L);
+  rc = kernels_init(p);
   if (rc != GPRFWI_OK) return rc;
   if (L.full_history) GPR_CUDA(cudaMemsetAsync(h->c.hist, 0, S * L.plane * f, st));
   else GPR_CUDA(cudaMemsetAsync(h->c.ckpt, 0, S * L.full * f, st));       // checkpoint 0 = zero state
@@ -656,7 +590,6 @@ int gprfwi_adjoint(gprfwi_handle* h, const float* residual, float* grad_eps_r, f
   const Layout& L = h->L;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t S = p->nshots, f = sizeof(float);
-  const long long tstride = (long long)p->nt * p->nrec;
   GPR_CUDA(cudaMemsetAsync(h->c.gca, 0, (size_t)L.ngroups * L.plane * f, st));
   GPR_CUDA(cudaMemsetAsync(h->c.gcb, 0, (size_t)L.ngroups * L.plane * f, st));
   float* lam[2] = {h->c.lam, h->c.lam + (size_t)L.Sb * L.full};

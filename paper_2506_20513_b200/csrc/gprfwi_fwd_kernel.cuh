@@ -1,0 +1,210 @@
+// gprfwi_fwd_kernel.cuh -- forward kernel (kernels b, c, d of north_star fused): ONE launch advances
+// all shots by up to T = 4 time steps of Algorithm 1:
+//   stage 1  record receivers (trace sample n = Ez BEFORE step n)
+//   stage 2-3  H update + H-side CPML  (Eqs. (4)-(5))
+//   stage 4-5  E update + E-side CPML  (Eq. (3) in the Ca/Cb form of the paper's kernel)
+//   stage 6  source:  Ez[src] -= Cb[src] * w[n] / dx^2   (PAPER.md:364-384 with dl = dz)
+//   stage 7  save wavefield: every step's Ez plane of the owned cells (history / recompute segment)
+// on the register tile of gprfwi_tile.cuh.  Per step: H phase, barrier, E phase, barrier.
+//
+// CPML (reading R4): psi <- b psi + c d,  derivative term d/kappa + psi, with d the plain
+// difference quotient; b, c, 1/kappa from 1-D tables.  A cell uses the psi form iff its row / column
+// lies in the corresponding strip, else the plain fused-multiply-add form; which form a cell uses
+// depends only on where it is, never on which CTA computes it.
+#pragma once
+#include "gprfwi_tile.cuh"
+
+namespace gprfwi {
+
+struct FwdArgs {
+  Geo g;
+  State in, out;              // out.ez: Ez plane after the last step of this launch
+  const float *ca, *cb;       // [nz][pitch], 0 on the PEC ring, in PEC cells and in the pitch padding
+  float* ez_hist[kMaxT];      // [t]: plane for Ez after step t (1 <= t < nsub) or NULL; [0] unused
+  const float* wavelet;       // sample n of local shot 0
+  long long wav_stride;       // nt or 0
+  const int* src_off;         // [S] j*pitch + i
+  const int* rec_off;         // [S][nrec]
+  const int* blk_start;       // [S][tiles + 1] CSR of receivers by owning tile
+  const int* blk_rec;         // [S][nrec]
+  float* traces;              // sample n of local shot 0 (NULL: do not record)
+  long long trace_stride;     // nt * nrec
+  int nrec, nsub;             // receivers per shot; steps in this launch (<= hz)
+  int tiles_x, tiles_y;
+  int hz, oz;                 // halo rows; owned rows per tile (= NW*R - 2*hz)
+};
+
+#if defined(__CUDACC__)
+template <int R, int NW, int MINB>
+__global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
+{
+  using L = RegTile<R, NW>;
+  extern __shared__ float4 smem4[];
+  const Geo& g = a.g;
+  TileCtx<R, NW> c;
+  c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
+  const int s = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
+  const unsigned full = 0xffffffffu;
+  const float rdx = g.rdx, Db = g.Db, kap = g.Db * g.rdx;
+
+  c.stage_tables(g);
+
+  // rows of this warp that hold receivers owned by this tile (warp-uniform bit mask)
+  unsigned rflags = 0u;
+  const int* rs = a.blk_start + (long long)s * (a.tiles_x * a.tiles_y + 1);
+  const int rk0 = a.traces ? rs[tile] : 0, rk1 = a.traces ? rs[tile + 1] : 0;
+  for (int k = rk0 + c.lane; k < rk1; k += 32) {
+    const int lj = a.rec_off[(long long)s * a.nrec + a.blk_rec[(long long)s * a.nrec + k]] / g.pitch - c.gj0;
+    if (lj >= 0 && lj < R) rflags |= 1u << lj;
+  }
+  rflags = __reduce_or_sync(full, rflags);
+
+  // the source cell, if this thread holds it
+  int src_r = -1, src_c = 0;
+  {
+    const int src = a.src_off[s];
+    const int dj = src / g.pitch - c.gj0, di = src % g.pitch - c.gi;
+    if (dj >= 0 && dj < R && di >= 0 && di < 4) { src_r = dj; src_c = di; }
+  }
+
+  // ---- load the region into registers ------------------------------------------------------------
+  float e[R][4], hx[R][4], hy[R][4], ca[R][4], cb[R][4];
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    zero4(e[r]); zero4(hx[r]); zero4(hy[r]); zero4(ca[r]); zero4(cb[r]);
+    if (c.colin && ((c.rin >> r) & 1u)) {
+      const long long o = (long long)(c.gj0 + r) * g.pitch + c.gi;
+      ldg4a(a.in.ez + s * g.plane + o, e[r]);
+      ldg4a(a.in.hx + s * g.plane + o, hx[r]);
+      ldg4a(a.in.hy + s * g.plane + o, hy[r]);
+      ldg4a(a.ca + o, ca[r]);
+      ldg4a(a.cb + o, cb[r]);
+    }
+  }
+  c.load_psi(g, a.in, s);
+  st4a(c.xe_() + c.w * kRegW + c.l4, e[0]);
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+    if ((rflags >> r) & 1u) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
+  __syncthreads();
+
+  for (int t = 0; t < a.nsub; ++t) {
+    // ---- stage 1: trace sample n + t from the published receiver rows ----------------------------
+    for (int k = rk0 + threadIdx.x; k < rk1; k += L::THREADS) {
+      const int rr = a.blk_rec[(long long)s * a.nrec + k];
+      const int off = a.rec_off[(long long)s * a.nrec + rr];
+      a.traces[s * a.trace_stride + (long long)t * a.nrec + rr] =
+          c.rowbuf_()[(off / g.pitch - c.rj0) * kRegW + (off % g.pitch - c.ri0)];
+    }
+
+    // ---- stages 2-3: H update + H CPML -------------------------------------------------------------
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      float eb[4];                                      // Ez of the row below
+      if (r + 1 < R) { eb[0] = e[r + 1][0]; eb[1] = e[r + 1][1]; eb[2] = e[r + 1][2]; eb[3] = e[r + 1][3]; }
+      else lds4a(c.xe_() + (c.w + 1) * kRegW + c.l4, eb);
+      const float en[4] = {e[r][1], e[r][2], e[r][3], __shfl_down_sync(full, e[r][0], 1)};   // Ez to the right
+      if ((c.zsH >> r) & 1u) {
+        float p[4];
+        lds4a(c.phz_() + r * kRegW, p);
+        const float b = c.tabz_()[0 * L::ROWS + c.lr0 + r], cc = c.tabz_()[1 * L::ROWS + c.lr0 + r],
+                    ik = c.tabz_()[2 * L::ROWS + c.lr0 + r];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const float d = FM(FS(eb[q], e[r][q]), rdx);
+          p[q] = FF(b, p[q], FM(cc, d));
+          hx[r][q] = FF(-Db, FF(d, ik, p[q]), hx[r][q]);
+        }
+        st4a(c.phz_() + r * kRegW, p);
+      } else {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) hx[r][q] = FF(-kap, FS(eb[q], e[r][q]), hx[r][q]);
+      }
+      if (c.xsH) {
+        float p[4], b[4], cc[4], ik[4];
+        lds4a(c.phx_() + r * kRegW, p);
+        lds4a(c.tabx_() + 0 * kRegW + c.l4, b); lds4a(c.tabx_() + 1 * kRegW + c.l4, cc); lds4a(c.tabx_() + 2 * kRegW + c.l4, ik);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if ((c.xsH >> q) & 1u) {
+            const float d = FM(FS(en[q], e[r][q]), rdx);
+            p[q] = FF(b[q], p[q], FM(cc[q], d));
+            hy[r][q] = FF(Db, FF(d, ik[q], p[q]), hy[r][q]);
+          } else {
+            hy[r][q] = FF(kap, FS(en[q], e[r][q]), hy[r][q]);
+          }
+        }
+        st4a(c.phx_() + r * kRegW, p);
+      } else {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) hy[r][q] = FF(kap, FS(en[q], e[r][q]), hy[r][q]);
+      }
+    }
+    st4a(c.xh_() + (c.w + 1) * kRegW + c.l4, hx[R - 1]);
+    __syncthreads();
+
+    // ---- stages 4-7: E update + E CPML, source, save wavefield --------------------------------------
+    float* ez_out = (t + 1 == a.nsub) ? a.out.ez : a.ez_hist[t + 1];
+    const float wn = a.wavelet[s * a.wav_stride + t] * (rdx * rdx);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      float ha[4];                                      // Hx of the row above
+      if (r > 0) { ha[0] = hx[r - 1][0]; ha[1] = hx[r - 1][1]; ha[2] = hx[r - 1][2]; ha[3] = hx[r - 1][3]; }
+      else lds4a(c.xh_() + c.w * kRegW + c.l4, ha);
+      const float hl[4] = {__shfl_up_sync(full, hy[r][3], 1), hy[r][0], hy[r][1], hy[r][2]};  // Hy to the left
+      const bool zs = (c.zsE >> r) & 1u;
+      if (zs || c.xsE) {
+        float pz[4], px[4], bx[4], cx[4], kx[4];
+        float bz = 0.f, cz = 0.f, kz = 1.f;
+        if (zs) {
+          lds4a(c.pez_() + r * kRegW, pz);
+          bz = c.tabz_()[3 * L::ROWS + c.lr0 + r]; cz = c.tabz_()[4 * L::ROWS + c.lr0 + r]; kz = c.tabz_()[5 * L::ROWS + c.lr0 + r];
+        }
+        if (c.xsE) {
+          lds4a(c.pex_() + r * kRegW, px);
+          lds4a(c.tabx_() + 3 * kRegW + c.l4, bx); lds4a(c.tabx_() + 4 * kRegW + c.l4, cx); lds4a(c.tabx_() + 5 * kRegW + c.l4, kx);
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const bool xs = (c.xsE >> q) & 1u;
+          if (!zs && !xs) {
+            e[r][q] = FF(cb[r][q], FM(FS(FS(hy[r][q], hl[q]), FS(hx[r][q], ha[q])), rdx), FM(ca[r][q], e[r][q]));
+          } else {
+            float vx = FM(FS(hy[r][q], hl[q]), rdx), vz = FM(FS(hx[r][q], ha[q]), rdx);
+            if (xs) { px[q] = FF(bx[q], px[q], FM(cx[q], vx)); vx = FF(vx, kx[q], px[q]); }
+            if (zs) { pz[q] = FF(bz, pz[q], FM(cz, vz)); vz = FF(vz, kz, pz[q]); }
+            e[r][q] = FF(cb[r][q], FS(vx, vz), FM(ca[r][q], e[r][q]));
+          }
+        }
+        if (zs) st4a(c.pez_() + r * kRegW, pz);
+        if (c.xsE) st4a(c.pex_() + r * kRegW, px);
+      } else {
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          e[r][q] = FF(cb[r][q], FM(FS(FS(hy[r][q], hl[q]), FS(hx[r][q], ha[q])), rdx), FM(ca[r][q], e[r][q]));
+      }
+      if (r == src_r) {                                 // every CTA whose region holds the source injects
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          if (q == src_c) e[r][q] = FF(-cb[r][q], wn, e[r][q]);
+      }
+      if (ez_out && ((c.own >> r) & 1u)) stcs4a(ez_out + s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi, e[r]);
+      if ((rflags >> r) & 1u) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
+    }
+    st4a(c.xe_() + c.w * kRegW + c.l4, e[0]);
+    __syncthreads();
+  }
+
+  // ---- write back what this tile owns (out.ez was written by the last E phase) ----------------------
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    if (!((c.own >> r) & 1u)) continue;
+    const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
+    st4a(a.out.hx + o, hx[r]);
+    st4a(a.out.hy + o, hy[r]);
+  }
+  c.store_psi(g, a.out, s);
+}
+#endif
+
+}  // namespace gprfwi

@@ -37,7 +37,10 @@ __global__ void coef_kernel(const float* __restrict__ eps_r, const float* __rest
   const int j = blockIdx.y;
   if (i >= pitch || j >= nz) return;
   float a = 0.f, b = 0.f;
-  if (i < nx) coef_cell(eps_r[(long long)j * upitch + i], sigma[(long long)j * upitch + i], rdt, a, b);
+  // the PEC ring (never updated, reading R5) and the pitch padding carry Ca = Cb = 0: the update
+  // kernels then keep those nodes at zero without any bounds test
+  if (i >= 1 && i <= nx - 2 && j >= 1 && j <= nz - 2)
+    coef_cell(eps_r[(long long)j * upitch + i], sigma[(long long)j * upitch + i], rdt, a, b);
   ca[(long long)j * pitch + i] = a;
   cb[(long long)j * pitch + i] = b;
 }

@@ -1,0 +1,202 @@
+// gprfwi_tile.cuh -- the register tile shared by the forward and adjoint kernels of libgprfwi.
+//
+// A CTA of NW warps works on a REGION of NW*R rows x 128 columns of one shot: warp w holds rows
+// [w*R, w*R + R), lane l holds columns [4l, 4l + 4) of each of them, as float4 REGISTERS for the
+// whole launch (up to T = 4 leap-frog steps).  Nothing of the three fields lives in shared memory:
+//   x neighbours   come from the adjacent lane by warp shuffle,
+//   z neighbours   inside a warp's R rows are the thread's own registers; across warps ONE row per
+//                  warp per phase goes through a 512-byte shared-memory exchange slot.
+// The region is the owned tile (NW*R - 2*hz rows x 120 columns) plus a halo of hz rows / 4 columns
+// that is recomputed redundantly instead of exchanged between CTAs: after t steps the outermost t
+// rings of the region are stale (they have seen the garbage beyond the region edge), which is why
+// the halo is as deep as the number of fused steps.  State is ping-ponged between launches, so CTAs
+// never race.  Cells outside the grid are loaded as 0 and stay 0 by themselves (masked Ca = Cb = 0
+// there and on the PEC ring), so no update needs a bounds test.
+//
+// Shared memory (floats), per CTA:
+//   xe   [NW+1][128]  exchange slot A: row 0 of warp w (forward: Ez, adjoint: tz); slot NW stays 0
+//   xh   [NW+1][128]  exchange slot B: row R-1 of warp w in slot w+1 (forward: Hx, adjoint: sz); slot 0 stays 0
+//   rowbuf [NW*R][128] rows that hold receivers: forward publishes Ez there for the trace gather,
+//                     the adjoint stages the residual there for injection
+//   tabx [6][128]     CPML x tables of the region's columns: bhx chx khx bex cex kex
+//   tabz [6][NW*R]    CPML z tables of the region's rows:    bhz chz khz bez cez kez
+//   psi  [4][NW*R][128]  CPML psi of the region, thread-private (only when npml > 0): hz ez hx ex
+#pragma once
+#include "gprfwi_common.cuh"
+
+namespace gprfwi {
+
+constexpr int kMaxT = 4;       // fused steps per launch <= x halo (4 columns = one float4)
+constexpr int kRegW = 128;     // region width  = 32 lanes x float4
+constexpr int kOwnW = 120;     // owned width   = lanes 1..30
+
+template <int R, int NW>
+struct RegTile {
+  static constexpr int ROWS = R * NW;
+  static constexpr int THREADS = NW * 32;
+  static constexpr int XE = 0;
+  static constexpr int XH = XE + (NW + 1) * kRegW;
+  static constexpr int ROWBUF = XH + (NW + 1) * kRegW;
+  static constexpr int TABX = ROWBUF + ROWS * kRegW;
+  static constexpr int TABZ = TABX + 6 * kRegW;
+  static constexpr int PSI = (TABZ + 6 * ROWS + 3) / 4 * 4;
+  GPR_HD static size_t smem_bytes(bool pml) { return sizeof(float) * (size_t)(PSI + (pml ? 4 * ROWS * kRegW : 0)); }
+};
+
+#if defined(__CUDACC__)
+// exactly rounded, never contracted: every cell's arithmetic is the same whichever CTA computes it
+__device__ __forceinline__ float FM(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float FS(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float FA(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float FF(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+
+__device__ __forceinline__ void ldg4a(const float* p, float* o)
+{
+  const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+  o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+}
+__device__ __forceinline__ void ldcs4a(const float* p, float* o)      // streaming (evict-first) load
+{
+  const float4 v = __ldcs(reinterpret_cast<const float4*>(p));
+  o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+}
+__device__ __forceinline__ void lds4a(const float* p, float* o)
+{
+  const float4 v = *reinterpret_cast<const float4*>(p);
+  o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+}
+__device__ __forceinline__ void st4a(float* p, const float* v)
+{
+  *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+}
+__device__ __forceinline__ void stcs4a(float* p, const float* v)      // streaming (evict-first) store
+{
+  __stcs(reinterpret_cast<float4*>(p), make_float4(v[0], v[1], v[2], v[3]));
+}
+__device__ __forceinline__ void zero4(float* v) { v[0] = v[1] = v[2] = v[3] = 0.f; }
+
+// Per-thread view of the region: where this lane's 4 columns and this warp's R rows sit in the grid,
+// which of them carry CPML psi, and the shared-memory carve-up.
+template <int R, int NW>
+struct TileCtx {
+  using L = RegTile<R, NW>;
+  float* sm;            // shared-memory base; every array is a compile-time offset from it
+  int toff;             // lr0 * 128 + l4: this thread's row-0 slot inside a [ROWS][128] array
+  int lane, w, l4, lr0;
+  int gj0, gi;          // grid row of this warp's row 0, grid column of this lane's component 0
+  int rj0, ri0;         // grid row / column of the region's origin
+  bool colin;           // the lane's float4 lies inside [0, pitch)
+  unsigned xsH, xsE;    // bit c: column gi + c carries H- / E-located x psi
+  unsigned zsH, zsE;    // bit r: row gj0 + r carries H- / E-located z psi (warp-uniform)
+  unsigned rin;         // bit r: row inside the grid (warp-uniform)
+  unsigned own;         // bit r: row owned by this tile (and inside the grid); 0 for lanes 0 and 31
+
+  __device__ __forceinline__ float* xe_() const { return sm + L::XE; }
+  __device__ __forceinline__ float* xh_() const { return sm + L::XH; }
+  __device__ __forceinline__ float* rowbuf_() const { return sm + L::ROWBUF; }
+  __device__ __forceinline__ float* tabx_() const { return sm + L::TABX; }
+  __device__ __forceinline__ float* tabz_() const { return sm + L::TABZ; }
+  __device__ __forceinline__ float* phz_() const { return sm + L::PSI + 0 * L::ROWS * kRegW + toff; }
+  __device__ __forceinline__ float* pez_() const { return sm + L::PSI + 1 * L::ROWS * kRegW + toff; }
+  __device__ __forceinline__ float* phx_() const { return sm + L::PSI + 2 * L::ROWS * kRegW + toff; }
+  __device__ __forceinline__ float* pex_() const { return sm + L::PSI + 3 * L::ROWS * kRegW + toff; }
+
+  __device__ __forceinline__ void init(float* sm_, const Geo& g, int tile_x, int tile_y, int oz, int hz)
+  {
+    lane = threadIdx.x & 31; w = threadIdx.x >> 5; l4 = lane * 4; lr0 = w * R;
+    rj0 = tile_y * oz - hz; ri0 = tile_x * kOwnW - 4;
+    gj0 = rj0 + lr0; gi = ri0 + l4;
+    sm = sm_; toff = lr0 * kRegW + l4;
+    colin = gi >= 0 && gi < g.pitch;
+    xsH = xsE = zsH = zsE = rin = own = 0u;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      if (g.P > 0 && strip_h(gi + c, g.nx, g.P) >= 0) xsH |= 1u << c;
+      if (g.P > 0 && strip_e(gi + c, g.nx, g.P) >= 0) xsE |= 1u << c;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int gj = gj0 + r;
+      if (gj >= 0 && gj < g.nz) {
+        rin |= 1u << r;
+        if (g.P > 0 && strip_h(gj, g.nz, g.P) >= 0) zsH |= 1u << r;
+        if (g.P > 0 && strip_e(gj, g.nz, g.P) >= 0) zsE |= 1u << r;
+        if (lr0 + r >= hz && lr0 + r < L::ROWS - hz && lane >= 1 && lane <= 30 && colin) own |= 1u << r;
+      }
+    }
+  }
+
+  // CPML tables of the region's rows and columns -> shared memory (outside the grid: b = c = 0, 1/kappa = 1)
+  __device__ __forceinline__ void stage_tables(const Geo& g) const
+  {
+    if (w == 0) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int i = gi + c;
+        const bool in = i >= 0 && i < g.nx;
+        tabx_()[0 * kRegW + l4 + c] = in ? g.bhx[i] : 0.f; tabx_()[1 * kRegW + l4 + c] = in ? g.chx[i] : 0.f;
+        tabx_()[2 * kRegW + l4 + c] = in ? g.khx[i] : 1.f; tabx_()[3 * kRegW + l4 + c] = in ? g.bex[i] : 0.f;
+        tabx_()[4 * kRegW + l4 + c] = in ? g.cex[i] : 0.f; tabx_()[5 * kRegW + l4 + c] = in ? g.kex[i] : 1.f;
+      }
+    }
+    for (int k = threadIdx.x; k < L::ROWS; k += L::THREADS) {
+      const int gj = rj0 + k;
+      const bool in = gj >= 0 && gj < g.nz;
+      tabz_()[0 * L::ROWS + k] = in ? g.bhz[gj] : 0.f; tabz_()[1 * L::ROWS + k] = in ? g.chz[gj] : 0.f;
+      tabz_()[2 * L::ROWS + k] = in ? g.khz[gj] : 1.f; tabz_()[3 * L::ROWS + k] = in ? g.bez[gj] : 0.f;
+      tabz_()[4 * L::ROWS + k] = in ? g.cez[gj] : 0.f; tabz_()[5 * L::ROWS + k] = in ? g.kez[gj] : 1.f;
+    }
+    // the two exchange slots nobody publishes: below the last warp, above the first
+    if (w == NW - 1) *reinterpret_cast<float4*>(xe_() + NW * kRegW + l4) = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (w == 0) *reinterpret_cast<float4*>(xh_() + l4) = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+
+  // psi strips of shot s -> the thread's shared-memory slots (all four arrays, zero where no psi lives)
+  __device__ __forceinline__ void load_psi(const Geo& g, const State& st, int s) const
+  {
+    if (g.P <= 0) return;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int gj = gj0 + r;
+      const bool in = colin && ((rin >> r) & 1u);
+      float a[4], b[4], c[4], d[4];
+      zero4(a); zero4(b); zero4(c); zero4(d);
+      if (in && ((zsH >> r) & 1u)) ldg4a(st.phxz + s * g.zstrip + (long long)strip_h(gj, g.nz, g.P) * g.pitch + gi, a);
+      if (in && ((zsE >> r) & 1u)) ldg4a(st.pezz + s * g.zstrip + (long long)strip_e(gj, g.nz, g.P) * g.pitch + gi, b);
+      if (in && (xsH | xsE)) {
+        const long long po = s * g.xstrip + (long long)gj * g.xw;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if ((xsH >> q) & 1u) c[q] = __ldg(st.phyx + po + strip_h(gi + q, g.nx, g.P));
+          if ((xsE >> q) & 1u) d[q] = __ldg(st.pezx + po + strip_e(gi + q, g.nx, g.P));
+        }
+      }
+      st4a(phz_() + r * kRegW, a); st4a(pez_() + r * kRegW, b); st4a(phx_() + r * kRegW, c); st4a(pex_() + r * kRegW, d);
+    }
+  }
+
+  // owned psi -> the output state
+  __device__ __forceinline__ void store_psi(const Geo& g, const State& st, int s) const
+  {
+    if (g.P <= 0) return;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      if (!((own >> r) & 1u)) continue;
+      const int gj = gj0 + r;
+      float v[4];
+      if ((zsH >> r) & 1u) { lds4a(phz_() + r * kRegW, v); st4a(st.phxz + s * g.zstrip + (long long)strip_h(gj, g.nz, g.P) * g.pitch + gi, v); }
+      if ((zsE >> r) & 1u) { lds4a(pez_() + r * kRegW, v); st4a(st.pezz + s * g.zstrip + (long long)strip_e(gj, g.nz, g.P) * g.pitch + gi, v); }
+      if (xsH | xsE) {
+        const long long po = s * g.xstrip + (long long)gj * g.xw;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if ((xsH >> q) & 1u) st.phyx[po + strip_h(gi + q, g.nx, g.P)] = phx_()[r * kRegW + q];
+          if ((xsE >> q) & 1u) st.pezx[po + strip_e(gi + q, g.nx, g.P)] = pex_()[r * kRegW + q];
+        }
+      }
+    }
+  }
+};
+#endif
+
+}  // namespace gprfwi
