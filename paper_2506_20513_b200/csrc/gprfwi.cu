@@ -60,7 +60,7 @@ struct Tiling {
 
 struct Layout {
   // geometry-derived sizes (floats)
-  int pitch = 0, xw = 0;
+  int pitch = 0, xw = 0, xnl = 0, xur = 0;
   size_t plane = 0, zstrip = 0, xstrip = 0;
   size_t hslot = 0;        // Hx, Hy, 4 psi strips of ONE shot
   size_t full = 0;         // hslot + Ez plane
@@ -93,7 +93,9 @@ static int validate(const gprfwi_params* p)
 static void base_layout(const gprfwi_params* p, Layout& L)
 {
   L.pitch = (int)align_up((size_t)p->nx, 32);
-  L.xw = (int)align_up((size_t)2 * p->npml, 4);
+  L.xnl = (p->npml + 3) / 4;                                     // x-strip layout: gprfwi_common.cuh
+  L.xur = p->npml > 0 ? (p->nx - 1 - p->npml) / 4 : L.pitch / 4;
+  L.xw = 4 * (L.xnl + L.pitch / 4 - L.xur);
   L.plane = (size_t)p->nz * L.pitch;
   L.zstrip = (size_t)2 * p->npml * L.pitch;
   L.xstrip = (size_t)p->nz * L.xw;
@@ -354,7 +356,7 @@ static int upload_static(gprfwi_handle* h, cudaStream_t st)
   GPR_CUDA(cudaMemcpyAsync(h->c.reg_rec, h->h_reg_rec.data(), h->h_reg_rec.size() * sizeof(int),
                            cudaMemcpyHostToDevice, st));
   Geo& g = h->geo;
-  g.nz = p.nz; g.nx = p.nx; g.P = p.npml; g.pitch = L.pitch; g.xw = L.xw;
+  g.nz = p.nz; g.nx = p.nx; g.P = p.npml; g.pitch = L.pitch; g.xw = L.xw; g.xnl = L.xnl; g.xur = L.xur;
   g.plane = (long long)L.plane; g.zstrip = (long long)L.zstrip; g.xstrip = (long long)L.xstrip;
   g.rdx = (float)(1.0 / (double)p.dx);
   g.Db = (float)((double)p.dt / kMu0);

@@ -38,6 +38,176 @@ struct AdjArgs {
 };
 
 #if defined(__CUDACC__)
+// transpose of recording: residual sample n_hi - t enters lamE at the start of reverse step n_hi-1-t;
+// it is staged in rowbuf (zero between uses) one barrier ahead of its use
+template <int R, int NW>
+__device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW>& c, int s, int rk0, int rk1, int t)
+{
+  using L = RegTile<R, NW>;
+  if (a.n_hi - t >= a.nt) return;
+  for (int k = rk0 + threadIdx.x; k < rk1; k += L::THREADS) {
+    const int rr = a.reg_rec[k];
+    const int off = a.rec_off[(long long)s * a.nrec + rr];
+    atomicAdd(c.rowbuf_() + (off / a.g.pitch - c.rj0) * kRegW + (off % a.g.pitch - c.ri0),   // coincident receivers sum
+              a.residual[s * a.trace_stride - (long long)t * a.nrec + rr]);
+  }
+}
+
+// The T reverse steps of one warp for one shot; PML as in fwd_steps.
+template <int R, int NW, bool PML>
+__device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW>& c, int s, int rk0, int rk1,
+                                          unsigned iflags, float (&le)[R][4], float (&lhx)[R][4], float (&lhy)[R][4],
+                                          const float (&ca)[R][4], const float (&cb)[R][4],
+                                          float (&ga)[R][4], float (&gb)[R][4])
+{
+  using L = RegTile<R, NW>;
+  const Geo& g = a.g;
+  const unsigned full = 0xffffffffu;
+  const float rdx = g.rdx, Db = g.Db;
+  #pragma unroll 1
+  for (int t = 0; t < a.nsub; ++t) {
+    // ---- [A] adjoint source, gradient terms ------------------------------------------------------
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      if ((iflags >> r) & 1u) {
+        float v[4];
+        float* rb = c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4;
+        lds4a(rb, v);
+        le[r][0] = FA(le[r][0], v[0]); le[r][1] = FA(le[r][1], v[1]);
+        le[r][2] = FA(le[r][2], v[2]); le[r][3] = FA(le[r][3], v[3]);
+        zero4(v);
+        st4a(rb, v);
+      }
+      if ((c.own >> r) & 1u) {
+        const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
+        float e0[4], e1[4];
+        ldcs4a(a.ez_planes[t + 1] + o, e0);          // E^n
+        ldcs4a(a.ez_planes[t] + o, e1);              // E^{n+1}
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          ga[r][q] = FF(le[r][q], e0[q], ga[r][q]);
+          gb[r][q] = FF(le[r][q], FF(-ca[r][q], e0[q], e1[q]), gb[r][q]);
+        }
+      }
+    }
+    // ---- [B] transpose of the E update + E CPML ----------------------------------------------------
+    float tzp[4], tz0[4];                             // tz of the previous row; of the warp's row R-1
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      float tx[4], tz[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const float qv = FM(cb[r][q], le[r][q]);
+        tx[q] = qv; tz[q] = -qv;
+        le[r][q] = FM(ca[r][q], le[r][q]);
+      }
+      if (PML && ((c.zsE >> r) & 1u)) {
+        float p[4];
+        lds4a(c.pez_() + r * kRegW, p);
+        const float b = c.tabz_()[3 * L::ROWS + c.lr0 + r], cc = c.tabz_()[4 * L::ROWS + c.lr0 + r],
+                    ik = c.tabz_()[5 * L::ROWS + c.lr0 + r];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const float T_ = FA(p[q], tz[q]);           // psiEz - q
+          tz[q] = FF(cc, T_, FM(tz[q], ik));
+          p[q] = FM(b, T_);
+        }
+        st4a(c.pez_() + r * kRegW, p);
+      }
+      if (PML && c.xsE) {
+        float p[4], b[4], cc[4], ik[4];
+        lds4a(c.pex_() + r * kRegW, p);
+        lds4a(c.tabx_() + 3 * kRegW + c.l4, b); lds4a(c.tabx_() + 4 * kRegW + c.l4, cc); lds4a(c.tabx_() + 5 * kRegW + c.l4, ik);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if ((c.xsE >> q) & 1u) {
+            const float T_ = FA(p[q], tx[q]);         // psiEx + q
+            tx[q] = FF(cc[q], T_, FM(tx[q], ik[q]));
+            p[q] = FM(b[q], T_);
+          }
+        }
+        st4a(c.pex_() + r * kRegW, p);
+      }
+      const float txn[4] = {tx[1], tx[2], tx[3], __shfl_down_sync(full, tx[0], 1)};     // tx to the right
+#pragma unroll
+      for (int q = 0; q < 4; ++q) lhy[r][q] = FF(rdx, FS(tx[q], txn[q]), lhy[r][q]);
+      if (r == 0) st4a(c.xe_() + c.w * kRegW + c.l4, tz);
+      else {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) lhx[r - 1][q] = FF(rdx, FS(tzp[q], tz[q]), lhx[r - 1][q]);
+      }
+#pragma unroll
+      for (int q = 0; q < 4; ++q) tzp[q] = tz[q];
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) tz0[q] = tzp[q];
+    __syncthreads();
+    if (t + 1 < a.nsub) adj_stage<R, NW>(a, c, s, rk0, rk1, t + 1);
+    {
+      float tzb[4];                                   // tz of the row below the warp's last row
+      lds4a(c.xe_() + (c.w + 1) * kRegW + c.l4, tzb);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) lhx[R - 1][q] = FF(rdx, FS(tz0[q], tzb[q]), lhx[R - 1][q]);
+    }
+    // ---- [C] transpose of the H update + H CPML ----------------------------------------------------
+    float szp[4], sz0[4];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      float sx[4], sz[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) { sz[q] = FM(-Db, lhx[r][q]); sx[q] = FM(Db, lhy[r][q]); }
+      if (PML && ((c.zsH >> r) & 1u)) {
+        float p[4];
+        lds4a(c.phz_() + r * kRegW, p);
+        const float b = c.tabz_()[0 * L::ROWS + c.lr0 + r], cc = c.tabz_()[1 * L::ROWS + c.lr0 + r],
+                    ik = c.tabz_()[2 * L::ROWS + c.lr0 + r];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const float T_ = FA(p[q], sz[q]);
+          sz[q] = FF(cc, T_, FM(sz[q], ik));
+          p[q] = FM(b, T_);
+        }
+        st4a(c.phz_() + r * kRegW, p);
+      }
+      if (PML && c.xsH) {
+        float p[4], b[4], cc[4], ik[4];
+        lds4a(c.phx_() + r * kRegW, p);
+        lds4a(c.tabx_() + 0 * kRegW + c.l4, b); lds4a(c.tabx_() + 1 * kRegW + c.l4, cc); lds4a(c.tabx_() + 2 * kRegW + c.l4, ik);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if ((c.xsH >> q) & 1u) {
+            const float T_ = FA(p[q], sx[q]);
+            sx[q] = FF(cc[q], T_, FM(sx[q], ik[q]));
+            p[q] = FM(b[q], T_);
+          }
+        }
+        st4a(c.phx_() + r * kRegW, p);
+      }
+      const float sxl[4] = {__shfl_up_sync(full, sx[3], 1), sx[0], sx[1], sx[2]};       // sx to the left
+#pragma unroll
+      for (int q = 0; q < 4; ++q) le[r][q] = FF(rdx, FS(sxl[q], sx[q]), le[r][q]);
+      if (r == 0) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) sz0[q] = sz[q];
+      } else {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) le[r][q] = FF(rdx, FS(szp[q], sz[q]), le[r][q]);
+      }
+      if (r == R - 1) st4a(c.xh_() + (c.w + 1) * kRegW + c.l4, sz);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) szp[q] = sz[q];
+    }
+    __syncthreads();
+    {
+      float sza[4];                                   // sz of the row above the warp's first row
+      lds4a(c.xh_() + c.w * kRegW + c.l4, sza);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) le[0][q] = FF(rdx, FS(sza[q], sz0[q]), le[0][q]);
+    }
+  }
+
+}
+
 template <int R, int NW, int MINB>
 __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
 {
@@ -48,9 +218,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
   const int grp = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
   const unsigned full = 0xffffffffu;
-  const float rdx = g.rdx, Db = g.Db;
 
   c.stage_tables(g);
+  const bool pml = __any_sync(full, (c.zsH | c.zsE | c.xsH | c.xsE) != 0u);    // warp-uniform
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
     reinterpret_cast<float4*>(c.rowbuf_())[k] = make_float4(0.f, 0.f, 0.f, 0.f);
 
@@ -77,17 +247,6 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
       if (lj >= 0 && lj < R) iflags |= 1u << lj;
     }
     iflags = __reduce_or_sync(full, iflags);
-    // transpose of recording: residual sample n_hi - t enters lamE at the start of reverse step n_hi-1-t
-    auto stage = [&](int t) {
-      if (a.n_hi - t >= a.nt) return;
-      for (int k = rk0 + threadIdx.x; k < rk1; k += L::THREADS) {
-        const int rr = a.reg_rec[k];
-        const int off = a.rec_off[(long long)s * a.nrec + rr];
-        atomicAdd(c.rowbuf_() + (off / g.pitch - c.rj0) * kRegW + (off % g.pitch - c.ri0),   // coincident receivers sum
-                  a.residual[s * a.trace_stride - (long long)t * a.nrec + rr]);
-      }
-    };
-
     float le[R][4], lhx[R][4], lhy[R][4];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -99,150 +258,12 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
         ldg4a(a.in.hy + o, lhy[r]);
       }
     }
-    c.load_psi(g, a.in, s);
-    stage(0);
+    if (pml) c.load_psi(g, a.in, s);
+    adj_stage<R, NW>(a, c, s, rk0, rk1, 0);
     __syncthreads();
 
-    for (int t = 0; t < a.nsub; ++t) {
-      // ---- [A] adjoint source, gradient terms ------------------------------------------------------
-#pragma unroll
-      for (int r = 0; r < R; ++r) {
-        if ((iflags >> r) & 1u) {
-          float v[4];
-          float* rb = c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4;
-          lds4a(rb, v);
-          le[r][0] = FA(le[r][0], v[0]); le[r][1] = FA(le[r][1], v[1]);
-          le[r][2] = FA(le[r][2], v[2]); le[r][3] = FA(le[r][3], v[3]);
-          zero4(v);
-          st4a(rb, v);
-        }
-        if ((c.own >> r) & 1u) {
-          const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-          float e0[4], e1[4];
-          ldcs4a(a.ez_planes[t + 1] + o, e0);          // E^n
-          ldcs4a(a.ez_planes[t] + o, e1);              // E^{n+1}
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            ga[r][q] = FF(le[r][q], e0[q], ga[r][q]);
-            gb[r][q] = FF(le[r][q], FF(-ca[r][q], e0[q], e1[q]), gb[r][q]);
-          }
-        }
-      }
-      // ---- [B] transpose of the E update + E CPML ----------------------------------------------------
-      float tzp[4], tz0[4];                             // tz of the previous row; of the warp's row R-1
-#pragma unroll
-      for (int r = 0; r < R; ++r) {
-        float tx[4], tz[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const float qv = FM(cb[r][q], le[r][q]);
-          tx[q] = qv; tz[q] = -qv;
-          le[r][q] = FM(ca[r][q], le[r][q]);
-        }
-        if ((c.zsE >> r) & 1u) {
-          float p[4];
-          lds4a(c.pez_() + r * kRegW, p);
-          const float b = c.tabz_()[3 * L::ROWS + c.lr0 + r], cc = c.tabz_()[4 * L::ROWS + c.lr0 + r],
-                      ik = c.tabz_()[5 * L::ROWS + c.lr0 + r];
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const float T_ = FA(p[q], tz[q]);           // psiEz - q
-            tz[q] = FF(cc, T_, FM(tz[q], ik));
-            p[q] = FM(b, T_);
-          }
-          st4a(c.pez_() + r * kRegW, p);
-        }
-        if (c.xsE) {
-          float p[4], b[4], cc[4], ik[4];
-          lds4a(c.pex_() + r * kRegW, p);
-          lds4a(c.tabx_() + 3 * kRegW + c.l4, b); lds4a(c.tabx_() + 4 * kRegW + c.l4, cc); lds4a(c.tabx_() + 5 * kRegW + c.l4, ik);
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            if ((c.xsE >> q) & 1u) {
-              const float T_ = FA(p[q], tx[q]);         // psiEx + q
-              tx[q] = FF(cc[q], T_, FM(tx[q], ik[q]));
-              p[q] = FM(b[q], T_);
-            }
-          }
-          st4a(c.pex_() + r * kRegW, p);
-        }
-        const float txn[4] = {tx[1], tx[2], tx[3], __shfl_down_sync(full, tx[0], 1)};     // tx to the right
-#pragma unroll
-        for (int q = 0; q < 4; ++q) lhy[r][q] = FF(rdx, FS(tx[q], txn[q]), lhy[r][q]);
-        if (r == 0) st4a(c.xe_() + c.w * kRegW + c.l4, tz);
-        else {
-#pragma unroll
-          for (int q = 0; q < 4; ++q) lhx[r - 1][q] = FF(rdx, FS(tzp[q], tz[q]), lhx[r - 1][q]);
-        }
-#pragma unroll
-        for (int q = 0; q < 4; ++q) tzp[q] = tz[q];
-      }
-#pragma unroll
-      for (int q = 0; q < 4; ++q) tz0[q] = tzp[q];
-      __syncthreads();
-      if (t + 1 < a.nsub) stage(t + 1);
-      {
-        float tzb[4];                                   // tz of the row below the warp's last row
-        lds4a(c.xe_() + (c.w + 1) * kRegW + c.l4, tzb);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) lhx[R - 1][q] = FF(rdx, FS(tz0[q], tzb[q]), lhx[R - 1][q]);
-      }
-      // ---- [C] transpose of the H update + H CPML ----------------------------------------------------
-      float szp[4], sz0[4];
-#pragma unroll
-      for (int r = 0; r < R; ++r) {
-        float sx[4], sz[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) { sz[q] = FM(-Db, lhx[r][q]); sx[q] = FM(Db, lhy[r][q]); }
-        if ((c.zsH >> r) & 1u) {
-          float p[4];
-          lds4a(c.phz_() + r * kRegW, p);
-          const float b = c.tabz_()[0 * L::ROWS + c.lr0 + r], cc = c.tabz_()[1 * L::ROWS + c.lr0 + r],
-                      ik = c.tabz_()[2 * L::ROWS + c.lr0 + r];
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const float T_ = FA(p[q], sz[q]);
-            sz[q] = FF(cc, T_, FM(sz[q], ik));
-            p[q] = FM(b, T_);
-          }
-          st4a(c.phz_() + r * kRegW, p);
-        }
-        if (c.xsH) {
-          float p[4], b[4], cc[4], ik[4];
-          lds4a(c.phx_() + r * kRegW, p);
-          lds4a(c.tabx_() + 0 * kRegW + c.l4, b); lds4a(c.tabx_() + 1 * kRegW + c.l4, cc); lds4a(c.tabx_() + 2 * kRegW + c.l4, ik);
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            if ((c.xsH >> q) & 1u) {
-              const float T_ = FA(p[q], sx[q]);
-              sx[q] = FF(cc[q], T_, FM(sx[q], ik[q]));
-              p[q] = FM(b[q], T_);
-            }
-          }
-          st4a(c.phx_() + r * kRegW, p);
-        }
-        const float sxl[4] = {__shfl_up_sync(full, sx[3], 1), sx[0], sx[1], sx[2]};       // sx to the left
-#pragma unroll
-        for (int q = 0; q < 4; ++q) le[r][q] = FF(rdx, FS(sxl[q], sx[q]), le[r][q]);
-        if (r == 0) {
-#pragma unroll
-          for (int q = 0; q < 4; ++q) sz0[q] = sz[q];
-        } else {
-#pragma unroll
-          for (int q = 0; q < 4; ++q) le[r][q] = FF(rdx, FS(szp[q], sz[q]), le[r][q]);
-        }
-        if (r == R - 1) st4a(c.xh_() + (c.w + 1) * kRegW + c.l4, sz);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) szp[q] = sz[q];
-      }
-      __syncthreads();
-      {
-        float sza[4];                                   // sz of the row above the warp's first row
-        lds4a(c.xh_() + c.w * kRegW + c.l4, sza);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) le[0][q] = FF(rdx, FS(sza[q], sz0[q]), le[0][q]);
-      }
-    }
+    if (pml) adj_steps<R, NW, true>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    else adj_steps<R, NW, false>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
 
     // ---- write back the owned part of the adjoint state ------------------------------------------------
 #pragma unroll
@@ -253,7 +274,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
       st4a(a.out.hx + o, lhx[r]);
       st4a(a.out.hy + o, lhy[r]);
     }
-    c.store_psi(g, a.out, s);
+    if (pml) c.store_psi(g, a.out, s);
   }
 
   // ---- once per CTA: add the register partial sums to this group's gCa / gCb planes --------------------

@@ -5,7 +5,8 @@
 //                 Ez at (j,i); Hx at (j+1/2,i) (row nz-1 unused, kept 0); Hy at (j,i+1/2)
 //                 (column nx-1 unused, kept 0); columns [nx, roundup4(nx)) are written as 0.
 //   z-strips      [S][2P][pitch]     CPML psi of the z-derivative, only the 2P rows where it lives
-//   x-strips      [S][nz][xw]        CPML psi of the x-derivative, only the 2P columns (xw = roundup4(2P))
+//   x-strips      [S][nz][xw]        CPML psi of the x-derivative, only the float4 units of a row that
+//                                    touch the left / right CPML: units [0, xnl) then [xur, pitch/4)
 //   Ca, Cb        [nz][pitch]        shared by all shots
 //   1-D CPML tables (b, c, 1/kappa) per axis and per E/H location, built on the host in float64.
 #pragma once
@@ -23,7 +24,8 @@ namespace gprfwi {
 struct Geo {
   int nz, nx, P;        // full grid, CPML thickness
   int pitch;            // internal row pitch in floats
-  int xw;               // x-strip row width in floats
+  int xw;               // x-strip row width in floats = 4 * (xnl + pitch/4 - xur)
+  int xnl, xur;         // float4 units [0, xnl) hold the left CPML columns, units [xur, pitch/4) the right ones
   long long plane;      // nz * pitch
   long long zstrip;     // 2P * pitch   (per shot)
   long long xstrip;     // nz * xw      (per shot)
@@ -54,14 +56,15 @@ GPR_HD int strip_h(int i, int n, int P)
   return i < P ? i : ((i >= n - 1 - P && i < n - 1) ? i - (n - 1 - P) + P : -1);
 }
 
+// float offset of float4 unit u (columns 4u..4u+3) inside an x-strip row, or -1 if the unit holds no CPML column
+GPR_HD int xstrip_slot(int u, int xnl, int xur, int pitch)
+{
+  return u < 0 ? -1 : (u < xnl ? 4 * u : ((u >= xur && 4 * u < pitch) ? 4 * (xnl + u - xur) : -1));
+}
+
 GPR_HD float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
 GPR_HD void st4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
 GPR_HD float4 mk4(float a, float b, float c, float d) { float4 v; v.x = a; v.y = b; v.z = c; v.w = d; return v; }
 GPR_HD void unpack(float4 v, float* o) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
-
-constexpr int kRZ = 8;        // rows streamed per thread (v1 kernels)
-constexpr int kWarpsY = 4;    // warps per block, stacked in z
-constexpr int kBlockRows = kRZ * kWarpsY;
-constexpr int kBlockCols = 128;   // 32 lanes x float4
 
 }  // namespace gprfwi

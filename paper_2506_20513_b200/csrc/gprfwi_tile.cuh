@@ -86,6 +86,7 @@ struct TileCtx {
   int gj0, gi;          // grid row of this warp's row 0, grid column of this lane's component 0
   int rj0, ri0;         // grid row / column of the region's origin
   bool colin;           // the lane's float4 lies inside [0, pitch)
+  int xslot;            // float offset of this lane's unit in an x-strip row, -1 if it holds no CPML column
   unsigned xsH, xsE;    // bit c: column gi + c carries H- / E-located x psi
   unsigned zsH, zsE;    // bit r: row gj0 + r carries H- / E-located z psi (warp-uniform)
   unsigned rin;         // bit r: row inside the grid (warp-uniform)
@@ -108,6 +109,7 @@ struct TileCtx {
     gj0 = rj0 + lr0; gi = ri0 + l4;
     sm = sm_; toff = lr0 * kRegW + l4;
     colin = gi >= 0 && gi < g.pitch;
+    xslot = (g.P > 0 && colin) ? xstrip_slot(gi >> 2, g.xnl, g.xur, g.pitch) : -1;
     xsH = xsE = zsH = zsE = rin = own = 0u;
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
@@ -163,13 +165,10 @@ struct TileCtx {
       zero4(a); zero4(b); zero4(c); zero4(d);
       if (in && ((zsH >> r) & 1u)) ldg4a(st.phxz + s * g.zstrip + (long long)strip_h(gj, g.nz, g.P) * g.pitch + gi, a);
       if (in && ((zsE >> r) & 1u)) ldg4a(st.pezz + s * g.zstrip + (long long)strip_e(gj, g.nz, g.P) * g.pitch + gi, b);
-      if (in && (xsH | xsE)) {
-        const long long po = s * g.xstrip + (long long)gj * g.xw;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          if ((xsH >> q) & 1u) c[q] = __ldg(st.phyx + po + strip_h(gi + q, g.nx, g.P));
-          if ((xsE >> q) & 1u) d[q] = __ldg(st.pezx + po + strip_e(gi + q, g.nx, g.P));
-        }
+      if (in && xslot >= 0) {
+        const long long po = s * g.xstrip + (long long)gj * g.xw + xslot;
+        ldg4a(st.phyx + po, c);
+        ldg4a(st.pezx + po, d);
       }
       st4a(phz_() + r * kRegW, a); st4a(pez_() + r * kRegW, b); st4a(phx_() + r * kRegW, c); st4a(pex_() + r * kRegW, d);
     }
@@ -186,13 +185,10 @@ struct TileCtx {
       float v[4];
       if ((zsH >> r) & 1u) { lds4a(phz_() + r * kRegW, v); st4a(st.phxz + s * g.zstrip + (long long)strip_h(gj, g.nz, g.P) * g.pitch + gi, v); }
       if ((zsE >> r) & 1u) { lds4a(pez_() + r * kRegW, v); st4a(st.pezz + s * g.zstrip + (long long)strip_e(gj, g.nz, g.P) * g.pitch + gi, v); }
-      if (xsH | xsE) {
-        const long long po = s * g.xstrip + (long long)gj * g.xw;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          if ((xsH >> q) & 1u) st.phyx[po + strip_h(gi + q, g.nx, g.P)] = phx_()[r * kRegW + q];
-          if ((xsE >> q) & 1u) st.pezx[po + strip_e(gi + q, g.nx, g.P)] = pex_()[r * kRegW + q];
-        }
+      if (xslot >= 0) {
+        const long long po = s * g.xstrip + (long long)gj * g.xw + xslot;
+        lds4a(phx_() + r * kRegW, v); st4a(st.phyx + po, v);
+        lds4a(pex_() + r * kRegW, v); st4a(st.pezx + po, v);
       }
     }
   }
