@@ -151,7 +151,7 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
   Carve& o = c ? *c : tmp;
   o.ca = (float*)take(L.plane * f);
   o.cb = (float*)take(L.plane * f);
-  o.tables = (float*)take((size_t)6 * (p->nx + p->nz) * f);
+  o.tables = (float*)take((size_t)10 * (p->nx + p->nz) * f);
   o.gca = (float*)take((size_t)L.ngroups * L.plane * f);
   o.gcb = (float*)take((size_t)L.ngroups * L.plane * f);
   o.src_off = (int*)take(S * sizeof(int));
@@ -333,15 +333,21 @@ static int upload_static(gprfwi_handle* h, cudaStream_t st)
   const gprfwi_params& p = h->p;
   const Layout& L = h->L;
   const int n = p.nx + p.nz;
-  h->h_tables.assign((size_t)6 * n, 0.f);
+  h->h_tables.assign((size_t)10 * n, 0.f);
   float* t = h->h_tables.data();
-  // order: ex(b,c,k)[nx] ez(b,c,k)[nz] hx(b,c,k)[nx] hz(b,c,k)[nz]
-  float* ex = t;             float* ez = ex + 3 * p.nx;
-  float* hx = ez + 3 * p.nz; float* hz = hx + 3 * p.nx;
-  build_table(&p, p.nx, false, ex, ex + p.nx, ex + 2 * p.nx);
-  build_table(&p, p.nz, false, ez, ez + p.nz, ez + 2 * p.nz);
-  build_table(&p, p.nx, true, hx, hx + p.nx, hx + 2 * p.nx);
-  build_table(&p, p.nz, true, hz, hz + p.nz, hz + 2 * p.nz);
+  const float rdx_f = (float)(1.0 / (double)p.dx), Db_f = (float)((double)p.dt / kMu0);
+  const float kap_f = Db_f * rdx_f;                      // exactly what the kernels compute
+  // four sets of [5][len]: ex[nx] ez[nz] hx[nx] hz[nz]; rows b, c, 1/kappa, c/dx, Db/(dx kappa)
+  auto fill = [&](float* set, int len, bool hloc) {
+    build_table(&p, len, hloc, set, set + len, set + 2 * len);
+    for (int i = 0; i < len; ++i) {
+      set[3 * len + i] = (float)((double)set[len + i] / (double)p.dx);
+      set[4 * len + i] = kap_f * set[2 * len + i];
+    }
+  };
+  float* ex = t;             float* ez = ex + 5 * p.nx;
+  float* hx = ez + 5 * p.nz; float* hz = hx + 5 * p.nx;
+  fill(ex, p.nx, false); fill(ez, p.nz, false); fill(hx, p.nx, true); fill(hz, p.nz, true);
   GPR_CUDA(cudaMemcpyAsync(h->c.tables, t, h->h_tables.size() * sizeof(float), cudaMemcpyHostToDevice, st));
   GPR_CUDA(cudaMemcpyAsync(h->c.src_off, h->h_src_off.data(), h->h_src_off.size() * sizeof(int),
                            cudaMemcpyHostToDevice, st));
@@ -358,13 +364,11 @@ static int upload_static(gprfwi_handle* h, cudaStream_t st)
   Geo& g = h->geo;
   g.nz = p.nz; g.nx = p.nx; g.P = p.npml; g.pitch = L.pitch; g.xw = L.xw; g.xnl = L.xnl; g.xur = L.xur;
   g.plane = (long long)L.plane; g.zstrip = (long long)L.zstrip; g.xstrip = (long long)L.xstrip;
-  g.rdx = (float)(1.0 / (double)p.dx);
-  g.Db = (float)((double)p.dt / kMu0);
-  const float* d = h->c.tables;
-  g.bex = d; g.cex = d + p.nx; g.kex = d + 2 * p.nx; d += 3 * p.nx;
-  g.bez = d; g.cez = d + p.nz; g.kez = d + 2 * p.nz; d += 3 * p.nz;
-  g.bhx = d; g.chx = d + p.nx; g.khx = d + 2 * p.nx; d += 3 * p.nx;
-  g.bhz = d; g.chz = d + p.nz; g.khz = d + 2 * p.nz;
+  g.rdx = rdx_f;
+  g.Db = Db_f;
+  g.kap = kap_f;
+  g.tex = h->c.tables;       g.tez = g.tex + 5 * p.nx;
+  g.thx = g.tez + 5 * p.nz;  g.thz = g.thx + 5 * p.nx;
   return GPRFWI_OK;
 }
 

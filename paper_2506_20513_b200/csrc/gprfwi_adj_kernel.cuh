@@ -53,8 +53,9 @@ __device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW>
   }
 }
 
-// The T reverse steps of one warp for one shot; PML as in fwd_steps.
-template <int R, int NW, bool PML>
+// The T reverse steps of one warp for one shot; ZP / XP as in fwd_steps (the psi forms below give
+// exactly tx = q, tz = -q, sx, sz = +-Db lamH with the trivial coefficients outside the CPML).
+template <int R, int NW, bool ZP, bool XP>
 __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW>& c, int s, int rk0, int rk1,
                                           unsigned iflags, float (&le)[R][4], float (&lhx)[R][4], float (&lhy)[R][4],
                                           const float (&ca)[R][4], const float (&cb)[R][4],
@@ -101,7 +102,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW>
         tx[q] = qv; tz[q] = -qv;
         le[r][q] = FM(ca[r][q], le[r][q]);
       }
-      if (PML && ((c.zsE >> r) & 1u)) {
+      if (ZP) {
         float p[4];
         lds4a(c.pez_() + r * kRegW, p);
         const float b = c.tabz_()[3 * L::ROWS + c.lr0 + r], cc = c.tabz_()[4 * L::ROWS + c.lr0 + r],
@@ -114,13 +115,13 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW>
         }
         st4a(c.pez_() + r * kRegW, p);
       }
-      if (PML && c.xsE) {
+      if (XP) {
         float p[4], b[4], cc[4], ik[4];
         lds4a(c.pex_() + r * kRegW, p);
         lds4a(c.tabx_() + 3 * kRegW + c.l4, b); lds4a(c.tabx_() + 4 * kRegW + c.l4, cc); lds4a(c.tabx_() + 5 * kRegW + c.l4, ik);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          if ((c.xsE >> q) & 1u) {
+          {
             const float T_ = FA(p[q], tx[q]);         // psiEx + q
             tx[q] = FF(cc[q], T_, FM(tx[q], ik[q]));
             p[q] = FM(b[q], T_);
@@ -156,7 +157,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW>
       float sx[4], sz[4];
 #pragma unroll
       for (int q = 0; q < 4; ++q) { sz[q] = FM(-Db, lhx[r][q]); sx[q] = FM(Db, lhy[r][q]); }
-      if (PML && ((c.zsH >> r) & 1u)) {
+      if (ZP) {
         float p[4];
         lds4a(c.phz_() + r * kRegW, p);
         const float b = c.tabz_()[0 * L::ROWS + c.lr0 + r], cc = c.tabz_()[1 * L::ROWS + c.lr0 + r],
@@ -169,13 +170,13 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW>
         }
         st4a(c.phz_() + r * kRegW, p);
       }
-      if (PML && c.xsH) {
+      if (XP) {
         float p[4], b[4], cc[4], ik[4];
         lds4a(c.phx_() + r * kRegW, p);
         lds4a(c.tabx_() + 0 * kRegW + c.l4, b); lds4a(c.tabx_() + 1 * kRegW + c.l4, cc); lds4a(c.tabx_() + 2 * kRegW + c.l4, ik);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          if ((c.xsH >> q) & 1u) {
+          {
             const float T_ = FA(p[q], sx[q]);
             sx[q] = FF(cc[q], T_, FM(sx[q], ik[q]));
             p[q] = FM(b[q], T_);
@@ -219,8 +220,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   const int grp = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
   const unsigned full = 0xffffffffu;
 
-  c.stage_tables(g);
-  const bool pml = __any_sync(full, (c.zsH | c.zsE | c.xsH | c.xsE) != 0u);    // warp-uniform
+  c.template stage_tables<false>(g);
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
     reinterpret_cast<float4*>(c.rowbuf_())[k] = make_float4(0.f, 0.f, 0.f, 0.f);
 
@@ -258,12 +258,14 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
         ldg4a(a.in.hy + o, lhy[r]);
       }
     }
-    if (pml) c.load_psi(g, a.in, s);
+    if (c.zp || c.xp) c.load_psi(g, a.in, s);
     adj_stage<R, NW>(a, c, s, rk0, rk1, 0);
     __syncthreads();
 
-    if (pml) adj_steps<R, NW, true>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
-    else adj_steps<R, NW, false>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    if (c.zp && c.xp) adj_steps<R, NW, true, true>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    else if (c.zp) adj_steps<R, NW, true, false>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    else if (c.xp) adj_steps<R, NW, false, true>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    else adj_steps<R, NW, false, false>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
 
     // ---- write back the owned part of the adjoint state ------------------------------------------------
 #pragma unroll
@@ -274,7 +276,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
       st4a(a.out.hx + o, lhx[r]);
       st4a(a.out.hy + o, lhy[r]);
     }
-    if (pml) c.store_psi(g, a.out, s);
+    if (c.zp || c.xp) c.store_psi(g, a.out, s);
   }
 
   // ---- once per CTA: add the register partial sums to this group's gCa / gCb planes --------------------

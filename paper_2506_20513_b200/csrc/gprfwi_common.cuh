@@ -8,7 +8,8 @@
 //   x-strips      [S][nz][xw]        CPML psi of the x-derivative, only the float4 units of a row that
 //                                    touch the left / right CPML: units [0, xnl) then [xur, pitch/4)
 //   Ca, Cb        [nz][pitch]        shared by all shots
-//   1-D CPML tables (b, c, 1/kappa) per axis and per E/H location, built on the host in float64.
+//   1-D CPML tables (b, c, 1/kappa, c/dx, Db/(dx kappa)) per axis and per E/H location, built on the
+//   host in float64.
 #pragma once
 #include <stdint.h>
 #include <vector_types.h>
@@ -29,12 +30,11 @@ struct Geo {
   long long plane;      // nz * pitch
   long long zstrip;     // 2P * pitch   (per shot)
   long long xstrip;     // nz * xw      (per shot)
-  float rdx, Db;        // 1/dx ; dt/mu0 (the paper's uH4 with mu_r = 1)
-  // 1-D CPML tables, E-located (n entries) and H-located (n-1 entries)
-  const float *bex, *cex, *kex;   // x axis, E nodes
-  const float *bez, *cez, *kez;   // z axis, E nodes
-  const float *bhx, *chx, *khx;   // x axis, H nodes (i + 1/2)
-  const float *bhz, *chz, *khz;   // z axis, H nodes (j + 1/2)
+  float rdx, Db, kap;   // 1/dx ; dt/mu0 (the paper's uH4 with mu_r = 1) ; fp32 product Db*rdx
+  // 1-D CPML tables, one set per axis and per E/H location, each [5][n]: b, c, 1/kappa, c/dx, and
+  // (H sets) Db/(dx kappa).  The last two are the forward kernel's pre-multiplied forms.
+  const float *tex, *tez;   // E nodes: x axis (n = nx), z axis (n = nz)
+  const float *thx, *thz;   // H nodes (i + 1/2): x axis, z axis
 };
 
 // One complete state of the scheme for a batch of shots (pointers are for local shot 0).

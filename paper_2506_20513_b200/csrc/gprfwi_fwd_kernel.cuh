@@ -7,10 +7,13 @@
 //   stage 7  save wavefield: every step's Ez plane of the owned cells (history / recompute segment)
 // on the register tile of gprfwi_tile.cuh.  Per step: H phase, barrier, E phase, barrier.
 //
-// CPML (reading R4): psi <- b psi + c d,  derivative term d/kappa + psi, with d the plain
-// difference quotient; b, c, 1/kappa from 1-D tables.  A cell uses the psi form iff its row / column
-// lies in the corresponding strip, else the plain fused-multiply-add form; which form a cell uses
-// depends only on where it is, never on which CTA computes it.
+// CPML (reading R4): psi <- b psi + c d, derivative term d/kappa + psi with d the difference
+// quotient, written with pre-multiplied tables so that with the trivial coefficients outside the CPML
+// (b = c = 0, kappa = 1) every expression rounds EXACTLY like the plain one:
+//   Hx -= Db psi + (Db/(dx kappa)) (E[j+1] - E[j]),   psi <- b psi + (c/dx) (E[j+1] - E[j])
+//   Ez  = Ca Ez + Cb (((Hy - Hy[i-1])/kx - (Hx - Hx[j-1])/kz)/dx + (psix - psiz))
+// A warp whose rows (ZP) / whose CTA's columns (XP) touch the CPML runs the psi form on all its
+// cells, every other warp the plain form; a cell's value does not depend on which form computed it.
 #pragma once
 #include "gprfwi_tile.cuh"
 
@@ -35,10 +38,9 @@ struct FwdArgs {
 };
 
 #if defined(__CUDACC__)
-// The T-step loop of one warp.  PML = false: none of the warp's rows and none of the CTA's columns
-// carries CPML psi -> straight-line plain updates.  PML = true: per row / per column selects.
-// Both variants hit the same barriers, so warps of one CTA may run different variants.
-template <int R, int NW, bool PML>
+// The T-step loop of one warp.  All variants hit the same barriers, so the warps of one CTA may run
+// different variants.
+template <int R, int NW, bool ZP, bool XP>
 __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>& c, int s, int rk0, int rk1,
                                           unsigned rflags, int src_r, int src_c,
                                           float (&e)[R][4], float (&hx)[R][4], float (&hy)[R][4],
@@ -47,7 +49,7 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
   using L = RegTile<R, NW>;
   const Geo& g = a.g;
   const unsigned full = 0xffffffffu;
-  const float rdx = g.rdx, Db = g.Db, kap = g.Db * g.rdx;
+  const float rdx = g.rdx, Db = g.Db, kap = g.kap;
   float wv[kMaxT];
 #pragma unroll
   for (int t = 0; t < kMaxT; ++t) wv[t] = t < a.nsub ? a.wavelet[s * a.wav_stride + t] * (rdx * rdx) : 0.f;
@@ -63,41 +65,38 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
     }
 
     // ---- stages 2-3: H update + H CPML -------------------------------------------------------------
+    float xb[4], xc[4], xk[4];                          // x tables of this lane's columns (XP only)
+    if (XP) { lds4a(c.tabx_() + 0 * kRegW + c.l4, xb); lds4a(c.tabx_() + 1 * kRegW + c.l4, xc); lds4a(c.tabx_() + 2 * kRegW + c.l4, xk); }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       float eb[4];                                      // Ez of the row below
       if (r + 1 < R) { eb[0] = e[r + 1][0]; eb[1] = e[r + 1][1]; eb[2] = e[r + 1][2]; eb[3] = e[r + 1][3]; }
       else lds4a(c.xe_() + (c.w + 1) * kRegW + c.l4, eb);
       const float en[4] = {e[r][1], e[r][2], e[r][3], __shfl_down_sync(full, e[r][0], 1)};   // Ez to the right
-      if (PML && ((c.zsH >> r) & 1u)) {
+      if (ZP) {
         float p[4];
         lds4a(c.phz_() + r * kRegW, p);
-        const float b = c.tabz_()[0 * L::ROWS + c.lr0 + r], cc = c.tabz_()[1 * L::ROWS + c.lr0 + r],
-                    ik = c.tabz_()[2 * L::ROWS + c.lr0 + r];
+        const float b = c.tabz_()[0 * L::ROWS + c.lr0 + r], cr = c.tabz_()[1 * L::ROWS + c.lr0 + r],
+                    kk = c.tabz_()[2 * L::ROWS + c.lr0 + r];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          const float d = FM(FS(eb[q], e[r][q]), rdx);
-          p[q] = FF(b, p[q], FM(cc, d));
-          hx[r][q] = FF(-Db, FF(d, ik, p[q]), hx[r][q]);
+          const float d = FS(eb[q], e[r][q]);
+          p[q] = FF(b, p[q], FM(cr, d));
+          hx[r][q] = FF(-Db, p[q], FF(-kk, d, hx[r][q]));
         }
         st4a(c.phz_() + r * kRegW, p);
       } else {
 #pragma unroll
         for (int q = 0; q < 4; ++q) hx[r][q] = FF(-kap, FS(eb[q], e[r][q]), hx[r][q]);
       }
-      if (PML && c.xsH) {
-        float p[4], b[4], cc[4], ik[4];
+      if (XP) {
+        float p[4];
         lds4a(c.phx_() + r * kRegW, p);
-        lds4a(c.tabx_() + 0 * kRegW + c.l4, b); lds4a(c.tabx_() + 1 * kRegW + c.l4, cc); lds4a(c.tabx_() + 2 * kRegW + c.l4, ik);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          if ((c.xsH >> q) & 1u) {
-            const float d = FM(FS(en[q], e[r][q]), rdx);
-            p[q] = FF(b[q], p[q], FM(cc[q], d));
-            hy[r][q] = FF(Db, FF(d, ik[q], p[q]), hy[r][q]);
-          } else {
-            hy[r][q] = FF(kap, FS(en[q], e[r][q]), hy[r][q]);
-          }
+          const float d = FS(en[q], e[r][q]);
+          p[q] = FF(xb[q], p[q], FM(xc[q], d));
+          hy[r][q] = FF(Db, p[q], FF(xk[q], d, hy[r][q]));
         }
         st4a(c.phx_() + r * kRegW, p);
       } else {
@@ -109,59 +108,64 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
     __syncthreads();
 
     // ---- stages 4-7: E update + E CPML, source, save wavefield --------------------------------------
-    const bool last = t + 1 == a.nsub;
-    float* ez_out = last ? a.out.ez : a.ez_hist[t + 1];
-    float wn = wv[0];
-#pragma unroll
-    for (int k = 1; k < kMaxT; ++k) wn = t == k ? wv[k] : wn;
+    if (XP) { lds4a(c.tabx_() + 3 * kRegW + c.l4, xb); lds4a(c.tabx_() + 4 * kRegW + c.l4, xc); lds4a(c.tabx_() + 5 * kRegW + c.l4, xk); }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       float ha[4];                                      // Hx of the row above
       if (r > 0) { ha[0] = hx[r - 1][0]; ha[1] = hx[r - 1][1]; ha[2] = hx[r - 1][2]; ha[3] = hx[r - 1][3]; }
       else lds4a(c.xh_() + c.w * kRegW + c.l4, ha);
       const float hl[4] = {__shfl_up_sync(full, hy[r][3], 1), hy[r][0], hy[r][1], hy[r][2]};  // Hy to the left
-      const bool zs = PML && ((c.zsE >> r) & 1u);
-      if (PML && (zs || c.xsE)) {
-        float pz[4], px[4], bx[4], cx[4], kx[4];
+      if (ZP || XP) {
+        float pz[4], px[4];
         float bz = 0.f, cz = 0.f, kz = 1.f;
-        zero4(pz); zero4(px); zero4(bx); zero4(cx); zero4(kx);
-        if (zs) {
+        if (ZP) {
           lds4a(c.pez_() + r * kRegW, pz);
           bz = c.tabz_()[3 * L::ROWS + c.lr0 + r]; cz = c.tabz_()[4 * L::ROWS + c.lr0 + r]; kz = c.tabz_()[5 * L::ROWS + c.lr0 + r];
         }
-        if (c.xsE) {
-          lds4a(c.pex_() + r * kRegW, px);
-          lds4a(c.tabx_() + 3 * kRegW + c.l4, bx); lds4a(c.tabx_() + 4 * kRegW + c.l4, cx); lds4a(c.tabx_() + 5 * kRegW + c.l4, kx);
-        }
+        if (XP) lds4a(c.pex_() + r * kRegW, px);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          const bool xs = (c.xsE >> q) & 1u;
-          if (!zs && !xs) {
-            e[r][q] = FF(cb[r][q], FM(FS(FS(hy[r][q], hl[q]), FS(hx[r][q], ha[q])), rdx), FM(ca[r][q], e[r][q]));
-          } else {
-            float vx = FM(FS(hy[r][q], hl[q]), rdx), vz = FM(FS(hx[r][q], ha[q]), rdx);
-            if (xs) { px[q] = FF(bx[q], px[q], FM(cx[q], vx)); vx = FF(vx, kx[q], px[q]); }
-            if (zs) { pz[q] = FF(bz, pz[q], FM(cz, vz)); vz = FF(vz, kz, pz[q]); }
-            e[r][q] = FF(cb[r][q], FS(vx, vz), FM(ca[r][q], e[r][q]));
-          }
+          const float tx = FS(hy[r][q], hl[q]), tz = FS(hx[r][q], ha[q]);
+          float dd, pp;                                 // (tx/kx - tz/kz) and (psix - psiz)
+          if (ZP) pz[q] = FF(bz, pz[q], FM(cz, tz));
+          if (XP) px[q] = FF(xb[q], px[q], FM(xc[q], tx));
+          if (ZP && XP) { dd = FF(tx, xk[q], -FM(tz, kz)); pp = FS(px[q], pz[q]); }
+          else if (ZP)  { dd = FS(tx, FM(tz, kz));         pp = -pz[q]; }
+          else          { dd = FF(tx, xk[q], -tz);         pp = px[q]; }
+          e[r][q] = FF(cb[r][q], FF(dd, rdx, pp), FM(ca[r][q], e[r][q]));
         }
-        if (zs) st4a(c.pez_() + r * kRegW, pz);
-        if (c.xsE) st4a(c.pex_() + r * kRegW, px);
+        if (ZP) st4a(c.pez_() + r * kRegW, pz);
+        if (XP) st4a(c.pex_() + r * kRegW, px);
       } else {
 #pragma unroll
         for (int q = 0; q < 4; ++q)
           e[r][q] = FF(cb[r][q], FM(FS(FS(hy[r][q], hl[q]), FS(hx[r][q], ha[q])), rdx), FM(ca[r][q], e[r][q]));
       }
-      if (r == src_r) {                                 // every CTA whose region holds the source injects
+    }
+    if (src_r >= 0) {                                   // every CTA whose region holds the source injects
+      float wn = wv[0];
+#pragma unroll
+      for (int k = 1; k < kMaxT; ++k) wn = t == k ? wv[k] : wn;
+#pragma unroll
+      for (int r = 0; r < R; ++r)
 #pragma unroll
         for (int q = 0; q < 4; ++q)
-          if (q == src_c) e[r][q] = FF(-cb[r][q], wn, e[r][q]);
-      }
-      if (ez_out && ((c.own >> r) & 1u)) {
-        float* dst = ez_out + s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-        if (last) st4a(dst, e[r]); else stcs4a(dst, e[r]);     // intermediate planes are history only: stream them
-      }
-      if ((rflags >> r) & 1u) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
+          if (r == src_r && q == src_c) e[r][q] = FF(-cb[r][q], wn, e[r][q]);
+    }
+    const bool last = t + 1 == a.nsub;
+    float* ez_out = last ? a.out.ez : a.ez_hist[t + 1];
+    if (ez_out) {
+      float* dst = ez_out + s * g.plane + (long long)c.gj0 * g.pitch + c.gi;
+#pragma unroll
+      for (int r = 0; r < R; ++r)
+        if ((c.own >> r) & 1u) {
+          if (last) st4a(dst + r * g.pitch, e[r]); else stcs4a(dst + r * g.pitch, e[r]);   // history only: stream
+        }
+    }
+    if (rflags) {
+#pragma unroll
+      for (int r = 0; r < R; ++r)
+        if ((rflags >> r) & 1u) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
     }
     st4a(c.xe_() + c.w * kRegW + c.l4, e[0]);
     __syncthreads();
@@ -178,7 +182,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
   const int s = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
   const unsigned full = 0xffffffffu;
 
-  c.stage_tables(g);
+  c.template stage_tables<true>(g);
 
   // rows of this warp that hold receivers owned by this tile (warp-uniform bit mask)
   unsigned rflags = 0u;
@@ -212,16 +216,17 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
       ldg4a(a.cb + o, cb[r]);
     }
   }
-  const bool pml = __any_sync(full, (c.zsH | c.zsE | c.xsH | c.xsE) != 0u);    // warp-uniform
-  if (pml) c.load_psi(g, a.in, s);
+  if (c.zp || c.xp) c.load_psi(g, a.in, s);
   st4a(c.xe_() + c.w * kRegW + c.l4, e[0]);
 #pragma unroll
   for (int r = 0; r < R; ++r)
     if ((rflags >> r) & 1u) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
   __syncthreads();
 
-  if (pml) fwd_steps<R, NW, true>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
-  else fwd_steps<R, NW, false>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
+  if (c.zp && c.xp) fwd_steps<R, NW, true, true>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
+  else if (c.zp) fwd_steps<R, NW, true, false>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
+  else if (c.xp) fwd_steps<R, NW, false, true>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
+  else fwd_steps<R, NW, false, false>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
 
   // ---- write back what this tile owns (out.ez was written by the last E phase) ----------------------
 #pragma unroll
@@ -231,7 +236,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
     st4a(a.out.hx + o, hx[r]);
     st4a(a.out.hy + o, hy[r]);
   }
-  if (pml) c.store_psi(g, a.out, s);
+  if (c.zp || c.xp) c.store_psi(g, a.out, s);
 }
 #endif
 

@@ -87,7 +87,7 @@ struct TileCtx {
   int rj0, ri0;         // grid row / column of the region's origin
   bool colin;           // the lane's float4 lies inside [0, pitch)
   int xslot;            // float offset of this lane's unit in an x-strip row, -1 if it holds no CPML column
-  unsigned xsH, xsE;    // bit c: column gi + c carries H- / E-located x psi
+  bool xp, zp;          // the CTA's columns / this warp's rows touch the x / z CPML (warp-uniform)
   unsigned zsH, zsE;    // bit r: row gj0 + r carries H- / E-located z psi (warp-uniform)
   unsigned rin;         // bit r: row inside the grid (warp-uniform)
   unsigned own;         // bit r: row owned by this tile (and inside the grid); 0 for lanes 0 and 31
@@ -110,12 +110,8 @@ struct TileCtx {
     sm = sm_; toff = lr0 * kRegW + l4;
     colin = gi >= 0 && gi < g.pitch;
     xslot = (g.P > 0 && colin) ? xstrip_slot(gi >> 2, g.xnl, g.xur, g.pitch) : -1;
-    xsH = xsE = zsH = zsE = rin = own = 0u;
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      if (g.P > 0 && strip_h(gi + c, g.nx, g.P) >= 0) xsH |= 1u << c;
-      if (g.P > 0 && strip_e(gi + c, g.nx, g.P) >= 0) xsE |= 1u << c;
-    }
+    zsH = zsE = rin = own = 0u;
+    xp = g.P > 0 && (ri0 < g.P || ri0 + kRegW > g.nx - 1 - g.P);
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       const int gj = gj0 + r;
@@ -126,27 +122,38 @@ struct TileCtx {
         if (lr0 + r >= hz && lr0 + r < L::ROWS - hz && lane >= 1 && lane <= 30 && colin) own |= 1u << r;
       }
     }
+    zp = (zsH | zsE) != 0u;
   }
 
-  // CPML tables of the region's rows and columns -> shared memory (outside the grid: b = c = 0, 1/kappa = 1)
+  // CPML tables of the region's rows and columns -> shared memory (outside the grid: b = c = 0, 1/kappa = 1).
+  // FWD: (b, c/dx, Db/(dx kappa)) at H nodes and (b, c/dx, 1/kappa) at E nodes; else (b, c, 1/kappa) at both.
+  template <bool FWD>
   __device__ __forceinline__ void stage_tables(const Geo& g) const
   {
+    const int r1 = FWD ? 3 : 1, r2h = FWD ? 4 : 2;
+    const float k0 = FWD ? g.kap : 1.f;
     if (w == 0) {
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         const int i = gi + c;
         const bool in = i >= 0 && i < g.nx;
-        tabx_()[0 * kRegW + l4 + c] = in ? g.bhx[i] : 0.f; tabx_()[1 * kRegW + l4 + c] = in ? g.chx[i] : 0.f;
-        tabx_()[2 * kRegW + l4 + c] = in ? g.khx[i] : 1.f; tabx_()[3 * kRegW + l4 + c] = in ? g.bex[i] : 0.f;
-        tabx_()[4 * kRegW + l4 + c] = in ? g.cex[i] : 0.f; tabx_()[5 * kRegW + l4 + c] = in ? g.kex[i] : 1.f;
+        tabx_()[0 * kRegW + l4 + c] = in ? g.thx[i] : 0.f;
+        tabx_()[1 * kRegW + l4 + c] = in ? g.thx[r1 * g.nx + i] : 0.f;
+        tabx_()[2 * kRegW + l4 + c] = in ? g.thx[r2h * g.nx + i] : k0;
+        tabx_()[3 * kRegW + l4 + c] = in ? g.tex[i] : 0.f;
+        tabx_()[4 * kRegW + l4 + c] = in ? g.tex[r1 * g.nx + i] : 0.f;
+        tabx_()[5 * kRegW + l4 + c] = in ? g.tex[2 * g.nx + i] : 1.f;
       }
     }
     for (int k = threadIdx.x; k < L::ROWS; k += L::THREADS) {
       const int gj = rj0 + k;
       const bool in = gj >= 0 && gj < g.nz;
-      tabz_()[0 * L::ROWS + k] = in ? g.bhz[gj] : 0.f; tabz_()[1 * L::ROWS + k] = in ? g.chz[gj] : 0.f;
-      tabz_()[2 * L::ROWS + k] = in ? g.khz[gj] : 1.f; tabz_()[3 * L::ROWS + k] = in ? g.bez[gj] : 0.f;
-      tabz_()[4 * L::ROWS + k] = in ? g.cez[gj] : 0.f; tabz_()[5 * L::ROWS + k] = in ? g.kez[gj] : 1.f;
+      tabz_()[0 * L::ROWS + k] = in ? g.thz[gj] : 0.f;
+      tabz_()[1 * L::ROWS + k] = in ? g.thz[r1 * g.nz + gj] : 0.f;
+      tabz_()[2 * L::ROWS + k] = in ? g.thz[r2h * g.nz + gj] : k0;
+      tabz_()[3 * L::ROWS + k] = in ? g.tez[gj] : 0.f;
+      tabz_()[4 * L::ROWS + k] = in ? g.tez[r1 * g.nz + gj] : 0.f;
+      tabz_()[5 * L::ROWS + k] = in ? g.tez[2 * g.nz + gj] : 1.f;
     }
     // the two exchange slots nobody publishes: below the last warp, above the first
     if (w == NW - 1) *reinterpret_cast<float4*>(xe_() + NW * kRegW + l4) = make_float4(0.f, 0.f, 0.f, 0.f);
