@@ -51,7 +51,7 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 #define GPR_FWD_TILE 4, 8, 2
 #define GPR_ADJ_TILE 3, 8, 2
 using FwdShape = RegTile<4, 8>;
-using AdjShape = RegTile<3, 8>;
+using AdjShape = RegTile<3, 8, 3>;
 
 struct Tiling {
   int oz = 0, tiles_x = 0, tiles_y = 0;   // owned rows per tile; tiles of kOwnW columns x oz rows

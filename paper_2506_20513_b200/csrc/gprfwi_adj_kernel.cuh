@@ -41,9 +41,9 @@ struct AdjArgs {
 // transpose of recording: residual sample n_hi - t enters lamE at the start of reverse step n_hi-1-t;
 // it is staged in rowbuf (zero between uses) one barrier ahead of its use
 template <int R, int NW>
-__device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW>& c, int s, int rk0, int rk1, int t)
+__device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1, int t)
 {
-  using L = RegTile<R, NW>;
+  using L = RegTile<R, NW, 3>;
   if (a.n_hi - t >= a.nt) return;
   for (int k = rk0 + threadIdx.x; k < rk1; k += L::THREADS) {
     const int rr = a.reg_rec[k];
@@ -53,21 +53,40 @@ __device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW>
   }
 }
 
+// owned rows of forward plane Ez^{n_hi - t} -> slot t % 3 of the thread's history ring (one commit group)
+template <int R, int NW>
+__device__ __forceinline__ void adj_fetch(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int t)
+{
+  using L = RegTile<R, NW, 3>;
+  if (t <= a.nsub) {
+    const float* src = a.ez_planes[t] + s * a.g.plane + (long long)c.gj0 * a.g.pitch + c.gi;
+    float* dst = c.hist_() + (t % 3) * (L::ROWS * kRegW);
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+      if ((c.own >> r) & 1u) cp_async16(dst + r * kRegW, src + (long long)r * a.g.pitch);
+  }
+  cp_async_commit();
+}
+
 // The T reverse steps of one warp for one shot; ZP / XP as in fwd_steps (the psi forms below give
 // exactly tx = q, tz = -q, sx, sz = +-Db lamH with the trivial coefficients outside the CPML).
 template <int R, int NW, bool ZP, bool XP>
-__device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW>& c, int s, int rk0, int rk1,
+__device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
                                           unsigned iflags, float (&le)[R][4], float (&lhx)[R][4], float (&lhy)[R][4],
                                           const float (&ca)[R][4], const float (&cb)[R][4],
                                           float (&ga)[R][4], float (&gb)[R][4])
 {
-  using L = RegTile<R, NW>;
+  using L = RegTile<R, NW, 3>;
   const Geo& g = a.g;
   const unsigned full = 0xffffffffu;
   const float rdx = g.rdx, Db = g.Db;
   #pragma unroll 1
   for (int t = 0; t < a.nsub; ++t) {
     // ---- [A] adjoint source, gradient terms ------------------------------------------------------
+    adj_fetch<R, NW>(a, c, s, t + 2);                   // two steps ahead; planes t and t+1 have landed after the wait
+    cp_async_wait<1>();
+    const float* h1 = c.hist_() + (t % 3) * (L::ROWS * kRegW);
+    const float* h0 = c.hist_() + ((t + 1) % 3) * (L::ROWS * kRegW);
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       if ((iflags >> r) & 1u) {
@@ -80,10 +99,9 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW>
         st4a(rb, v);
       }
       if ((c.own >> r) & 1u) {
-        const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
         float e0[4], e1[4];
-        ldcs4a(a.ez_planes[t + 1] + o, e0);          // E^n
-        ldcs4a(a.ez_planes[t] + o, e1);              // E^{n+1}
+        lds4a(h0 + r * kRegW, e0);                     // E^n
+        lds4a(h1 + r * kRegW, e1);                     // E^{n+1}
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           ga[r][q] = FF(le[r][q], e0[q], ga[r][q]);
@@ -212,10 +230,10 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW>
 template <int R, int NW, int MINB>
 __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
 {
-  using L = RegTile<R, NW>;
+  using L = RegTile<R, NW, 3>;
   extern __shared__ float4 smem4[];
   const Geo& g = a.g;
-  TileCtx<R, NW> c;
+  TileCtx<R, NW, 3> c;
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
   const int grp = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
   const unsigned full = 0xffffffffu;
@@ -258,6 +276,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
         ldg4a(a.in.hy + o, lhy[r]);
       }
     }
+    adj_fetch<R, NW>(a, c, s, 0);
+    adj_fetch<R, NW>(a, c, s, 1);
     if (c.zp || c.xp) c.load_psi(g, a.in, s);
     adj_stage<R, NW>(a, c, s, rk0, rk1, 0);
     __syncthreads();

@@ -20,6 +20,7 @@
 //                     the adjoint stages the residual there for injection
 //   tabx [6][128]     CPML x tables of the region's columns: bhx chx khx bex cex kex
 //   tabz [6][NW*R]    CPML z tables of the region's rows:    bhz chz khz bez cez kez
+//   hist [NH][NW*R][128] adjoint only: ring of forward Ez planes fetched ahead with cp.async, thread-private
 //   psi  [4][NW*R][128]  CPML psi of the region, thread-private (only when npml > 0): hz ez hx ex
 #pragma once
 #include "gprfwi_common.cuh"
@@ -30,7 +31,7 @@ constexpr int kMaxT = 4;       // fused steps per launch <= x halo (4 columns = 
 constexpr int kRegW = 128;     // region width  = 32 lanes x float4
 constexpr int kOwnW = 120;     // owned width   = lanes 1..30
 
-template <int R, int NW>
+template <int R, int NW, int NH = 0>
 struct RegTile {
   static constexpr int ROWS = R * NW;
   static constexpr int THREADS = NW * 32;
@@ -39,7 +40,8 @@ struct RegTile {
   static constexpr int ROWBUF = XH + (NW + 1) * kRegW;
   static constexpr int TABX = ROWBUF + ROWS * kRegW;
   static constexpr int TABZ = TABX + 6 * kRegW;
-  static constexpr int PSI = (TABZ + 6 * ROWS + 3) / 4 * 4;
+  static constexpr int HIST = (TABZ + 6 * ROWS + 3) / 4 * 4;
+  static constexpr int PSI = HIST + NH * ROWS * kRegW;
   GPR_HD static size_t smem_bytes(bool pml) { return sizeof(float) * (size_t)(PSI + (pml ? 4 * ROWS * kRegW : 0)); }
 };
 
@@ -73,13 +75,21 @@ __device__ __forceinline__ void stcs4a(float* p, const float* v)      // streami
 {
   __stcs(reinterpret_cast<float4*>(p), make_float4(v[0], v[1], v[2], v[3]));
 }
+// 16-byte asynchronous copy global -> shared (bypasses L1 and the register file)
+__device__ __forceinline__ void cp_async16(float* smem, const float* gmem)
+{
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void zero4(float* v) { v[0] = v[1] = v[2] = v[3] = 0.f; }
 
 // Per-thread view of the region: where this lane's 4 columns and this warp's R rows sit in the grid,
 // which of them carry CPML psi, and the shared-memory carve-up.
-template <int R, int NW>
+template <int R, int NW, int NH = 0>
 struct TileCtx {
-  using L = RegTile<R, NW>;
+  using L = RegTile<R, NW, NH>;
   float* sm;            // shared-memory base; every array is a compile-time offset from it
   int toff;             // lr0 * 128 + l4: this thread's row-0 slot inside a [ROWS][128] array
   int lane, w, l4, lr0;
@@ -97,6 +107,7 @@ struct TileCtx {
   __device__ __forceinline__ float* rowbuf_() const { return sm + L::ROWBUF; }
   __device__ __forceinline__ float* tabx_() const { return sm + L::TABX; }
   __device__ __forceinline__ float* tabz_() const { return sm + L::TABZ; }
+  __device__ __forceinline__ float* hist_() const { return sm + L::HIST + toff; }
   __device__ __forceinline__ float* phz_() const { return sm + L::PSI + 0 * L::ROWS * kRegW + toff; }
   __device__ __forceinline__ float* pez_() const { return sm + L::PSI + 1 * L::ROWS * kRegW + toff; }
   __device__ __forceinline__ float* phx_() const { return sm + L::PSI + 2 * L::ROWS * kRegW + toff; }
