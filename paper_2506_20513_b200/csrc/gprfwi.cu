@@ -47,11 +47,42 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 // ------------------------------------------------------------------------------------------------
 // memory plan
 // ------------------------------------------------------------------------------------------------
-// register-tile shapes (rows per thread, warps per CTA, min CTAs per SM): gprfwi_tile.cuh
-#define GPR_FWD_TILE 4, 8, 2
-#define GPR_ADJ_TILE 3, 8, 2
-using FwdShape = RegTile<4, 8>;
-using AdjShape = RegTile<3, 8, 3>;
+// Register-tile shapes (rows per thread R, warps per CTA NW, min CTAs per SM): gprfwi_tile.cuh.
+// Entry 0 of each table is the default; GPRFWI_FWD_SHAPE / GPRFWI_ADJ_SHAPE pick another (tuning).
+struct Shape {
+  int R, NW, minb;
+  const void* func;
+  size_t smem_pml, smem_plain;
+  int rows() const { return R * NW; }
+  int threads() const { return NW * 32; }
+  size_t smem(bool pml) const { return pml ? smem_pml : smem_plain; }
+};
+#if defined(__CUDACC__)
+template <int R, int NW, int MINB>
+static Shape fwd_shape()
+{
+  return {R, NW, MINB, (const void*)fwd_kernel<R, NW, MINB>, RegTile<R, NW, 0>::smem_bytes(true),
+          RegTile<R, NW, 0>::smem_bytes(false)};
+}
+template <int R, int NW, int MINB>
+static Shape adj_shape()
+{
+  return {R, NW, MINB, (const void*)adj_kernel<R, NW, MINB>, RegTile<R, NW, 3>::smem_bytes(true),
+          RegTile<R, NW, 3>::smem_bytes(false)};
+}
+static const Shape kFwdShapes[] = {fwd_shape<4, 8, 2>(),  fwd_shape<3, 8, 2>(),  fwd_shape<3, 8, 3>(),
+                                   fwd_shape<2, 16, 2>(), fwd_shape<3, 12, 2>(), fwd_shape<2, 8, 4>(),
+                                   fwd_shape<4, 16, 1>(), fwd_shape<2, 12, 3>(), fwd_shape<6, 8, 1>()};
+static const Shape kAdjShapes[] = {adj_shape<3, 8, 2>(),  adj_shape<2, 8, 3>(),  adj_shape<2, 16, 2>(),
+                                   adj_shape<2, 12, 2>(), adj_shape<3, 16, 1>(), adj_shape<4, 8, 1>(),
+                                   adj_shape<3, 12, 1>(), adj_shape<2, 8, 4>(),  adj_shape<5, 8, 1>()};
+#endif
+static int shape_index(const char* env, int count)
+{
+  const char* e = std::getenv(env);
+  const int k = e ? std::atoi(e) : 0;
+  return (k >= 0 && k < count) ? k : 0;
+}
 
 struct Tiling {
   int oz = 0, tiles_x = 0, tiles_y = 0;   // owned rows per tile; tiles of kOwnW columns x oz rows
@@ -66,12 +97,14 @@ struct Layout {
   size_t full = 0;         // hslot + Ez plane
   int T = 4;               // time steps fused per launch = halo rows
   Tiling f, a;             // forward / adjoint tilings
+  int fv = 0, av = 0;      // kernel shapes in use (indices into kFwdShapes / kAdjShapes)
   // plan
   bool full_history = true;
   int K = 0;               // checkpoint stride (nt when full history)
   int ncheck = 0;          // checkpoints at n = 0, K, 2K, ... (< nt); slot ncheck = state at nt
   int Sb = 0;              // shots per adjoint pass
-  int group = 1, ngroups = 1;
+  int group = 1, ngroups = 1;      // adjoint: shots per CTA, CTAs per tile
+  int fgroup = 1, fngroups = 1;    // forward
   size_t bytes = 0;
 };
 
@@ -109,26 +142,50 @@ static void base_layout(const gprfwi_params* p, Layout& L)
     t.tiles_x = (p->nx + kOwnW - 1) / kOwnW;
     t.tiles_y = (p->nz + t.oz - 1) / t.oz;
   };
-  tiling(FwdShape::ROWS, L.f);
-  tiling(AdjShape::ROWS, L.a);
+  L.fv = shape_index("GPRFWI_FWD_SHAPE", (int)(sizeof(kFwdShapes) / sizeof(Shape)));
+  L.av = shape_index("GPRFWI_ADJ_SHAPE", (int)(sizeof(kAdjShapes) / sizeof(Shape)));
+  tiling(kFwdShapes[L.fv].rows(), L.f);
+  tiling(kAdjShapes[L.av].rows(), L.a);
 }
 
-// Shots of one adjoint pass are split into groups; a CTA sweeps the shots of its group one after the
-// other and keeps their gradient sum in registers.  Enough groups to fill the SMs a few times.
-static void set_groups(Layout& L)
+// A CTA owns one tile and sweeps a GROUP of shots one after the other (the adjoint keeps their
+// gradient sum in registers).  The number of groups is chosen to minimise
+//   waves(ngroups) * (group * t_shot + t_fixed),  waves = ceil(tiles * ngroups / slots),
+// i.e. CTA count a whole number of waves where possible, with t_fixed (per-CTA set-up, flush) taken
+// as `fixed_over_shot` shot-times.
+static void pick_groups(int tiles, int shots, int slots, double fixed_over_shot, int& group, int& ngroups)
 {
-  const int tiles = L.a.tiles();
-  int want = std::max(1, (4 * 148 + tiles - 1) / tiles);
-  int ng = std::min(L.Sb, want);
-  L.group = (L.Sb + ng - 1) / ng;
-  L.ngroups = (L.Sb + L.group - 1) / L.group;
+  double best = 1e300;
+  group = shots; ngroups = 1;
+  for (int ng = 1; ng <= shots; ++ng) {
+    const int grp = (shots + ng - 1) / ng, n = (shots + grp - 1) / grp;
+    const double waves = std::ceil((double)tiles * n / slots);
+    const double cost = waves * (grp + fixed_over_shot);
+    if (cost < best - 1e-9) { best = cost; group = grp; ngroups = n; }
+  }
+}
+
+static int env_int(const char* name, int dflt)
+{
+  const char* e = std::getenv(name);
+  return e ? std::atoi(e) : dflt;
+}
+
+static void set_groups(const gprfwi_params* p, Layout& L)
+{
+  const int fslots = 148 * std::max(1, kFwdShapes[L.fv].minb), aslots = 148 * std::max(1, kAdjShapes[L.av].minb);
+  (void)fslots;
+  L.fgroup = 1; L.fngroups = p->nshots;          // forward: one shot per CTA (shots of a CTA run back to back, unoverlapped)
+  pick_groups(L.a.tiles(), L.Sb, aslots, 1.0, L.group, L.ngroups);
+  if (int g = env_int("GPRFWI_FWD_GROUP", 0)) { L.fgroup = std::min(g, p->nshots); L.fngroups = (p->nshots + L.fgroup - 1) / L.fgroup; }
+  if (int g = env_int("GPRFWI_ADJ_GROUP", 0)) { L.group = std::min(g, L.Sb); L.ngroups = (L.Sb + L.group - 1) / L.group; }
 }
 
 // device pointers carved out of the caller's workspace
 struct Carve {
   float *ca = nullptr, *cb = nullptr, *tables = nullptr, *gca = nullptr, *gcb = nullptr;
-  int *src_off = nullptr, *rec_off = nullptr, *blk_start = nullptr, *blk_rec = nullptr;
-  int *reg_start = nullptr, *reg_rec = nullptr;   // receivers by region (tile + halo), global CSR
+  int *src_off = nullptr, *blk_start = nullptr, *blk_ent = nullptr;   // receivers by owning tile (forward tiling)
+  int *reg_start = nullptr, *reg_ent = nullptr;   // receivers by region (tile + halo) of the adjoint tiling
   float* hist = nullptr;      // full history: (nt+1) * S planes
   float* ckpt = nullptr;      // (ncheck+1) * S full states
   float* seg = nullptr;       // (K-1) * Sb planes: Ez^{cK+1 .. cK+K-1}
@@ -155,11 +212,10 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
   o.gca = (float*)take((size_t)L.ngroups * L.plane * f);
   o.gcb = (float*)take((size_t)L.ngroups * L.plane * f);
   o.src_off = (int*)take(S * sizeof(int));
-  o.rec_off = (int*)take(std::max<size_t>(S * R, 1) * sizeof(int));
   o.blk_start = (int*)take(S * (ntile + 1) * sizeof(int));
-  o.blk_rec = (int*)take(std::max<size_t>(S * R, 1) * sizeof(int));
+  o.blk_ent = (int*)take(std::max<size_t>(S * R, 1) * 2 * sizeof(int));
   o.reg_start = (int*)take((S * natile + 1) * sizeof(int));
-  o.reg_rec = (int*)take(std::max<size_t>(6 * S * R, 1) * sizeof(int));
+  o.reg_ent = (int*)take(std::max<size_t>(6 * S * R, 1) * 2 * sizeof(int));
   o.fscratch = (float*)take(2 * S * L.full * f);
   o.lam = (float*)take(2 * (size_t)L.Sb * L.full * f);
   if (L.full_history) {
@@ -181,7 +237,7 @@ static bool make_plan(const gprfwi_params* p, size_t budget, Layout& L)
     L.K = p->nt;
     L.ncheck = 1;
     L.Sb = p->nshots;
-    set_groups(L);
+    set_groups(p, L);
     L.bytes = carve(p, L, nullptr, nullptr);
     if (budget == 0 || L.bytes <= budget) return true;
   }
@@ -193,7 +249,7 @@ static bool make_plan(const gprfwi_params* p, size_t budget, Layout& L)
     if (sb == prev_sb) continue;
     prev_sb = sb;
     L.Sb = sb;
-    set_groups(L);
+    set_groups(p, L);
     int candidates[3];
     int nc = 0;
     if (p->checkpoint_stride > 0) {
@@ -260,7 +316,7 @@ struct gprfwi_handle {
   const float *eps_r = nullptr, *sigma = nullptr, *wavelet = nullptr;
   void* workspace = nullptr;
   std::vector<float> h_tables;
-  std::vector<int> h_src_off, h_rec_off, h_blk_start, h_blk_rec, h_reg_start, h_reg_rec;
+  std::vector<int> h_src_off, h_blk_start, h_blk_ent, h_reg_start, h_reg_ent;
   bool forward_done = false;
   int64_t launches = 0;
 };
@@ -288,10 +344,10 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
   const Layout& L = h->L;
   const int S = p.nshots, R = p.nrec, ntile = L.f.tiles(), natile = L.a.tiles();
   h->h_src_off.assign(S, 0);
-  h->h_rec_off.assign(std::max(S * R, 1), 0);
   h->h_blk_start.assign((size_t)S * (ntile + 1), 0);
-  h->h_blk_rec.assign(std::max(S * R, 1), 0);
+  h->h_blk_ent.assign((size_t)std::max(S * R, 1) * 2, 0);
   auto ok = [&](int z, int x) { return z >= 1 && z <= p.nz - 2 && x >= 1 && x <= p.nx - 2; };
+  // forward: receivers by OWNING tile; entry = (offset inside the tile's region rowbuf, receiver index)
   for (int s = 0; s < S; ++s) {
     const int z = src_zx[2 * s], x = src_zx[2 * s + 1];
     if (!ok(z, x)) return GPRFWI_EGEOM;
@@ -301,30 +357,48 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
     for (int r = 0; r < R; ++r) {
       const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
       if (!ok(rz, rx)) return GPRFWI_EGEOM;
-      h->h_rec_off[(size_t)s * R + r] = rz * L.pitch + rx;
       tile_of[r] = (rz / L.f.oz) * L.f.tiles_x + rx / kOwnW;
       start[tile_of[r] + 1]++;
     }
     for (int t = 0; t < ntile; ++t) start[t + 1] += start[t];
     std::vector<int> fill(start, start + ntile);
-    for (int r = 0; r < R; ++r) h->h_blk_rec[(size_t)s * R + fill[tile_of[r]]++] = r;
+    for (int r = 0; r < R; ++r) {
+      const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
+      const int ty = rz / L.f.oz, tx = rx / kOwnW;
+      const size_t k = (size_t)s * R + fill[tile_of[r]]++;
+      h->h_blk_ent[2 * k] = (rz - (ty * L.f.oz - L.T)) * kRegW + (rx - (tx * kOwnW - 4));
+      h->h_blk_ent[2 * k + 1] = r;
+    }
   }
-  // receivers by region of the adjoint tiling: a receiver within the halo of a tile is injected there too
+  // adjoint: receivers by REGION (a receiver within the halo of a tile is injected there too)
+  const int arows = kAdjShapes[L.av].rows();
   h->h_reg_start.assign((size_t)S * natile + 1, 0);
-  h->h_reg_rec.clear();
-  for (int s = 0; s < S; ++s)
-    for (int ty = 0; ty < L.a.tiles_y; ++ty)
-      for (int tx = 0; tx < L.a.tiles_x; ++tx) {
-        const int z0 = ty * L.a.oz - L.T, z1 = z0 + AdjShape::ROWS;
-        const int x0 = tx * kOwnW - 4, x1 = x0 + kRegW;
-        for (int r = 0; r < R; ++r) {
-          const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
-          if (rz >= z0 && rz < z1 && rx >= x0 && rx < x1) h->h_reg_rec.push_back(r);
-        }
-        h->h_reg_start[(size_t)s * natile + ty * L.a.tiles_x + tx + 1] = (int)h->h_reg_rec.size();
+  h->h_reg_ent.clear();
+  std::vector<std::vector<int>> bucket(natile);
+  for (int s = 0; s < S; ++s) {
+    for (auto& b : bucket) b.clear();
+    for (int r = 0; r < R; ++r) {
+      const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
+      // tiles ty with ty*oz - T <= rz < ty*oz - T + arows, tx with tx*120 - 4 <= rx < tx*120 + 124
+      const int ty_lo = std::max(0, (rz + L.T - arows) / L.a.oz + ((rz + L.T - arows) >= 0 ? 1 : 0));
+      const int ty_hi = std::min(L.a.tiles_y - 1, (rz + L.T) / L.a.oz);
+      const int tx_lo = std::max(0, (rx + 4 - kRegW) / kOwnW + ((rx + 4 - kRegW) >= 0 ? 1 : 0));
+      const int tx_hi = std::min(L.a.tiles_x - 1, (rx + 4) / kOwnW);
+      for (int ty = ty_lo; ty <= ty_hi; ++ty)
+        for (int tx = tx_lo; tx <= tx_hi; ++tx) bucket[(size_t)ty * L.a.tiles_x + tx].push_back(r);
+    }
+    for (int t = 0; t < natile; ++t) {
+      const int ty = t / L.a.tiles_x, tx = t % L.a.tiles_x;
+      for (int r : bucket[t]) {
+        const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
+        h->h_reg_ent.push_back((rz - (ty * L.a.oz - L.T)) * kRegW + (rx - (tx * kOwnW - 4)));
+        h->h_reg_ent.push_back(r);
       }
-  if (h->h_reg_rec.size() > (size_t)std::max(6 * S * R, 1)) return GPRFWI_EINVAL;
-  if (h->h_reg_rec.empty()) h->h_reg_rec.push_back(0);
+      h->h_reg_start[(size_t)s * natile + t + 1] = (int)(h->h_reg_ent.size() / 2);
+    }
+  }
+  if (h->h_reg_ent.size() / 2 > (size_t)std::max(6 * S * R, 1)) return GPRFWI_EINVAL;
+  if (h->h_reg_ent.empty()) h->h_reg_ent.assign(2, 0);
   return GPRFWI_OK;
 }
 
@@ -351,15 +425,13 @@ static int upload_static(gprfwi_handle* h, cudaStream_t st)
   GPR_CUDA(cudaMemcpyAsync(h->c.tables, t, h->h_tables.size() * sizeof(float), cudaMemcpyHostToDevice, st));
   GPR_CUDA(cudaMemcpyAsync(h->c.src_off, h->h_src_off.data(), h->h_src_off.size() * sizeof(int),
                            cudaMemcpyHostToDevice, st));
-  GPR_CUDA(cudaMemcpyAsync(h->c.rec_off, h->h_rec_off.data(), h->h_rec_off.size() * sizeof(int),
-                           cudaMemcpyHostToDevice, st));
   GPR_CUDA(cudaMemcpyAsync(h->c.blk_start, h->h_blk_start.data(), h->h_blk_start.size() * sizeof(int),
                            cudaMemcpyHostToDevice, st));
-  GPR_CUDA(cudaMemcpyAsync(h->c.blk_rec, h->h_blk_rec.data(), h->h_blk_rec.size() * sizeof(int),
+  GPR_CUDA(cudaMemcpyAsync(h->c.blk_ent, h->h_blk_ent.data(), h->h_blk_ent.size() * sizeof(int),
                            cudaMemcpyHostToDevice, st));
   GPR_CUDA(cudaMemcpyAsync(h->c.reg_start, h->h_reg_start.data(), h->h_reg_start.size() * sizeof(int),
                            cudaMemcpyHostToDevice, st));
-  GPR_CUDA(cudaMemcpyAsync(h->c.reg_rec, h->h_reg_rec.data(), h->h_reg_rec.size() * sizeof(int),
+  GPR_CUDA(cudaMemcpyAsync(h->c.reg_ent, h->h_reg_ent.data(), h->h_reg_ent.size() * sizeof(int),
                            cudaMemcpyHostToDevice, st));
   Geo& g = h->geo;
   g.nz = p.nz; g.nx = p.nx; g.P = p.npml; g.pitch = L.pitch; g.xw = L.xw; g.xnl = L.xnl; g.xur = L.xur;
@@ -372,17 +444,13 @@ static int upload_static(gprfwi_handle* h, cudaStream_t st)
   return GPRFWI_OK;
 }
 
-#ifndef GPR_LAUNCH_SMEM
-#define GPR_LAUNCH_SMEM(kernel, grid, block, smem, stream, ...) kernel<<<grid, block, smem, stream>>>(__VA_ARGS__)
-#endif
-
-static int kernels_init(const gprfwi_params* p)
+static int kernels_init(const gprfwi_params* p, const Layout& L)
 {
   const bool pml = p->npml > 0;
-  GPR_CUDA(cudaFuncSetAttribute(fwd_kernel<GPR_FWD_TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)FwdShape::smem_bytes(pml)));
-  GPR_CUDA(cudaFuncSetAttribute(adj_kernel<GPR_ADJ_TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)AdjShape::smem_bytes(pml)));
+  GPR_CUDA(cudaFuncSetAttribute(kFwdShapes[L.fv].func, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)kFwdShapes[L.fv].smem(pml)));
+  GPR_CUDA(cudaFuncSetAttribute(kAdjShapes[L.av].func, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)kAdjShapes[L.av].smem(pml)));
   return GPRFWI_OK;
 }
 
@@ -404,19 +472,22 @@ static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, 
   a.wav_stride = p.wavelet_per_shot ? p.nt : 0;
   a.wavelet = h->wavelet + n + (size_t)shot0 * a.wav_stride;
   a.src_off = h->c.src_off + shot0;
-  a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
   a.blk_start = h->c.blk_start + (size_t)shot0 * (L.f.tiles() + 1);
-  a.blk_rec = h->c.blk_rec + (size_t)shot0 * p.nrec;
+  a.blk_ent = reinterpret_cast<const int2*>(h->c.blk_ent) + (size_t)shot0 * p.nrec;
   a.trace_stride = (long long)p.nt * p.nrec;
   a.traces = (traces && p.nrec > 0) ? traces + (size_t)shot0 * a.trace_stride + (size_t)n * p.nrec : nullptr;
   a.nrec = p.nrec;
   a.nsub = nsub;
+  a.nshots = ns;
+  a.group = L.fgroup;
   a.tiles_x = L.f.tiles_x;
   a.tiles_y = L.f.tiles_y;
   a.hz = L.T;
   a.oz = L.f.oz;
-  dim3 grid(L.f.tiles_x, L.f.tiles_y, ns), block(FwdShape::THREADS);
-  GPR_LAUNCH_SMEM(fwd_kernel<GPR_FWD_TILE>, grid, block, FwdShape::smem_bytes(p.npml > 0), st, a);
+  const Shape& sh = kFwdShapes[L.fv];
+  dim3 grid(L.f.tiles_x, L.f.tiles_y, (ns + L.fgroup - 1) / L.fgroup), block(sh.threads());
+  void* args[] = {&a};
+  GPR_CUDA(cudaLaunchKernel(sh.func, grid, block, args, sh.smem(p.npml > 0), st));
   h->launches++;
   return GPRFWI_OK;
 }
@@ -441,9 +512,8 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   a.gcb = h->c.gcb;
   a.trace_stride = tstride;
   a.residual = residual ? residual + (size_t)shot0 * tstride + (long long)n_hi * p.nrec : nullptr;
-  a.rec_off = h->c.rec_off + (size_t)shot0 * p.nrec;
   a.reg_start = h->c.reg_start;
-  a.reg_rec = h->c.reg_rec;
+  a.reg_ent = reinterpret_cast<const int2*>(h->c.reg_ent);
   a.nrec = p.nrec;
   a.nsub = nsub;
   a.n_hi = n_hi;
@@ -455,8 +525,10 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   a.hz = L.T;
   a.oz = L.a.oz;
   a.shot_base = shot0;
-  dim3 grid(L.a.tiles_x, L.a.tiles_y, ngrp), block(AdjShape::THREADS);
-  GPR_LAUNCH_SMEM(adj_kernel<GPR_ADJ_TILE>, grid, block, AdjShape::smem_bytes(p.npml > 0), st, a);
+  const Shape& sh = kAdjShapes[L.av];
+  dim3 grid(L.a.tiles_x, L.a.tiles_y, ngrp), block(sh.threads());
+  void* args[] = {&a};
+  GPR_CUDA(cudaLaunchKernel(sh.func, grid, block, args, sh.smem(p.npml > 0), st));
   h->launches++;
   return GPRFWI_OK;
 }
@@ -556,7 +628,7 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
   // fields are zero at n = 0
   GPR_CUDA(cudaMemsetAsync(h->c.fscratch, 0, 2 * S * L.full * f, st));
   float* slot[2] = {h->c.fscratch, h->c.fscratch + S * L.full};
-  rc = kernels_init(p);
+  rc = kernels_init(p, L);
   if (rc != GPRFWI_OK) return rc;
   if (L.full_history) GPR_CUDA(cudaMemsetAsync(h->c.hist, 0, S * L.plane * f, st));
   else GPR_CUDA(cudaMemsetAsync(h->c.ckpt, 0, S * L.full * f, st));       // checkpoint 0 = zero state

@@ -27,9 +27,8 @@ struct AdjArgs {
   float *gca, *gcb;                   // [ngroups][nz][pitch]
   const float* residual;              // sample n_hi of local shot 0 (sample n_hi - t at - t*nrec)
   long long trace_stride;             // nt * nrec
-  const int* rec_off;                 // [S][nrec]
   const int* reg_start;               // [S*tiles + 1] CSR of receivers by REGION (tile + halo)
-  const int* reg_rec;
+  const int2* reg_ent;                // in CSR order: (row*128 + column inside the region, receiver index)
   int nrec, nsub, n_hi, nt;
   int nshots, group;
   int tiles_x, tiles_y;
@@ -39,17 +38,23 @@ struct AdjArgs {
 
 #if defined(__CUDACC__)
 // transpose of recording: residual sample n_hi - t enters lamE at the start of reverse step n_hi-1-t;
-// it is staged in rowbuf (zero between uses) one barrier ahead of its use
+// it is staged in rowbuf (zero between uses) one barrier ahead of its use.  The receivers of the
+// region are dealt out one per thread (entry + its residual samples in registers).
 template <int R, int NW>
-__device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1, int t)
+__device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
+                                          int2 ent, const float (&rv)[kMaxT], int t)
 {
   using L = RegTile<R, NW, 3>;
   if (a.n_hi - t >= a.nt) return;
-  for (int k = rk0 + threadIdx.x; k < rk1; k += L::THREADS) {
-    const int rr = a.reg_rec[k];
-    const int off = a.rec_off[(long long)s * a.nrec + rr];
-    atomicAdd(c.rowbuf_() + (off / a.g.pitch - c.rj0) * kRegW + (off % a.g.pitch - c.ri0),   // coincident receivers sum
-              a.residual[s * a.trace_stride - (long long)t * a.nrec + rr]);
+  if (ent.x >= 0) {
+    float v = rv[0];
+#pragma unroll
+    for (int k = 1; k < kMaxT; ++k) v = t == k ? rv[k] : v;
+    atomicAdd(c.rowbuf_() + ent.x, v);                                 // coincident receivers sum
+  }
+  for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {   // more receivers than threads
+    const int2 e2 = a.reg_ent[k];
+    atomicAdd(c.rowbuf_() + e2.x, a.residual[s * a.trace_stride - (long long)t * a.nrec + e2.y]);
   }
 }
 
@@ -72,7 +77,7 @@ __device__ __forceinline__ void adj_fetch(const AdjArgs& a, const TileCtx<R, NW,
 // exactly tx = q, tz = -q, sx, sz = +-Db lamH with the trivial coefficients outside the CPML).
 template <int R, int NW, bool ZP, bool XP>
 __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
-                                          unsigned iflags, float (&le)[R][4], float (&lhx)[R][4], float (&lhy)[R][4],
+                                          int2 ent, const float (&rv)[kMaxT], unsigned iflags, float (&le)[R][4], float (&lhx)[R][4], float (&lhy)[R][4],
                                           const float (&ca)[R][4], const float (&cb)[R][4],
                                           float (&ga)[R][4], float (&gb)[R][4])
 {
@@ -161,7 +166,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
 #pragma unroll
     for (int q = 0; q < 4; ++q) tz0[q] = tzp[q];
     __syncthreads();
-    if (t + 1 < a.nsub) adj_stage<R, NW>(a, c, s, rk0, rk1, t + 1);
+    if (t + 1 < a.nsub) adj_stage<R, NW>(a, c, s, rk0, rk1, ent, rv, t + 1);
     {
       float tzb[4];                                   // tz of the row below the warp's last row
       lds4a(c.xe_() + (c.w + 1) * kRegW + c.l4, tzb);
@@ -236,8 +241,6 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   TileCtx<R, NW, 3> c;
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
   const int grp = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
-  const unsigned full = 0xffffffffu;
-
   c.template stage_tables<false>(g);
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
     reinterpret_cast<float4*>(c.rowbuf_())[k] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -255,16 +258,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
 
   const int s_end = min((grp + 1) * a.group, a.nshots);
   for (int s = grp * a.group; s < s_end; ++s) {
-    __syncthreads();                   // the previous shot is done with shared memory; rowbuf is all zero
-    // receivers of this shot inside the region: which of this warp's rows they touch
+    // ---- everything this shot needs from global memory, issued together ----------------------------
     const long long row = (long long)(a.shot_base + s) * (a.tiles_x * a.tiles_y) + tile;
     const int rk0 = a.reg_start[row], rk1 = a.reg_start[row + 1];
-    unsigned iflags = 0u;
-    for (int k = rk0 + c.lane; k < rk1; k += 32) {
-      const int lj = a.rec_off[(long long)s * a.nrec + a.reg_rec[k]] / g.pitch - c.gj0;
-      if (lj >= 0 && lj < R) iflags |= 1u << lj;
-    }
-    iflags = __reduce_or_sync(full, iflags);
     float le[R][4], lhx[R][4], lhy[R][4];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -278,14 +274,33 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
     }
     adj_fetch<R, NW>(a, c, s, 0);
     adj_fetch<R, NW>(a, c, s, 1);
+    if (threadIdx.x < 2) c.mask_()[threadIdx.x] = 0u;
     if (c.zp || c.xp) c.load_psi(g, a.in, s);
-    adj_stage<R, NW>(a, c, s, rk0, rk1, 0);
+    // the receiver this thread injects, with its residual samples of this launch
+    int2 ent = make_int2(-1, 0);
+    float rv[kMaxT];
+#pragma unroll
+    for (int t = 0; t < kMaxT; ++t) rv[t] = 0.f;
+    if (rk0 + (int)threadIdx.x < rk1) {
+      ent = a.reg_ent[rk0 + threadIdx.x];
+#pragma unroll
+      for (int t = 0; t < kMaxT; ++t)
+        if (t < a.nsub && a.n_hi - t < a.nt) rv[t] = a.residual[s * a.trace_stride - (long long)t * a.nrec + ent.y];
+    }
+    __syncthreads();                   // mask zeroed; the previous shot left rowbuf all zero
+    if (ent.x >= 0) atomicOr(c.mask_() + ((ent.x / kRegW) >> 5), 1u << ((ent.x / kRegW) & 31));
+    for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {
+      const int rw = a.reg_ent[k].x / kRegW;
+      atomicOr(c.mask_() + (rw >> 5), 1u << (rw & 31));
+    }
+    adj_stage<R, NW>(a, c, s, rk0, rk1, ent, rv, 0);
     __syncthreads();
+    const unsigned iflags = c.row_flags();
 
-    if (c.zp && c.xp) adj_steps<R, NW, true, true>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
-    else if (c.zp) adj_steps<R, NW, true, false>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
-    else if (c.xp) adj_steps<R, NW, false, true>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
-    else adj_steps<R, NW, false, false>(a, c, s, rk0, rk1, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    if (c.zp && c.xp) adj_steps<R, NW, true, true>(a, c, s, rk0, rk1, ent, rv, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    else if (c.zp) adj_steps<R, NW, true, false>(a, c, s, rk0, rk1, ent, rv, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    else if (c.xp) adj_steps<R, NW, false, true>(a, c, s, rk0, rk1, ent, rv, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    else adj_steps<R, NW, false, false>(a, c, s, rk0, rk1, ent, rv, iflags, le, lhx, lhy, ca, cb, ga, gb);
 
     // ---- write back the owned part of the adjoint state ------------------------------------------------
 #pragma unroll

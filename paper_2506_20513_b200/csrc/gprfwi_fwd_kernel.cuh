@@ -27,22 +27,28 @@ struct FwdArgs {
   const float* wavelet;       // sample n of local shot 0
   long long wav_stride;       // nt or 0
   const int* src_off;         // [S] j*pitch + i
-  const int* rec_off;         // [S][nrec]
   const int* blk_start;       // [S][tiles + 1] CSR of receivers by owning tile
-  const int* blk_rec;         // [S][nrec]
+  const int2* blk_ent;        // [S][nrec] in CSR order: (row*128 + column inside the tile's region, receiver index)
   float* traces;              // sample n of local shot 0 (NULL: do not record)
   long long trace_stride;     // nt * nrec
   int nrec, nsub;             // receivers per shot; steps in this launch (<= hz)
+  int nshots, group;          // shots in this launch; shots swept by one CTA, one after the other
   int tiles_x, tiles_y;
   int hz, oz;                 // halo rows; owned rows per tile (= NW*R - 2*hz)
 };
 
 #if defined(__CUDACC__)
+#ifdef GPRFWI_TIMING
+__device__ unsigned long long g_tcount = 0;
+#define TICK(k) do { if (dbg) tk[k] = clock64(); } while (0)
+#else
+#define TICK(k)
+#endif
 // The T-step loop of one warp.  All variants hit the same barriers, so the warps of one CTA may run
 // different variants.
 template <int R, int NW, bool ZP, bool XP>
 __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>& c, int s, int rk0, int rk1,
-                                          unsigned rflags, int src_r, int src_c,
+                                          int2 ent, unsigned rflags, int src_r, int src_c, const float (&wv)[kMaxT],
                                           float (&e)[R][4], float (&hx)[R][4], float (&hy)[R][4],
                                           const float (&ca)[R][4], const float (&cb)[R][4])
 {
@@ -50,18 +56,13 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
   const Geo& g = a.g;
   const unsigned full = 0xffffffffu;
   const float rdx = g.rdx, Db = g.Db, kap = g.kap;
-  float wv[kMaxT];
-#pragma unroll
-  for (int t = 0; t < kMaxT; ++t) wv[t] = t < a.nsub ? a.wavelet[s * a.wav_stride + t] * (rdx * rdx) : 0.f;
-
 #pragma unroll 1
   for (int t = 0; t < a.nsub; ++t) {
     // ---- stage 1: trace sample n + t from the published receiver rows ----------------------------
-    for (int k = rk0 + threadIdx.x; k < rk1; k += L::THREADS) {
-      const int rr = a.blk_rec[(long long)s * a.nrec + k];
-      const int off = a.rec_off[(long long)s * a.nrec + rr];
-      a.traces[s * a.trace_stride + (long long)t * a.nrec + rr] =
-          c.rowbuf_()[(off / g.pitch - c.rj0) * kRegW + (off % g.pitch - c.ri0)];
+    if (ent.x >= 0) a.traces[s * a.trace_stride + (long long)t * a.nrec + ent.y] = c.rowbuf_()[ent.x];
+    for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {      // more receivers than threads
+      const int2 en2 = a.blk_ent[(long long)s * a.nrec + k];
+      a.traces[s * a.trace_stride + (long long)t * a.nrec + en2.y] = c.rowbuf_()[en2.x];
     }
 
     // ---- stages 2-3: H update + H CPML -------------------------------------------------------------
@@ -175,68 +176,108 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
 template <int R, int NW, int MINB>
 __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
 {
+  using L = RegTile<R, NW>;
   extern __shared__ float4 smem4[];
   const Geo& g = a.g;
   TileCtx<R, NW> c;
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
-  const int s = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
-  const unsigned full = 0xffffffffu;
+  const int tile = blockIdx.y * a.tiles_x + blockIdx.x, ntile = a.tiles_x * a.tiles_y;
+  const int s0 = blockIdx.z * a.group, s1 = min(s0 + a.group, a.nshots);
+#ifdef GPRFWI_TIMING
+  long long tk[12];
+  bool dbg = false;
+  if (blockIdx.x == 1 && blockIdx.y == 3 && blockIdx.z == 0 && threadIdx.x == 64) dbg = (atomicAdd(&g_tcount, 1ULL) == 300ULL);
+  TICK(0);
+#endif
 
+  // once per CTA: CPML tables -> shared memory, Ca / Cb of the region -> registers
   c.template stage_tables<true>(g);
-
-  // rows of this warp that hold receivers owned by this tile (warp-uniform bit mask)
-  unsigned rflags = 0u;
-  const int* rs = a.blk_start + (long long)s * (a.tiles_x * a.tiles_y + 1);
-  const int rk0 = a.traces ? rs[tile] : 0, rk1 = a.traces ? rs[tile + 1] : 0;
-  for (int k = rk0 + c.lane; k < rk1; k += 32) {
-    const int lj = a.rec_off[(long long)s * a.nrec + a.blk_rec[(long long)s * a.nrec + k]] / g.pitch - c.gj0;
-    if (lj >= 0 && lj < R) rflags |= 1u << lj;
-  }
-  rflags = __reduce_or_sync(full, rflags);
-
-  // the source cell, if this thread holds it
-  int src_r = -1, src_c = 0;
-  {
-    const int src = a.src_off[s];
-    const int dj = src / g.pitch - c.gj0, di = src % g.pitch - c.gi;
-    if (dj >= 0 && dj < R && di >= 0 && di < 4) { src_r = dj; src_c = di; }
-  }
-
-  // ---- load the region into registers ------------------------------------------------------------
-  float e[R][4], hx[R][4], hy[R][4], ca[R][4], cb[R][4];
+  float ca[R][4], cb[R][4];
 #pragma unroll
   for (int r = 0; r < R; ++r) {
-    zero4(e[r]); zero4(hx[r]); zero4(hy[r]); zero4(ca[r]); zero4(cb[r]);
+    zero4(ca[r]); zero4(cb[r]);
     if (c.colin && ((c.rin >> r) & 1u)) {
       const long long o = (long long)(c.gj0 + r) * g.pitch + c.gi;
-      ldg4a(a.in.ez + s * g.plane + o, e[r]);
-      ldg4a(a.in.hx + s * g.plane + o, hx[r]);
-      ldg4a(a.in.hy + s * g.plane + o, hy[r]);
       ldg4a(a.ca + o, ca[r]);
       ldg4a(a.cb + o, cb[r]);
     }
   }
-  if (c.zp || c.xp) c.load_psi(g, a.in, s);
-  st4a(c.xe_() + c.w * kRegW + c.l4, e[0]);
-#pragma unroll
-  for (int r = 0; r < R; ++r)
-    if ((rflags >> r) & 1u) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
-  __syncthreads();
 
-  if (c.zp && c.xp) fwd_steps<R, NW, true, true>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
-  else if (c.zp) fwd_steps<R, NW, true, false>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
-  else if (c.xp) fwd_steps<R, NW, false, true>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
-  else fwd_steps<R, NW, false, false>(a, c, s, rk0, rk1, rflags, src_r, src_c, e, hx, hy, ca, cb);
-
-  // ---- write back what this tile owns (out.ez was written by the last E phase) ----------------------
+  TICK(1);
+#pragma unroll 1
+  for (int s = s0; s < s1; ++s) {
+    TICK(2);
+    // ---- everything this shot needs from global memory, issued together ----------------------------
+    const int rk0 = a.traces ? a.blk_start[(long long)s * (ntile + 1) + tile] : 0;
+    const int rk1 = a.traces ? a.blk_start[(long long)s * (ntile + 1) + tile + 1] : 0;
+    const int src = a.src_off[s];
+    float wv[kMaxT];
 #pragma unroll
-  for (int r = 0; r < R; ++r) {
-    if (!((c.own >> r) & 1u)) continue;
-    const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-    st4a(a.out.hx + o, hx[r]);
-    st4a(a.out.hy + o, hy[r]);
+    for (int t = 0; t < kMaxT; ++t) wv[t] = t < a.nsub ? a.wavelet[s * a.wav_stride + t] : 0.f;
+    float e[R][4], hx[R][4], hy[R][4];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      zero4(e[r]); zero4(hx[r]); zero4(hy[r]);
+      if (c.colin && ((c.rin >> r) & 1u)) {
+        const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
+        ldg4a(a.in.ez + o, e[r]);
+        ldg4a(a.in.hx + o, hx[r]);
+        ldg4a(a.in.hy + o, hy[r]);
+      }
+    }
+    // (the previous shot's last barrier already fenced its use of rowbuf and the exchange slots; psi,
+    // rowbuf and exchange slots are rewritten below by the threads that own them)
+    if (threadIdx.x < 2) c.mask_()[threadIdx.x] = 0u;
+    if (c.zp || c.xp) c.load_psi(g, a.in, s);
+    // the receiver this thread records (receivers of the tile are dealt out one per thread)
+    int2 ent = make_int2(-1, 0);
+    if (rk0 + (int)threadIdx.x < rk1) ent = a.blk_ent[(long long)s * a.nrec + rk0 + threadIdx.x];
+    // the source cell, if this thread holds it
+    int src_r = -1, src_c = 0;
+    {
+      const int dj = src / g.pitch - c.gj0, di = src % g.pitch - c.gi;
+      if (dj >= 0 && dj < R && di >= 0 && di < 4) { src_r = dj; src_c = di; }
+    }
+#pragma unroll
+    for (int t = 0; t < kMaxT; ++t) wv[t] *= g.rdx * g.rdx;
+    TICK(3);
+    // publish: row 0 for the warp above, all rows for the first trace sample
+    st4a(c.xe_() + c.w * kRegW + c.l4, e[0]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
+    TICK(4);
+    __syncthreads();                   // mask zeroed
+    TICK(5);
+    if (ent.x >= 0) atomicOr(c.mask_() + ((ent.x / kRegW) >> 5), 1u << ((ent.x / kRegW) & 31));
+    for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {
+      const int row = a.blk_ent[(long long)s * a.nrec + k].x / kRegW;
+      atomicOr(c.mask_() + (row >> 5), 1u << (row & 31));
+    }
+    __syncthreads();
+    const unsigned rflags = c.row_flags();
+    TICK(6);
+
+    if (c.zp && c.xp) fwd_steps<R, NW, true, true>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
+    else if (c.zp) fwd_steps<R, NW, true, false>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
+    else if (c.xp) fwd_steps<R, NW, false, true>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
+    else fwd_steps<R, NW, false, false>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
+
+    TICK(7);
+    // ---- write back what this tile owns (out.ez was written by the last E phase) --------------------
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      if (!((c.own >> r) & 1u)) continue;
+      const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
+      st4a(a.out.hx + o, hx[r]);
+      st4a(a.out.hy + o, hy[r]);
+    }
+    if (c.zp || c.xp) c.store_psi(g, a.out, s);
+    TICK(8);
+#ifdef GPRFWI_TIMING
+    if (dbg) printf("TIMING shot %d: setup %lld | issue-loads %lld | loads-arrive %lld | bar1 %lld | mask+bar2 %lld | steps(%d) %lld | stores %lld\n",
+                    s, tk[1] - tk[0], tk[3] - tk[2], tk[4] - tk[3], tk[5] - tk[4], tk[6] - tk[5], a.nsub, tk[7] - tk[6], tk[8] - tk[7]);
+#endif
   }
-  if (c.zp || c.xp) c.store_psi(g, a.out, s);
 }
 #endif
 

@@ -20,6 +20,7 @@
 //                     the adjoint stages the residual there for injection
 //   tabx [6][128]     CPML x tables of the region's columns: bhx chx khx bex cex kex
 //   tabz [6][NW*R]    CPML z tables of the region's rows:    bhz chz khz bez cez kez
+//   mask [2]          bit j: region row j holds a receiver of the current shot
 //   hist [NH][NW*R][128] adjoint only: ring of forward Ez planes fetched ahead with cp.async, thread-private
 //   psi  [4][NW*R][128]  CPML psi of the region, thread-private (only when npml > 0): hz ez hx ex
 #pragma once
@@ -40,7 +41,8 @@ struct RegTile {
   static constexpr int ROWBUF = XH + (NW + 1) * kRegW;
   static constexpr int TABX = ROWBUF + ROWS * kRegW;
   static constexpr int TABZ = TABX + 6 * kRegW;
-  static constexpr int HIST = (TABZ + 6 * ROWS + 3) / 4 * 4;
+  static constexpr int MASK = TABZ + 6 * ROWS;                 // 2 words: rows of the region that hold receivers
+  static constexpr int HIST = (MASK + 2 + 3) / 4 * 4;
   static constexpr int PSI = HIST + NH * ROWS * kRegW;
   GPR_HD static size_t smem_bytes(bool pml) { return sizeof(float) * (size_t)(PSI + (pml ? 4 * ROWS * kRegW : 0)); }
 };
@@ -107,6 +109,13 @@ struct TileCtx {
   __device__ __forceinline__ float* rowbuf_() const { return sm + L::ROWBUF; }
   __device__ __forceinline__ float* tabx_() const { return sm + L::TABX; }
   __device__ __forceinline__ float* tabz_() const { return sm + L::TABZ; }
+  __device__ __forceinline__ unsigned* mask_() const { return reinterpret_cast<unsigned*>(sm + L::MASK); }
+  // this warp's R bits of the receiver-row mask (valid after the barrier that follows the atomicOr's)
+  __device__ __forceinline__ unsigned row_flags() const
+  {
+    const unsigned long long m = (unsigned long long)mask_()[0] | ((unsigned long long)mask_()[1] << 32);
+    return (unsigned)(m >> lr0) & ((1u << R) - 1u);
+  }
   __device__ __forceinline__ float* hist_() const { return sm + L::HIST + toff; }
   __device__ __forceinline__ float* phz_() const { return sm + L::PSI + 0 * L::ROWS * kRegW + toff; }
   __device__ __forceinline__ float* pez_() const { return sm + L::PSI + 1 * L::ROWS * kRegW + toff; }
