@@ -61,8 +61,8 @@ struct Shape {
 template <int R, int NW, int MINB>
 static Shape fwd_shape()
 {
-  return {R, NW, MINB, (const void*)fwd_kernel<R, NW, MINB>, RegTile<R, NW, 0>::smem_bytes(true),
-          RegTile<R, NW, 0>::smem_bytes(false)};
+  return {R, NW, MINB, (const void*)fwd_kernel<R, NW, MINB>, RegTile<R, NW, 3>::smem_bytes(true),
+          RegTile<R, NW, 3>::smem_bytes(false)};
 }
 template <int R, int NW, int MINB>
 static Shape adj_shape()
@@ -174,8 +174,7 @@ static int env_int(const char* name, int dflt)
 static void set_groups(const gprfwi_params* p, Layout& L)
 {
   const int fslots = 148 * std::max(1, kFwdShapes[L.fv].minb), aslots = 148 * std::max(1, kAdjShapes[L.av].minb);
-  (void)fslots;
-  L.fgroup = 1; L.fngroups = p->nshots;          // forward: one shot per CTA (shots of a CTA run back to back, unoverlapped)
+  pick_groups(L.f.tiles(), p->nshots, fslots, 0.5, L.fgroup, L.fngroups);
   pick_groups(L.a.tiles(), L.Sb, aslots, 1.0, L.group, L.ngroups);
   if (int g = env_int("GPRFWI_FWD_GROUP", 0)) { L.fgroup = std::min(g, p->nshots); L.fngroups = (p->nshots + L.fgroup - 1) / L.fgroup; }
   if (int g = env_int("GPRFWI_ADJ_GROUP", 0)) { L.group = std::min(g, L.Sb); L.ngroups = (L.Sb + L.group - 1) / L.group; }

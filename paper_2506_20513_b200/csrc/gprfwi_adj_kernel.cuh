@@ -138,7 +138,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
         }
         st4a(c.pez_() + r * kRegW, p);
       }
-      if (XP) {
+      if (XP && c.xslot >= 0) {          // lanes off the x CPML keep tx = q
         float p[4], b[4], cc[4], ik[4];
         lds4a(c.pex_() + r * kRegW, p);
         lds4a(c.tabx_() + 3 * kRegW + c.l4, b); lds4a(c.tabx_() + 4 * kRegW + c.l4, cc); lds4a(c.tabx_() + 5 * kRegW + c.l4, ik);
@@ -193,7 +193,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
         }
         st4a(c.phz_() + r * kRegW, p);
       }
-      if (XP) {
+      if (XP && c.xslot >= 0) {          // lanes off the x CPML keep sx = Db lamHy
         float p[4], b[4], cc[4], ik[4];
         lds4a(c.phx_() + r * kRegW, p);
         lds4a(c.tabx_() + 0 * kRegW + c.l4, b); lds4a(c.tabx_() + 1 * kRegW + c.l4, cc); lds4a(c.tabx_() + 2 * kRegW + c.l4, ik);
@@ -242,6 +242,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
   const int grp = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
   c.template stage_tables<false>(g);
+  c.zero_psi(g);
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
     reinterpret_cast<float4*>(c.rowbuf_())[k] = make_float4(0.f, 0.f, 0.f, 0.f);
 
@@ -275,7 +276,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
     adj_fetch<R, NW>(a, c, s, 0);
     adj_fetch<R, NW>(a, c, s, 1);
     if (threadIdx.x < 2) c.mask_()[threadIdx.x] = 0u;
-    if (c.zp || c.xp) c.load_psi(g, a.in, s);
+    c.fetch_psi(g, a.in, s);           // lands with the history planes: step 0 waits for all but the newest group
     // the receiver this thread injects, with its residual samples of this launch
     int2 ent = make_int2(-1, 0);
     float rv[kMaxT];

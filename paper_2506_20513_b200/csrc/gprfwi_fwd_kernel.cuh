@@ -38,21 +38,15 @@ struct FwdArgs {
 };
 
 #if defined(__CUDACC__)
-#ifdef GPRFWI_TIMING
-__device__ unsigned long long g_tcount = 0;
-#define TICK(k) do { if (dbg) tk[k] = clock64(); } while (0)
-#else
-#define TICK(k)
-#endif
 // The T-step loop of one warp.  All variants hit the same barriers, so the warps of one CTA may run
 // different variants.
 template <int R, int NW, bool ZP, bool XP>
-__device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>& c, int s, int rk0, int rk1,
+__device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
                                           int2 ent, unsigned rflags, int src_r, int src_c, const float (&wv)[kMaxT],
                                           float (&e)[R][4], float (&hx)[R][4], float (&hy)[R][4],
                                           const float (&ca)[R][4], const float (&cb)[R][4])
 {
-  using L = RegTile<R, NW>;
+  using L = RegTile<R, NW, 3>;
   const Geo& g = a.g;
   const unsigned full = 0xffffffffu;
   const float rdx = g.rdx, Db = g.Db, kap = g.kap;
@@ -66,8 +60,11 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
     }
 
     // ---- stages 2-3: H update + H CPML -------------------------------------------------------------
-    float xb[4], xc[4], xk[4];                          // x tables of this lane's columns (XP only)
-    if (XP) { lds4a(c.tabx_() + 0 * kRegW + c.l4, xb); lds4a(c.tabx_() + 1 * kRegW + c.l4, xc); lds4a(c.tabx_() + 2 * kRegW + c.l4, xk); }
+    // x tables of this lane's columns (XP only; lanes off the CPML use the trivial coefficients
+    // and a psi of zero without touching shared memory)
+    float xb[4] = {0.f, 0.f, 0.f, 0.f}, xc[4] = {0.f, 0.f, 0.f, 0.f}, xk[4] = {kap, kap, kap, kap};
+    const bool xl = XP && c.xslot >= 0;
+    if (xl) { lds4a(c.tabx_() + 0 * kRegW + c.l4, xb); lds4a(c.tabx_() + 1 * kRegW + c.l4, xc); lds4a(c.tabx_() + 2 * kRegW + c.l4, xk); }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       float eb[4];                                      // Ez of the row below
@@ -91,15 +88,15 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
         for (int q = 0; q < 4; ++q) hx[r][q] = FF(-kap, FS(eb[q], e[r][q]), hx[r][q]);
       }
       if (XP) {
-        float p[4];
-        lds4a(c.phx_() + r * kRegW, p);
+        float p[4] = {0.f, 0.f, 0.f, 0.f};
+        if (xl) lds4a(c.phx_() + r * kRegW, p);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           const float d = FS(en[q], e[r][q]);
           p[q] = FF(xb[q], p[q], FM(xc[q], d));
           hy[r][q] = FF(Db, p[q], FF(xk[q], d, hy[r][q]));
         }
-        st4a(c.phx_() + r * kRegW, p);
+        if (xl) st4a(c.phx_() + r * kRegW, p);
       } else {
 #pragma unroll
         for (int q = 0; q < 4; ++q) hy[r][q] = FF(kap, FS(en[q], e[r][q]), hy[r][q]);
@@ -109,7 +106,8 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
     __syncthreads();
 
     // ---- stages 4-7: E update + E CPML, source, save wavefield --------------------------------------
-    if (XP) { lds4a(c.tabx_() + 3 * kRegW + c.l4, xb); lds4a(c.tabx_() + 4 * kRegW + c.l4, xc); lds4a(c.tabx_() + 5 * kRegW + c.l4, xk); }
+    if (XP) { xk[0] = xk[1] = xk[2] = xk[3] = 1.f; }
+    if (xl) { lds4a(c.tabx_() + 3 * kRegW + c.l4, xb); lds4a(c.tabx_() + 4 * kRegW + c.l4, xc); lds4a(c.tabx_() + 5 * kRegW + c.l4, xk); }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       float ha[4];                                      // Hx of the row above
@@ -117,13 +115,13 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
       else lds4a(c.xh_() + c.w * kRegW + c.l4, ha);
       const float hl[4] = {__shfl_up_sync(full, hy[r][3], 1), hy[r][0], hy[r][1], hy[r][2]};  // Hy to the left
       if (ZP || XP) {
-        float pz[4], px[4];
+        float pz[4], px[4] = {0.f, 0.f, 0.f, 0.f};
         float bz = 0.f, cz = 0.f, kz = 1.f;
         if (ZP) {
           lds4a(c.pez_() + r * kRegW, pz);
           bz = c.tabz_()[3 * L::ROWS + c.lr0 + r]; cz = c.tabz_()[4 * L::ROWS + c.lr0 + r]; kz = c.tabz_()[5 * L::ROWS + c.lr0 + r];
         }
-        if (XP) lds4a(c.pex_() + r * kRegW, px);
+        if (xl) lds4a(c.pex_() + r * kRegW, px);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           const float tx = FS(hy[r][q], hl[q]), tz = FS(hx[r][q], ha[q]);
@@ -136,7 +134,7 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
           e[r][q] = FF(cb[r][q], FF(dd, rdx, pp), FM(ca[r][q], e[r][q]));
         }
         if (ZP) st4a(c.pez_() + r * kRegW, pz);
-        if (XP) st4a(c.pex_() + r * kRegW, px);
+        if (xl) st4a(c.pex_() + r * kRegW, px);
       } else {
 #pragma unroll
         for (int q = 0; q < 4; ++q)
@@ -173,25 +171,50 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW>
   }
 }
 
+// per-shot scalars, word k of 8: receiver range [rk0, rk1) of the tile, source offset, 4 wavelet samples
+__device__ __forceinline__ int fwd_meta_word(const FwdArgs& a, int s, int tile, int ntile, int k)
+{
+  if (k == 0) return a.traces ? a.blk_start[(long long)s * (ntile + 1) + tile] : 0;
+  if (k == 1) return a.traces ? a.blk_start[(long long)s * (ntile + 1) + tile + 1] : 0;
+  if (k == 2) return a.src_off[s];
+  return (k - 3 < a.nsub) ? __float_as_int(a.wavelet[s * a.wav_stride + (k - 3)]) : 0;
+}
+
+// Ez, Hx, Hy of shot s (this thread's cells) -> the thread's landing slots, one commit group
+template <int R, int NW>
+__device__ __forceinline__ void fwd_fetch(const FwdArgs& a, const TileCtx<R, NW, 3>& c, int s)
+{
+  using L = RegTile<R, NW, 3>;
+  const Geo& g = a.g;
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+    if (c.colin && ((c.rin >> r) & 1u)) {
+      const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
+      cp_async16(c.hist_() + 0 * L::ROWS * kRegW + r * kRegW, a.in.ez + o);
+      cp_async16(c.hist_() + 1 * L::ROWS * kRegW + r * kRegW, a.in.hx + o);
+      cp_async16(c.hist_() + 2 * L::ROWS * kRegW + r * kRegW, a.in.hy + o);
+    }
+  cp_async_commit();
+}
+
 template <int R, int NW, int MINB>
 __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
 {
-  using L = RegTile<R, NW>;
+  using L = RegTile<R, NW, 3>;
   extern __shared__ float4 smem4[];
   const Geo& g = a.g;
-  TileCtx<R, NW> c;
+  TileCtx<R, NW, 3> c;
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
   const int tile = blockIdx.y * a.tiles_x + blockIdx.x, ntile = a.tiles_x * a.tiles_y;
   const int s0 = blockIdx.z * a.group, s1 = min(s0 + a.group, a.nshots);
-#ifdef GPRFWI_TIMING
-  long long tk[12];
-  bool dbg = false;
-  if (blockIdx.x == 1 && blockIdx.y == 3 && blockIdx.z == 0 && threadIdx.x == 64) dbg = (atomicAdd(&g_tcount, 1ULL) == 300ULL);
-  TICK(0);
-#endif
+  const int tid = threadIdx.x;
 
-  // once per CTA: CPML tables -> shared memory, Ca / Cb of the region -> registers
+  // once per CTA: first shot's fields and scalars on their way, CPML tables -> shared memory,
+  // Ca / Cb of the region -> registers
+  fwd_fetch<R, NW>(a, c, s0);
+  if (tid < 7) c.meta_()[tid] = fwd_meta_word(a, s0, tile, ntile, tid);
   c.template stage_tables<true>(g);
+  c.zero_psi(g);
   float ca[R][4], cb[R][4];
 #pragma unroll
   for (int r = 0; r < R; ++r) {
@@ -202,67 +225,68 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
       ldg4a(a.cb + o, cb[r]);
     }
   }
+  __syncthreads();
+  // the receiver this thread records (receivers of the tile are dealt out one per thread)
+  int2 ent_next = make_int2(-1, 0);
+  if (c.meta_()[0] + tid < c.meta_()[1]) ent_next = a.blk_ent[(long long)s0 * a.nrec + c.meta_()[0] + tid];
 
-  TICK(1);
 #pragma unroll 1
   for (int s = s0; s < s1; ++s) {
-    TICK(2);
-    // ---- everything this shot needs from global memory, issued together ----------------------------
-    const int rk0 = a.traces ? a.blk_start[(long long)s * (ntile + 1) + tile] : 0;
-    const int rk1 = a.traces ? a.blk_start[(long long)s * (ntile + 1) + tile + 1] : 0;
-    const int src = a.src_off[s];
+    const int* m = c.meta_() + ((s - s0) & 1) * 8;
+    const int rk0 = m[0], rk1 = m[1], src = m[2];
     float wv[kMaxT];
 #pragma unroll
-    for (int t = 0; t < kMaxT; ++t) wv[t] = t < a.nsub ? a.wavelet[s * a.wav_stride + t] : 0.f;
-    float e[R][4], hx[R][4], hy[R][4];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-      zero4(e[r]); zero4(hx[r]); zero4(hy[r]);
-      if (c.colin && ((c.rin >> r) & 1u)) {
-        const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-        ldg4a(a.in.ez + o, e[r]);
-        ldg4a(a.in.hx + o, hx[r]);
-        ldg4a(a.in.hy + o, hy[r]);
-      }
-    }
-    // (the previous shot's last barrier already fenced its use of rowbuf and the exchange slots; psi,
-    // rowbuf and exchange slots are rewritten below by the threads that own them)
-    if (threadIdx.x < 2) c.mask_()[threadIdx.x] = 0u;
-    if (c.zp || c.xp) c.load_psi(g, a.in, s);
-    // the receiver this thread records (receivers of the tile are dealt out one per thread)
-    int2 ent = make_int2(-1, 0);
-    if (rk0 + (int)threadIdx.x < rk1) ent = a.blk_ent[(long long)s * a.nrec + rk0 + threadIdx.x];
+    for (int t = 0; t < kMaxT; ++t) wv[t] = __int_as_float(m[3 + t]) * (g.rdx * g.rdx);
+    const int2 ent = ent_next;
     // the source cell, if this thread holds it
     int src_r = -1, src_c = 0;
     {
       const int dj = src / g.pitch - c.gj0, di = src % g.pitch - c.gi;
       if (dj >= 0 && dj < R && di >= 0 && di < 4) { src_r = dj; src_c = di; }
     }
+    // ---- this shot's fields have landed in the thread's slots: move them to registers ---------------
+    float e[R][4], hx[R][4], hy[R][4];
+    c.fetch_psi(g, a.in, s);           // (the previous shot's psi went out in its store_psi)
+    cp_async_wait<1>();                // fields: landed; psi: on its way
 #pragma unroll
-    for (int t = 0; t < kMaxT; ++t) wv[t] *= g.rdx * g.rdx;
-    TICK(3);
+    for (int r = 0; r < R; ++r) {
+      zero4(e[r]); zero4(hx[r]); zero4(hy[r]);
+      if (c.colin && ((c.rin >> r) & 1u)) {
+        lds4a(c.hist_() + 0 * L::ROWS * kRegW + r * kRegW, e[r]);
+        lds4a(c.hist_() + 1 * L::ROWS * kRegW + r * kRegW, hx[r]);
+        lds4a(c.hist_() + 2 * L::ROWS * kRegW + r * kRegW, hy[r]);
+      }
+    }
+    if (tid < 2) c.mask_()[tid] = 0u;
     // publish: row 0 for the warp above, all rows for the first trace sample
     st4a(c.xe_() + c.w * kRegW + c.l4, e[0]);
 #pragma unroll
     for (int r = 0; r < R; ++r) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
-    TICK(4);
-    __syncthreads();                   // mask zeroed
-    TICK(5);
+    // ---- next shot: fields into the (now free) landing slots, scalars into the other meta slot ------
+    cp_async_wait<0>();                // psi landed
+    if (s + 1 < s1) {
+      fwd_fetch<R, NW>(a, c, s + 1);
+      if (tid < 7) c.meta_()[(((s - s0) & 1) ^ 1) * 8 + tid] = fwd_meta_word(a, s + 1, tile, ntile, tid);
+    }
+    __syncthreads();                   // mask zeroed, next shot's scalars visible
     if (ent.x >= 0) atomicOr(c.mask_() + ((ent.x / kRegW) >> 5), 1u << ((ent.x / kRegW) & 31));
-    for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {
+    for (int k = rk0 + L::THREADS + tid; k < rk1; k += L::THREADS) {
       const int row = a.blk_ent[(long long)s * a.nrec + k].x / kRegW;
       atomicOr(c.mask_() + (row >> 5), 1u << (row & 31));
     }
+    ent_next = make_int2(-1, 0);
+    if (s + 1 < s1) {
+      const int* mn = c.meta_() + (((s - s0) & 1) ^ 1) * 8;
+      if (mn[0] + tid < mn[1]) ent_next = a.blk_ent[(long long)(s + 1) * a.nrec + mn[0] + tid];
+    }
     __syncthreads();
     const unsigned rflags = c.row_flags();
-    TICK(6);
 
     if (c.zp && c.xp) fwd_steps<R, NW, true, true>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
     else if (c.zp) fwd_steps<R, NW, true, false>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
     else if (c.xp) fwd_steps<R, NW, false, true>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
     else fwd_steps<R, NW, false, false>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
 
-    TICK(7);
     // ---- write back what this tile owns (out.ez was written by the last E phase) --------------------
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -272,11 +296,6 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
       st4a(a.out.hy + o, hy[r]);
     }
     if (c.zp || c.xp) c.store_psi(g, a.out, s);
-    TICK(8);
-#ifdef GPRFWI_TIMING
-    if (dbg) printf("TIMING shot %d: setup %lld | issue-loads %lld | loads-arrive %lld | bar1 %lld | mask+bar2 %lld | steps(%d) %lld | stores %lld\n",
-                    s, tk[1] - tk[0], tk[3] - tk[2], tk[4] - tk[3], tk[5] - tk[4], tk[6] - tk[5], a.nsub, tk[7] - tk[6], tk[8] - tk[7]);
-#endif
   }
 }
 #endif

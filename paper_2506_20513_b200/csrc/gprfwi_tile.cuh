@@ -21,7 +21,9 @@
 //   tabx [6][128]     CPML x tables of the region's columns: bhx chx khx bex cex kex
 //   tabz [6][NW*R]    CPML z tables of the region's rows:    bhz chz khz bez cez kez
 //   mask [2]          bit j: region row j holds a receiver of the current shot
-//   hist [NH][NW*R][128] adjoint only: ring of forward Ez planes fetched ahead with cp.async, thread-private
+//   meta [2][8]       per-shot scalars of the current and the next shot (receiver range, source, wavelet)
+//   hist [NH][NW*R][128] thread-private cp.async landing zone: adjoint = ring of forward Ez planes fetched two
+//                     steps ahead; forward = Ez, Hx, Hy of the NEXT shot fetched while this one is stepped
 //   psi  [4][NW*R][128]  CPML psi of the region, thread-private (only when npml > 0): hz ez hx ex
 #pragma once
 #include "gprfwi_common.cuh"
@@ -42,7 +44,8 @@ struct RegTile {
   static constexpr int TABX = ROWBUF + ROWS * kRegW;
   static constexpr int TABZ = TABX + 6 * kRegW;
   static constexpr int MASK = TABZ + 6 * ROWS;                 // 2 words: rows of the region that hold receivers
-  static constexpr int HIST = (MASK + 2 + 3) / 4 * 4;
+  static constexpr int META = MASK + 2;                        // 2 x 8 words: per-shot scalars, fetched one shot ahead
+  static constexpr int HIST = (META + 16 + 3) / 4 * 4;
   static constexpr int PSI = HIST + NH * ROWS * kRegW;
   GPR_HD static size_t smem_bytes(bool pml) { return sizeof(float) * (size_t)(PSI + (pml ? 4 * ROWS * kRegW : 0)); }
 };
@@ -116,6 +119,7 @@ struct TileCtx {
     const unsigned long long m = (unsigned long long)mask_()[0] | ((unsigned long long)mask_()[1] << 32);
     return (unsigned)(m >> lr0) & ((1u << R) - 1u);
   }
+  __device__ __forceinline__ int* meta_() const { return reinterpret_cast<int*>(sm + L::META); }
   __device__ __forceinline__ float* hist_() const { return sm + L::HIST + toff; }
   __device__ __forceinline__ float* phz_() const { return sm + L::PSI + 0 * L::ROWS * kRegW + toff; }
   __device__ __forceinline__ float* pez_() const { return sm + L::PSI + 1 * L::ROWS * kRegW + toff; }
@@ -180,25 +184,38 @@ struct TileCtx {
     if (w == 0) *reinterpret_cast<float4*>(xh_() + l4) = make_float4(0.f, 0.f, 0.f, 0.f);
   }
 
-  // psi strips of shot s -> the thread's shared-memory slots (all four arrays, zero where no psi lives)
-  __device__ __forceinline__ void load_psi(const Geo& g, const State& st, int s) const
+  // once per CTA: all psi slots of this thread to zero (slots that hold no CPML psi stay zero for good:
+  // the trivial coefficients keep them there)
+  __device__ __forceinline__ void zero_psi(const Geo& g) const
   {
-    if (g.P <= 0) return;
+    if (g.P <= 0 || !(zp || xp)) return;
+    const float z[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      const int gj = gj0 + r;
-      const bool in = colin && ((rin >> r) & 1u);
-      float a[4], b[4], c[4], d[4];
-      zero4(a); zero4(b); zero4(c); zero4(d);
-      if (in && ((zsH >> r) & 1u)) ldg4a(st.phxz + s * g.zstrip + (long long)strip_h(gj, g.nz, g.P) * g.pitch + gi, a);
-      if (in && ((zsE >> r) & 1u)) ldg4a(st.pezz + s * g.zstrip + (long long)strip_e(gj, g.nz, g.P) * g.pitch + gi, b);
-      if (in && xslot >= 0) {
-        const long long po = s * g.xstrip + (long long)gj * g.xw + xslot;
-        ldg4a(st.phyx + po, c);
-        ldg4a(st.pezx + po, d);
-      }
-      st4a(phz_() + r * kRegW, a); st4a(pez_() + r * kRegW, b); st4a(phx_() + r * kRegW, c); st4a(pex_() + r * kRegW, d);
+      st4a(phz_() + r * kRegW, z); st4a(pez_() + r * kRegW, z); st4a(phx_() + r * kRegW, z); st4a(pex_() + r * kRegW, z);
     }
+  }
+
+  // psi strips of shot s -> the thread's shared-memory slots, asynchronously (one commit group)
+  __device__ __forceinline__ void fetch_psi(const Geo& g, const State& st, int s) const
+  {
+    if (g.P > 0 && (zp || xp)) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        const int gj = gj0 + r;
+        const bool in = colin && ((rin >> r) & 1u);
+        if (in && ((zsH >> r) & 1u))
+          cp_async16(phz_() + r * kRegW, st.phxz + s * g.zstrip + (long long)strip_h(gj, g.nz, g.P) * g.pitch + gi);
+        if (in && ((zsE >> r) & 1u))
+          cp_async16(pez_() + r * kRegW, st.pezz + s * g.zstrip + (long long)strip_e(gj, g.nz, g.P) * g.pitch + gi);
+        if (in && xslot >= 0) {
+          const long long po = s * g.xstrip + (long long)gj * g.xw + xslot;
+          cp_async16(phx_() + r * kRegW, st.phyx + po);
+          cp_async16(pex_() + r * kRegW, st.pezx + po);
+        }
+      }
+    }
+    cp_async_commit();
   }
 
   // owned psi -> the output state
