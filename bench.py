@@ -134,6 +134,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--budget-gb", type=float, default=0.0, help="workspace budget (0 = 92%% of free HBM)")
     ap.add_argument("--nt", type=int, default=0, help="tuning only: cut the number of time steps")
+    ap.add_argument("--shots", type=int, default=0, help="tuning only: use the first N shots")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -142,8 +143,8 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
 
     wl = load_workload(args.config)
-    if args.nt > 0:
-        wl = wl.subset(list(range(wl.nshots)), nt=args.nt)
+    if args.nt > 0 or args.shots > 0:
+        wl = wl.subset(list(range(args.shots or wl.nshots)), nt=args.nt or wl.nt)
     if args.impl == "reference":
         if rank == 0:
             run_reference(args, wl)

@@ -50,10 +50,12 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
   const Geo& g = a.g;
   const unsigned full = 0xffffffffu;
   const float rdx = g.rdx, Db = g.Db, kap = g.kap;
+  const long long hoff = s * g.plane + (long long)c.gj0 * g.pitch + c.gi;     // this thread's row 0 in a plane of shot s
+  float* const trp = a.traces + (s * a.trace_stride + ent.y);                 // this thread's receiver, sample n
 #pragma unroll 1
   for (int t = 0; t < a.nsub; ++t) {
     // ---- stage 1: trace sample n + t from the published receiver rows ----------------------------
-    if (ent.x >= 0) a.traces[s * a.trace_stride + (long long)t * a.nrec + ent.y] = c.rowbuf_()[ent.x];
+    if (ent.x >= 0) trp[(long long)t * a.nrec] = c.rowbuf_()[ent.x];
     for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {      // more receivers than threads
       const int2 en2 = a.blk_ent[(long long)s * a.nrec + k];
       a.traces[s * a.trace_stride + (long long)t * a.nrec + en2.y] = c.rowbuf_()[en2.x];
@@ -151,15 +153,14 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
         for (int q = 0; q < 4; ++q)
           if (r == src_r && q == src_c) e[r][q] = FF(-cb[r][q], wn, e[r][q]);
     }
-    const bool last = t + 1 == a.nsub;
-    float* ez_out = last ? a.out.ez : a.ez_hist[t + 1];
+    float* ez_out = (t + 1 == a.nsub) ? a.out.ez : a.ez_hist[t + 1];
     if (ez_out) {
-      float* dst = ez_out + s * g.plane + (long long)c.gj0 * g.pitch + c.gi;
+      float* dst = ez_out + hoff;
 #pragma unroll
-      for (int r = 0; r < R; ++r)
-        if ((c.own >> r) & 1u) {
-          if (last) st4a(dst + r * g.pitch, e[r]); else stcs4a(dst + r * g.pitch, e[r]);   // history only: stream
-        }
+      for (int r = 0; r < R; ++r) {
+        if ((c.own >> r) & 1u) st4a(dst, e[r]);
+        dst += g.pitch;
+      }
     }
     if (rflags) {
 #pragma unroll
