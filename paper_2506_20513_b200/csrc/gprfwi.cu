@@ -145,20 +145,14 @@ static void base_layout(const gprfwi_params* p, Layout& L)
 }
 
 // A CTA owns one tile and sweeps a GROUP of shots one after the other (the adjoint keeps their
-// gradient sum in registers).  The number of groups is chosen to minimise
-//   waves(ngroups) * (group * t_shot + t_fixed),  waves = ceil(tiles * ngroups / slots),
-// i.e. CTA count a whole number of waves where possible, with t_fixed (per-CTA set-up, flush) taken
-// as `fixed_over_shot` shot-times.
-static void pick_groups(int tiles, int shots, int slots, double fixed_over_shot, int& group, int& ngroups)
+// gradient sum in registers; per-CTA set-up is paid once per group).  Small grids get small groups
+// so that a launch still has a few CTAs per SM slot; once the tiles alone fill the machine `fill`
+// times over, one CTA per tile sweeps all the shots.
+static void pick_groups(int tiles, int shots, int slots, int fill, int& group, int& ngroups)
 {
-  double best = 1e300;
-  group = shots; ngroups = 1;
-  for (int ng = 1; ng <= shots; ++ng) {
-    const int grp = (shots + ng - 1) / ng, n = (shots + grp - 1) / grp;
-    const double waves = std::ceil((double)tiles * n / slots);
-    const double cost = waves * (grp + fixed_over_shot);
-    if (cost < best - 1e-9) { best = cost; group = grp; ngroups = n; }
-  }
+  const int want = std::max(1, std::min(shots, (fill * slots + tiles - 1) / tiles));
+  group = (shots + want - 1) / want;
+  ngroups = (shots + group - 1) / group;
 }
 
 static int env_int(const char* name, int dflt)
@@ -170,8 +164,8 @@ static int env_int(const char* name, int dflt)
 static void set_groups(const gprfwi_params* p, Layout& L)
 {
   const int fslots = 148 * std::max(1, kFwdShapes[L.fv].minb), aslots = 148 * std::max(1, kAdjShapes[L.av].minb);
-  pick_groups(L.f.tiles(), p->nshots, fslots, 0.5, L.fgroup, L.fngroups);
-  pick_groups(L.a.tiles(), L.Sb, aslots, 1.0, L.group, L.ngroups);
+  pick_groups(L.f.tiles(), p->nshots, fslots, 2, L.fgroup, L.fngroups);
+  pick_groups(L.a.tiles(), L.Sb, aslots, 3, L.group, L.ngroups);
   if (int g = env_int("GPRFWI_FWD_GROUP", 0)) { L.fgroup = std::min(g, p->nshots); L.fngroups = (p->nshots + L.fgroup - 1) / L.fgroup; }
   if (int g = env_int("GPRFWI_ADJ_GROUP", 0)) { L.group = std::min(g, L.Sb); L.ngroups = (L.Sb + L.group - 1) / L.group; }
 }
@@ -314,6 +308,18 @@ struct gprfwi_handle {
   std::vector<int> h_src_off, h_blk_start, h_blk_ent, h_reg_start, h_reg_ent;
   bool forward_done = false;
   int64_t launches = 0;
+  // Shots are independent, so the launch sequence is issued as `nlanes` interleaved chains on
+  // internal streams forked from / joined to the caller's stream: the tail of one chain's launch
+  // overlaps the head of another's instead of leaving SMs idle between dependent launches.
+  std::vector<cudaStream_t> lanes;
+  std::vector<cudaEvent_t> lane_done;
+  cudaEvent_t fork = nullptr;
+  ~gprfwi_handle()
+  {
+    for (cudaStream_t q : lanes) cudaStreamDestroy(q);
+    for (cudaEvent_t e : lane_done) cudaEventDestroy(e);
+    if (fork) cudaEventDestroy(fork);
+  }
 };
 
 namespace gprfwi {
@@ -449,6 +455,42 @@ static int kernels_init(const gprfwi_params* p, const Layout& L)
   return GPRFWI_OK;
 }
 
+static int lanes_init(gprfwi_handle* h)
+{
+  if (!h->lanes.empty()) return GPRFWI_OK;
+  const int n = std::max(1, std::min(8, env_int("GPRFWI_LANES", 3)));
+  GPR_CUDA(cudaEventCreateWithFlags(&h->fork, cudaEventDisableTiming));
+  for (int k = 0; k < n; ++k) {
+    cudaStream_t q; cudaEvent_t e;
+    GPR_CUDA(cudaStreamCreateWithFlags(&q, cudaStreamNonBlocking));
+    GPR_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    h->lanes.push_back(q); h->lane_done.push_back(e);
+  }
+  return GPRFWI_OK;
+}
+// shots [0, ns) split into at most `lanes` contiguous chunks whose sizes are multiples of `quantum`
+static std::vector<int> lane_bounds(int ns, int lanes, int quantum)
+{
+  const int units = (ns + quantum - 1) / quantum, nl = std::max(1, std::min(lanes, units));
+  std::vector<int> b(nl + 1, 0);
+  for (int k = 1; k <= nl; ++k) b[k] = std::min(ns, (int)((long long)units * k / nl) * quantum);
+  return b;
+}
+static int lanes_fork(gprfwi_handle* h, cudaStream_t st, int nl)
+{
+  GPR_CUDA(cudaEventRecord(h->fork, st));
+  for (int k = 0; k < nl; ++k) GPR_CUDA(cudaStreamWaitEvent(h->lanes[k], h->fork, 0));
+  return GPRFWI_OK;
+}
+static int lanes_join(gprfwi_handle* h, cudaStream_t st, int nl)
+{
+  for (int k = 0; k < nl; ++k) {
+    GPR_CUDA(cudaEventRecord(h->lane_done[k], h->lanes[k]));
+    GPR_CUDA(cudaStreamWaitEvent(st, h->lane_done[k], 0));
+  }
+  return GPRFWI_OK;
+}
+
 // Forward block: steps n .. n+nsub-1 for `ns` shots from global shot `shot0`.  ez_of(m) gives the
 // plane that must receive Ez^m (local shot 0) or NULL; in.ez / out.ez are already set by the caller.
 template <class EzOf>
@@ -489,7 +531,7 @@ static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, 
 
 // Adjoint block: reverse steps n_hi-1 .. n_hi-nsub for `ns` shots from global shot `shot0`.
 template <class EzOf>
-static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsub, int shot0, int ns,
+static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsub, int shot0, int ns, int grp0,
                             const State& in, const State& out, const float* residual, EzOf ez_of)
 {
   const gprfwi_params& p = h->p;
@@ -503,8 +545,8 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   a.ca = h->c.ca;
   a.cb = h->c.cb;
   for (int t = 0; t <= kMaxT; ++t) a.ez_planes[t] = t <= nsub ? ez_of(n_hi - t) : nullptr;
-  a.gca = h->c.gca;
-  a.gcb = h->c.gcb;
+  a.gca = h->c.gca + (size_t)grp0 * L.plane;        // this launch's groups start at plane pair grp0
+  a.gcb = h->c.gcb + (size_t)grp0 * L.plane;
   a.trace_stride = tstride;
   a.residual = residual ? residual + (size_t)shot0 * tstride + (long long)n_hi * p.nrec : nullptr;
   a.reg_start = h->c.reg_start;
@@ -627,28 +669,38 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
   if (rc != GPRFWI_OK) return rc;
   if (L.full_history) GPR_CUDA(cudaMemsetAsync(h->c.hist, 0, S * L.plane * f, st));
   else GPR_CUDA(cudaMemsetAsync(h->c.ckpt, 0, S * L.full * f, st));       // checkpoint 0 = zero state
-  // blocks of up to T steps that never cross a checkpoint boundary
+  // blocks of up to T steps that never cross a checkpoint boundary, issued lane by lane
+  rc = lanes_init(h);
+  if (rc != GPRFWI_OK) return rc;
+  const std::vector<int> lb = lane_bounds((int)S, (int)h->lanes.size(), L.fgroup);
+  const int nl = (int)lb.size() - 1;
+  rc = lanes_fork(h, st, nl);
+  if (rc != GPRFWI_OK) return rc;
   int idx = 0;
   for (int n = 0; n < p->nt; ++idx) {
     const int bound = L.full_history ? p->nt : std::min((n / L.K + 1) * L.K, p->nt);
     const int nsub = std::min(L.T, bound - n), m = n + nsub;
-    State in, out;
-    if (L.full_history) {
-      in = state_at(L, slot[idx & 1], S, 0);
-      out = state_at(L, slot[(idx + 1) & 1], S, 0);
-      in.ez = h->c.hist + (size_t)n * S * L.plane;
-      out.ez = h->c.hist + (size_t)m * S * L.plane;
-      launch_fwd_block(h, st, n, nsub, 0, (int)S, in, out, traces,
-                       [&](int q) { return h->c.hist + (size_t)q * S * L.plane; });
-    } else {
-      float* src = (n % L.K == 0) ? h->c.ckpt + (size_t)(n / L.K) * S * L.full : slot[idx & 1];
-      float* dst = (m == p->nt) ? h->c.ckpt + (size_t)L.ncheck * S * L.full
-                 : (m % L.K == 0) ? h->c.ckpt + (size_t)(m / L.K) * S * L.full : slot[(idx + 1) & 1];
-      launch_fwd_block(h, st, n, nsub, 0, (int)S, state_at(L, src, S, 0), state_at(L, dst, S, 0), traces,
-                       [](int) -> float* { return nullptr; });
+    for (int k = 0; k < nl && rc == GPRFWI_OK; ++k) {
+      const int sh0 = lb[k], ns = lb[k + 1] - lb[k];
+      if (L.full_history) {
+        State in = state_at(L, slot[idx & 1], S, sh0), out = state_at(L, slot[(idx + 1) & 1], S, sh0);
+        in.ez = h->c.hist + ((size_t)n * S + sh0) * L.plane;
+        out.ez = h->c.hist + ((size_t)m * S + sh0) * L.plane;
+        rc = launch_fwd_block(h, h->lanes[k], n, nsub, sh0, ns, in, out, traces,
+                              [&](int q) { return h->c.hist + ((size_t)q * S + sh0) * L.plane; });
+      } else {
+        float* src = (n % L.K == 0) ? h->c.ckpt + (size_t)(n / L.K) * S * L.full : slot[idx & 1];
+        float* dst = (m == p->nt) ? h->c.ckpt + (size_t)L.ncheck * S * L.full
+                   : (m % L.K == 0) ? h->c.ckpt + (size_t)(m / L.K) * S * L.full : slot[(idx + 1) & 1];
+        rc = launch_fwd_block(h, h->lanes[k], n, nsub, sh0, ns, state_at(L, src, S, sh0), state_at(L, dst, S, sh0),
+                              traces, [](int) -> float* { return nullptr; });
+      }
     }
+    if (rc != GPRFWI_OK) return rc;
     n = m;
   }
+  rc = lanes_join(h, st, nl);
+  if (rc != GPRFWI_OK) return rc;
   GPR_CUDA(cudaGetLastError());
   h->forward_done = true;
   return GPRFWI_OK;
@@ -668,47 +720,69 @@ int gprfwi_adjoint(gprfwi_handle* h, const float* residual, float* grad_eps_r, f
   float* lam[2] = {h->c.lam, h->c.lam + (size_t)L.Sb * L.full};
   float* rs[2] = {h->c.fscratch, h->c.fscratch + S * L.full};     // recompute ping-pong
 
+  int rc = lanes_init(h);
+  if (rc != GPRFWI_OK) return rc;
   for (int shot0 = 0; shot0 < (int)S; shot0 += L.Sb) {
     const int ns = std::min(L.Sb, (int)S - shot0);
     // lambda = 0 at the end time, Eq. (10)
     GPR_CUDA(cudaMemsetAsync(h->c.lam, 0, 2 * (size_t)L.Sb * L.full * f, st));
+    // the shots of this pass go down `nl` interleaved lanes (chunks are whole CTA groups)
+    const std::vector<int> lb = lane_bounds(ns, (int)h->lanes.size(), L.group);
+    const int nl = (int)lb.size() - 1;
+    rc = lanes_fork(h, st, nl);
+    if (rc != GPRFWI_OK) return rc;
     int flip = 0;
     const int nseg = L.full_history ? 1 : L.ncheck;
     for (int c = nseg - 1; c >= 0; --c) {
       const int n0 = L.full_history ? 0 : c * L.K;
       const int n1 = L.full_history ? p->nt : std::min(n0 + L.K, p->nt);
-      // forward Ez plane of step m for local shot 0 of this pass
-      auto ez_plane = [&](int m) -> float* {
-        if (L.full_history) return h->c.hist + ((size_t)m * S + shot0) * L.plane;
-        if (m == n0) return h->c.ckpt + (size_t)c * S * L.full + (size_t)shot0 * L.plane;
-        if (m == n1) {
-          const size_t slot = (m == p->nt) ? (size_t)L.ncheck : (size_t)(m / L.K);
-          return h->c.ckpt + slot * S * L.full + (size_t)shot0 * L.plane;
-        }
-        return h->c.seg + (size_t)(m - n0 - 1) * L.Sb * L.plane;
+      // forward Ez plane of step m for the first shot (pass-local l0) of a lane
+      auto ez_plane_of = [&, c, n0, n1](int l0) {
+        return [=](int m) -> float* {
+          const int g0 = shot0 + l0;
+          if (L.full_history) return h->c.hist + ((size_t)m * S + g0) * L.plane;
+          if (m == n0) return h->c.ckpt + (size_t)c * S * L.full + (size_t)g0 * L.plane;
+          if (m == n1) {
+            const size_t slot = (m == p->nt) ? (size_t)L.ncheck : (size_t)(m / L.K);
+            return h->c.ckpt + slot * S * L.full + (size_t)g0 * L.plane;
+          }
+          return h->c.seg + ((size_t)(m - n0 - 1) * L.Sb + l0) * L.plane;
+        };
       };
       if (!L.full_history) {
         // recompute Ez^{n0+1 .. n1-1} from checkpoint c with the same kernel (Ez^{n1} is a checkpoint)
         int idx = 0;
         for (int n = n0; n < n1 - 1; ++idx) {
           const int nsub = std::min(L.T, n1 - 1 - n);
-          State in = (n == n0) ? state_at(L, h->c.ckpt + (size_t)c * S * L.full, S, shot0)
-                               : state_at(L, rs[idx & 1], S, 0);
-          State out = state_at(L, rs[(idx + 1) & 1], S, 0);
-          in.ez = ez_plane(n);
-          out.ez = ez_plane(n + nsub);
-          launch_fwd_block(h, st, n, nsub, shot0, ns, in, out, nullptr, ez_plane);
+          for (int k = 0; k < nl; ++k) {
+            const int l0 = lb[k], nsl = lb[k + 1] - lb[k], g0 = shot0 + l0;
+            auto ez_plane = ez_plane_of(l0);
+            State in = (n == n0) ? state_at(L, h->c.ckpt + (size_t)c * S * L.full, S, g0)
+                                 : state_at(L, rs[idx & 1], S, l0);
+            State out = state_at(L, rs[(idx + 1) & 1], S, l0);
+            in.ez = ez_plane(n);
+            out.ez = ez_plane(n + nsub);
+            rc = launch_fwd_block(h, h->lanes[k], n, nsub, g0, nsl, in, out, nullptr, ez_plane);
+            if (rc != GPRFWI_OK) return rc;
+          }
           n += nsub;
         }
       }
       for (int n_hi = n1; n_hi > n0;) {
         const int nsub = std::min(L.T, n_hi - n0);
-        launch_adj_block(h, st, n_hi, nsub, shot0, ns, state_at(L, lam[flip], L.Sb, 0),
-                         state_at(L, lam[flip ^ 1], L.Sb, 0), residual, ez_plane);
+        for (int k = 0; k < nl; ++k) {
+          const int l0 = lb[k], nsl = lb[k + 1] - lb[k];
+          rc = launch_adj_block(h, h->lanes[k], n_hi, nsub, shot0 + l0, nsl, l0 / L.group,
+                                state_at(L, lam[flip], L.Sb, l0), state_at(L, lam[flip ^ 1], L.Sb, l0), residual,
+                                ez_plane_of(l0));
+          if (rc != GPRFWI_OK) return rc;
+        }
         flip ^= 1;
         n_hi -= nsub;
       }
     }
+    rc = lanes_join(h, st, nl);
+    if (rc != GPRFWI_OK) return rc;
   }
   {
     dim3 grid((p->nx + 127) / 128, p->nz), block(128);
