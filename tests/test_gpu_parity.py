@@ -233,3 +233,27 @@ def test_config3_checkpointed_subset_against_oracle():
     tr, ge, gs, plan = run_gpu(wl, res, checkpoint_stride=40)
     assert plan["full_history"] == 0
     assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
+
+
+def test_config4_grid_subset_against_oracle():
+    """Config 4 grid (1060x2060, 30-cell CPML, dx 5 mm, 1.2 GHz), nt cut to 300 and the first / last
+    shot for the oracle's sake, through checkpoint-and-recompute with a stride that is not a multiple
+    of the time block (ragged launches at segment ends)."""
+    wl = gi.config4(nt=300).subset([0, 99])
+    tr_o, res, ge_o, gs_o = oracle_all(wl)
+    tr, ge, gs, plan = run_gpu(wl, res, checkpoint_stride=37)
+    assert plan["full_history"] == 0 and plan["checkpoint_stride"] == 37
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
+
+
+def test_config5_per_shot_receivers_batched():
+    """Config 5 (512^2, uniform random eps_r / sigma per cell, every shot its own 64 receivers): a
+    batch of 8 in one call, shots 0 and 7 against the oracle, and batched == per-shot bit for bit."""
+    wl = gi.config5(n=512, batch=8, nt=250)
+    sub = wl.subset([0, 7])
+    tr_o, res_sub, ge_o, gs_o = oracle_all(sub)
+    t2, ge, gs, _ = run_gpu(sub, res_sub)
+    assert_parity(sub, (t2, ge, gs), (tr_o, ge_o, gs_o))
+    tr, _, _, plan = run_gpu(wl)
+    assert np.array_equal(tr[[0, 7]], t2)
+    assert plan["shots_per_pass"] == 8
