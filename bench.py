@@ -35,7 +35,9 @@ UNIT = "Gcell-updates/s"
 BYTES_FWD, BYTES_ADJ, BYTES_RECOMPUTE = 28.0, 32.0, 28.0
 
 
-def load_workload(cfg: int):
+def load_workload(cfg: int, n: int = 512, batch: int = 1):
+    if cfg == 5:
+        return gi.config5(n=n, batch=batch)
     return {1: gi.config1, 2: gi.config2, 3: gi.config3, 4: gi.config4}[cfg]()
 
 
@@ -133,6 +135,8 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--budget-gb", type=float, default=0.0, help="workspace budget (0 = 92%% of free HBM)")
+    ap.add_argument("--n", type=int, default=512, help="config 5: grid is n x n")
+    ap.add_argument("--batch", type=int, default=1, help="config 5: shots in the batch")
     ap.add_argument("--nt", type=int, default=0, help="tuning only: cut the number of time steps")
     ap.add_argument("--shots", type=int, default=0, help="tuning only: use the first N shots")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -142,7 +146,7 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
 
-    wl = load_workload(args.config)
+    wl = load_workload(args.config, args.n, args.batch)
     if args.nt > 0 or args.shots > 0:
         wl = wl.subset(list(range(args.shots or wl.nshots)), nt=args.nt or wl.nt)
     if args.impl == "reference":
@@ -152,8 +156,9 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2506_20513_b200 import (Simulation, build, gprfwi_gradient_host, gprfwi_residual,
-                                       gprfwi_workspace_bytes, gprfwi_workspace_bytes_host, make_params)
+    from paper_2506_20513_b200 import (Simulation, build, gprfwi_gradient_host, gprfwi_residual, gprfwi_update,
+                                       gprfwi_update_workspace_bytes, gprfwi_workspace_bytes,
+                                       gprfwi_workspace_bytes_host, make_params, make_update_params)
     build.build()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
@@ -178,6 +183,12 @@ def main():
     res = torch.empty_like(d_obs)
     misfit = torch.zeros(1, dtype=torch.float64, device=dev)
     stream = torch.cuda.current_stream()
+    # iteration epilogue (a7): TV term + mask + Adam + clamps on copies of the models, so that every
+    # timed step runs the same forward problem (the step size is tiny and the copies are reset)
+    eps_it, sig_it = eps.clone(), sig.clone()
+    adam = [torch.zeros_like(eps) for _ in range(4)]
+    ws_up = torch.empty(gprfwi_update_workspace_bytes(wl.nz, wl.nx), dtype=torch.uint8, device=dev)
+    upd = make_update_params(step=1, lr_eps_r=1e-3, lr_sigma=1e-6, tv_iters=10, mask_rows=wl.npml + 7)
 
     def step(timers=None):
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)] if timers is not None else None
@@ -190,8 +201,10 @@ def main():
         ge, gs = sim.adjoint(res)
         if world > 1:                      # shots are sharded over ranks: sum the gradients
             dist.all_reduce(ge); dist.all_reduce(gs)
+        if ev: ev[3].record(stream)
+        gprfwi_update(wl.nz, wl.nx, wl.nx, upd, eps_it, sig_it, ge, gs, adam[0], adam[1], adam[2], adam[3], ws_up)
         if ev:
-            ev[3].record(stream)
+            ev.append(torch.cuda.Event(enable_timing=True)); ev[4].record(stream)
             timers.append(ev)
 
     def barrier():
@@ -217,6 +230,7 @@ def main():
         ms = float(t.item())
     fwd_ms = statistics.mean(e[0].elapsed_time(e[1]) for e in timers)
     adj_ms = statistics.mean(e[2].elapsed_time(e[3]) for e in timers)
+    upd_ms = statistics.mean(e[3].elapsed_time(e[4]) for e in timers)
     launches = sim.launch_count()          # kernels of the last forward + adjoint
     plan = sim.plan
     cells = wl.nz * wl.nx * wl.nshots
@@ -296,7 +310,8 @@ def main():
                 "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": wl.name, "grid": [wl.nz, wl.nx], "nt": wl.nt, "shots_per_gpu": wl.nshots,
-                           "receivers": wl.nrec, "plan": plan, "fwd_ms": fwd_ms, "adj_ms": adj_ms,
+                           "receivers": wl.nrec, "plan": plan, "fwd_ms": fwd_ms, "adj_ms": adj_ms, "epilogue_ms": upd_ms,
+                           "iteration": "forward, residual+misfit, adjoint, TV term + mask + Adam step + clamps",
                            "s_per_fwi_iteration": ms / args.steps * 1e-3,
                            "l2": "inputs larger than L2 (Ez history / checkpoints stream through HBM)"},
                 "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int((launches + 1) * args.steps),

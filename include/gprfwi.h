@@ -138,6 +138,34 @@ size_t gprfwi_workspace_bytes_host(const gprfwi_params* p, size_t budget_bytes);
 int gprfwi_residual(const float* d_syn, const float* d_obs, float* residual, size_t n,
                     double* misfit, void* cuda_stream);
 
+/* Iteration epilogue: what the paper's script does between loss.backward() and
+ * the next epoch plus the TV term of Algorithm 3. */
+typedef struct {
+  int32_t step;                 /* Adam step counter t >= 1 (bias correction 1 - beta^t)                 */
+  float   lr_eps_r, lr_sigma;   /* one learning rate per parameter (Eqs. (14)-(15))   */
+  float   beta1, beta2, adam_eps;
+  int32_t tv_iters;             /* split-variable TV iterations of Algorithm 3; 0 = no TV term          */
+  float   tv_rho, tv_lambda, tv_alpha;   /* tv_grad = alpha (X - s U), shrink threshold lambda / rho    */
+  int32_t mask_rows;            /* gradient rows j < mask_rows are zeroed (near the sources,
+                                   PAPER.md:229-233)                                                     */
+  float   eps_r_min, sigma_min; /* clamps after the step                             */
+} gprfwi_update_params;
+
+/* Device scratch the epilogue needs for an nz x pitch plane: 7 planes + 256 B. */
+size_t gprfwi_update_workspace_bytes(int32_t nz, int32_t pitch);
+
+/* One optimiser step on the device, in place:
+ *   for X in (eps_r, sigma):  g = grad_X (+ TV term of X, Algorithm 3; reading R20);
+ *   g[j < mask_rows] = 0;  m = b1 m + (1-b1) g;  v = b2 v + (1-b2) g^2;
+ *   X -= lr_X (m / (1-b1^t)) / (sqrt(v / (1-b2^t)) + adam_eps);  X = max(X, X_min).
+ * eps_r, sigma, m_*, v_*  device [nz][pitch], updated in place (m, v: zero before the first step);
+ * grad_eps_r, grad_sigma  device [nz][pitch]; the TV term is added to them in place.
+ * Errors: EINVAL (null pointer, nz/nx < 2, pitch < nx, step < 1, tv_rho <= 0 with tv_iters > 0), ECUDA. */
+int gprfwi_update(int32_t nz, int32_t nx, int32_t pitch, const gprfwi_update_params* u,
+                  float* eps_r, float* sigma, float* grad_eps_r, float* grad_sigma,
+                  float* m_eps_r, float* v_eps_r, float* m_sigma, float* v_sigma,
+                  void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Number of kernel launches enqueued by the last forward / adjoint on this handle. */
 int64_t gprfwi_launch_count(const gprfwi_handle* h);
 

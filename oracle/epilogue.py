@@ -1,0 +1,70 @@
+"""TEST INFRASTRUCTURE, NOT PRODUCT CODE -- float64 NumPy statement of the iteration epilogue
+(SURVEY 8(a) row a7): TV term of Algorithm 3 (Eq. (17)), gradient mask near the
+sources, Adam step with one learning rate per parameter (Eqs. (14)-(15),
+PAPER.md:105-112) and the clamps of PAPER.md:258-260.  Shares nothing with csrc/.
+
+Readings (R18-R20).  The paper lists Algorithm 3's steps without constants or a
+definition of `*_tv_grad`; the reading below is the one both sides implement.
+
+Pins (tests/test_oracle_pins.py): Adam's first step equals -lr g/(|g| + eps) (closed form of
+Eqs. (14)-(15) at t = 1), masked rows do not move, clamps hold; shrink(v, t) = v max(1 - t/|v|, 0)
+(Eq. (17)); a constant X gives tv_grad = 0; the U update solves (I + rho D^T D) U = U0 + rho D^T (Z - B)
+in the limit of many sweeps (checked with one dense solve on a tiny grid).  Beyond those invariants
+the TV term is PARITY UNPINNED: the paper gives no value to compare with.
+"""
+import numpy as np
+
+
+def shrink(vx, vz, t):
+    """Isotropic soft threshold, Eq. (17): v * max(1 - t/|v|, 0)."""
+    nrm = np.sqrt(vx * vx + vz * vz)
+    f = np.where(nrm > t, 1.0 - t / np.where(nrm > t, nrm, 1.0), 0.0)
+    return f * vx, f * vz
+
+
+def tv_gradient(x, iters=10, rho=1.0, lam=0.01, alpha=1.0):
+    """Algorithm 3 (reading R20): returns alpha * (X - s U) after `iters` split-variable iterations."""
+    x = np.asarray(x, dtype=np.float64)
+    s = np.max(np.abs(x))
+    u0 = x / s if s > 0 else np.zeros_like(x)
+    u = u0.copy()
+    zx = np.zeros_like(u); zz = np.zeros_like(u); bx = np.zeros_like(u); bz = np.zeros_like(u)
+    for _ in range(iters):
+        wx, wz = zx - bx, zz - bz
+        div = (np.roll(wx, 1, axis=1) - wx) + (np.roll(wz, 1, axis=0) - wz)          # D^T (Z - B)
+        nb = np.roll(u, 1, axis=1) + np.roll(u, -1, axis=1) + np.roll(u, 1, axis=0) + np.roll(u, -1, axis=0)
+        u = (u0 + rho * div + rho * nb) / (1.0 + 4.0 * rho)                           # one Jacobi sweep
+        gx = np.roll(u, -1, axis=1) - u                                               # D U, circular forward
+        gz = np.roll(u, -1, axis=0) - u
+        zx, zz = shrink(gx + bx, gz + bz, lam / rho)
+        bx = bx + gx - zx
+        bz = bz + gz - zz
+    return alpha * (x - s * u)
+
+
+def adam_step(x, g, m, v, step, lr, beta1=0.9, beta2=0.999, eps=1e-8, mask_rows=0, xmin=-np.inf):
+    """Eqs. (14)-(15) with the epsilon outside the root (reading R19); returns (x, m, v)."""
+    g = np.array(g, dtype=np.float64)
+    g[:mask_rows] = 0.0                                                               # reading R18
+    m = beta1 * m + (1.0 - beta1) * g
+    v = beta2 * v + (1.0 - beta2) * g * g
+    mh = m / (1.0 - beta1 ** step)
+    vh = v / (1.0 - beta2 ** step)
+    x = np.maximum(x - lr * mh / (np.sqrt(vh) + eps), xmin)
+    return x, m, v
+
+
+def update(eps_r, sigma, g_eps, g_sig, state, step, lr_eps, lr_sig, beta1=0.9, beta2=0.999, adam_eps=1e-8,
+           tv_iters=10, tv_rho=1.0, tv_lambda=0.01, tv_alpha=1.0, mask_rows=0, eps_min=1.0, sig_min=0.0):
+    """One epilogue step; `state` = dict of m_eps, v_eps, m_sig, v_sig (float64 arrays)."""
+    out = {}
+    for name, x, g, lr, xmin in (("eps", eps_r, g_eps, lr_eps, eps_min), ("sig", sigma, g_sig, lr_sig, sig_min)):
+        x = np.asarray(x, dtype=np.float64)
+        g = np.asarray(g, dtype=np.float64).copy()
+        if tv_iters > 0:
+            g += tv_gradient(x, tv_iters, tv_rho, tv_lambda, tv_alpha)
+        xn, m, v = adam_step(x, g, state["m_" + name], state["v_" + name], step, lr, beta1, beta2, adam_eps,
+                             mask_rows, xmin)
+        out[name] = (xn, g)
+        state["m_" + name], state["v_" + name] = m, v
+    return out["eps"][0], out["sig"][0], out["eps"][1], out["sig"][1]

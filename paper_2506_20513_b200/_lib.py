@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "OK", -1: "EINVAL", -2: "ECFL", -3: "EGEOM", -4: "ENOMEM", -5
 EXPORTS = (
     "gprfwi_workspace_bytes", "gprfwi_forward", "gprfwi_adjoint", "gprfwi_gradient_host",
     "gprfwi_workspace_bytes_host", "gprfwi_residual", "gprfwi_launch_count", "gprfwi_get_plan",
-    "gprfwi_release", "gprfwi_strerror", "gprfwi_version",
+    "gprfwi_release", "gprfwi_strerror", "gprfwi_version", "gprfwi_update", "gprfwi_update_workspace_bytes",
 )
 
 
@@ -44,6 +44,17 @@ class Plan(ctypes.Structure):
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+class UpdateParams(ctypes.Structure):
+    """gprfwi_update_params"""
+    _fields_ = [
+        ("step", ctypes.c_int32), ("lr_eps_r", ctypes.c_float), ("lr_sigma", ctypes.c_float),
+        ("beta1", ctypes.c_float), ("beta2", ctypes.c_float), ("adam_eps", ctypes.c_float),
+        ("tv_iters", ctypes.c_int32), ("tv_rho", ctypes.c_float), ("tv_lambda", ctypes.c_float),
+        ("tv_alpha", ctypes.c_float), ("mask_rows", ctypes.c_int32),
+        ("eps_r_min", ctypes.c_float), ("sigma_min", ctypes.c_float),
+    ]
 
 
 class GprfwiError(RuntimeError):
@@ -79,6 +90,11 @@ def _declare(lib):
     lib.gprfwi_release.argtypes = [vp]
     lib.gprfwi_strerror.restype = ctypes.c_char_p
     lib.gprfwi_strerror.argtypes = [ctypes.c_int]
+    lib.gprfwi_update_workspace_bytes.restype = sz
+    lib.gprfwi_update_workspace_bytes.argtypes = [ctypes.c_int32, ctypes.c_int32]
+    lib.gprfwi_update.restype = ctypes.c_int
+    lib.gprfwi_update.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(UpdateParams),
+                                  fp, fp, fp, fp, fp, fp, fp, fp, vp, sz, vp]
     lib.gprfwi_version.restype = ctypes.c_int
     return lib
 

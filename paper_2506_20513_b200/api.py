@@ -11,7 +11,7 @@ import numpy as np
 import torch
 
 from . import _lib
-from ._lib import Params, Plan, check
+from ._lib import Params, Plan, UpdateParams, check
 
 
 def make_params(*, nz, nx, dx, dt, nt, npml, pml_order, pml_sigma_max, pml_kappa_max, pml_alpha_max,
@@ -122,6 +122,31 @@ def gprfwi_gradient_host(p: Params, eps_r, sigma, wavelet, src_zx, rec_zx, d_obs
         traces.ctypes.data if traces is not None else None, ge.ctypes.data, gs.ctypes.data,
         ctypes.byref(mf), _stream_ptr(stream)))
     return ge, gs, mf.value
+
+
+def make_update_params(*, step, lr_eps_r, lr_sigma, beta1=0.9, beta2=0.999, adam_eps=1e-8, tv_iters=10,
+                       tv_rho=1.0, tv_lambda=0.01, tv_alpha=1.0, mask_rows=0, eps_r_min=1.0,
+                       sigma_min=0.0) -> UpdateParams:
+    return UpdateParams(int(step), float(lr_eps_r), float(lr_sigma), float(beta1), float(beta2), float(adam_eps),
+                        int(tv_iters), float(tv_rho), float(tv_lambda), float(tv_alpha), int(mask_rows),
+                        float(eps_r_min), float(sigma_min))
+
+
+def gprfwi_update_workspace_bytes(nz: int, pitch: int) -> int:
+    return int(_lib.load().gprfwi_update_workspace_bytes(int(nz), int(pitch)))
+
+
+def gprfwi_update(nz, nx, pitch, u: UpdateParams, eps_r, sigma, grad_eps_r, grad_sigma, m_eps_r, v_eps_r,
+                  m_sigma, v_sigma, workspace, stream=None):
+    """Enqueue one optimiser step (TV term, mask, Adam, clamps) on `stream`; all planes updated in place."""
+    n = nz * pitch
+    ptrs = [_dev(t, nm, n) for t, nm in ((eps_r, "eps_r"), (sigma, "sigma"), (grad_eps_r, "grad_eps_r"),
+                                          (grad_sigma, "grad_sigma"), (m_eps_r, "m_eps_r"), (v_eps_r, "v_eps_r"),
+                                          (m_sigma, "m_sigma"), (v_sigma, "v_sigma"))]
+    if not (isinstance(workspace, torch.Tensor) and workspace.is_cuda and workspace.dtype == torch.uint8):
+        raise TypeError("workspace must be a CUDA uint8 tensor")
+    check(_lib.load().gprfwi_update(int(nz), int(nx), int(pitch), ctypes.byref(u), *ptrs, workspace.data_ptr(),
+                                    workspace.numel(), _stream_ptr(stream)))
 
 
 class Simulation:

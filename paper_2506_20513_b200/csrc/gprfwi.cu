@@ -16,6 +16,7 @@
 #include "gprfwi_fwd_kernel.cuh"
 #include "gprfwi_misc.cuh"
 #include "gprfwi_tile.cuh"
+#include "gprfwi_update.cuh"
 
 namespace gprfwi {
 
@@ -892,6 +893,60 @@ int gprfwi_gradient_host(const gprfwi_params* p, const float* eps_r, const float
   GPR_CUDA(cudaMemcpyAsync(&mf, hc.misfit, sizeof(double), cudaMemcpyDeviceToHost, st));
   GPR_CUDA(cudaStreamSynchronize(st));
   if (misfit) *misfit = mf;
+  return GPRFWI_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// iteration epilogue: TV term, gradient mask, Adam step, clamps (gprfwi_update.cuh)
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+size_t gprfwi_update_workspace_bytes(int32_t nz, int32_t pitch)
+{
+  if (nz < 2 || pitch < 2) return 0;
+  return (size_t)7 * align_up((size_t)nz * pitch * sizeof(float), 256) + 256;
+}
+
+int gprfwi_update(int32_t nz, int32_t nx, int32_t pitch, const gprfwi_update_params* u, float* eps_r, float* sigma,
+                  float* grad_eps_r, float* grad_sigma, float* m_eps_r, float* v_eps_r, float* m_sigma,
+                  float* v_sigma, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+  if (!u || !eps_r || !sigma || !grad_eps_r || !grad_sigma || !m_eps_r || !v_eps_r || !m_sigma || !v_sigma)
+    return GPRFWI_EINVAL;
+  if (nz < 2 || nx < 2 || pitch < nx || u->step < 1 || u->tv_iters < 0) return GPRFWI_EINVAL;
+  if (u->tv_iters > 0 && (!(u->tv_rho > 0.f) || !workspace)) return GPRFWI_EINVAL;
+  if (u->tv_iters > 0 && workspace_bytes < gprfwi_update_workspace_bytes(nz, pitch)) return GPRFWI_ENOMEM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t pb = align_up((size_t)nz * pitch * sizeof(float), 256);
+  char* w = (char*)workspace;
+  dim3 grid((nx + 127) / 128, nz), block(128);
+  const float c1 = (float)(1.0 / (1.0 - std::pow((double)u->beta1, (double)u->step)));
+  const float c2 = (float)(1.0 / (1.0 - std::pow((double)u->beta2, (double)u->step)));
+  struct Par { float *x, *g, *m, *v; float lr, xmin; };
+  const Par par[2] = {{eps_r, grad_eps_r, m_eps_r, v_eps_r, u->lr_eps_r, u->eps_r_min},
+                      {sigma, grad_sigma, m_sigma, v_sigma, u->lr_sigma, u->sigma_min}};
+  for (const Par& q : par) {
+    if (u->tv_iters > 0) {
+      float* u0 = (float*)(w + 0 * pb); float* ua = (float*)(w + 1 * pb); float* ub = (float*)(w + 2 * pb);
+      float* zx = (float*)(w + 3 * pb); float* zz = (float*)(w + 4 * pb);
+      float* bx = (float*)(w + 5 * pb); float* bz = (float*)(w + 6 * pb);
+      unsigned* smax = (unsigned*)(w + 7 * pb);
+      GPR_CUDA(cudaMemsetAsync(smax, 0, sizeof(unsigned), st));
+      GPR_LAUNCH(absmax_kernel, dim3(std::min(nz, 1024)), dim3(256), st, q.x, nz, nx, pitch, smax);
+      GPR_LAUNCH(tv_init_kernel, grid, block, st, q.x, nz, nx, pitch, smax, u0, ua, zx, zz, bx, bz);
+      for (int it = 0; it < u->tv_iters; ++it) {
+        GPR_LAUNCH(tv_jacobi_kernel, grid, block, st, nz, nx, pitch, u->tv_rho, u0, ua, zx, zz, bx, bz, ub);
+        GPR_LAUNCH(tv_shrink_kernel, grid, block, st, nz, nx, pitch, u->tv_lambda / u->tv_rho, ub, zx, zz, bx, bz);
+        std::swap(ua, ub);
+      }
+      GPR_LAUNCH(tv_add_kernel, grid, block, st, q.x, nz, nx, pitch, smax, u->tv_alpha, ua, q.g);
+    }
+    GPR_LAUNCH(adam_kernel, grid, block, st, nz, nx, pitch, u->mask_rows, q.lr, u->beta1, u->beta2, u->adam_eps,
+               c1, c2, q.xmin, q.g, q.m, q.v, q.x);
+  }
+  GPR_CUDA(cudaGetLastError());
   return GPRFWI_OK;
 }
 

@@ -257,3 +257,37 @@ def test_config5_per_shot_receivers_batched():
     tr, _, _, plan = run_gpu(wl)
     assert np.array_equal(tr[[0, 7]], t2)
     assert plan["shots_per_pass"] == 8
+
+
+def test_epilogue_update_matches_numpy_oracle():
+    """a7: TV term (Algorithm 3) + mask + Adam + clamps, three consecutive steps, vs oracle/epilogue.py
+    (float64).  Tolerances: the TV term is a small difference X - sU of O(s) numbers, so it is compared
+    against max|X| (1e-5); the updated models to 1e-5 relative."""
+    from oracle import epilogue as ep
+    from paper_2506_20513_b200 import gprfwi_update, gprfwi_update_workspace_bytes, make_update_params
+    wl = gi.small_random(nz=70, nx=150, nt=10, npml=10, nshots=1, nrec=2, seed=21)
+    nz, nx, pitch = wl.nz, wl.nx, wl.nx + 3
+    rng = np.random.default_rng(7)
+    d = dev()
+    eps = wl.eps_r.astype(np.float64); sig = wl.sigma.astype(np.float64)
+    st = {k: np.zeros((nz, nx)) for k in ("m_eps", "v_eps", "m_sig", "v_sig")}
+    t = lambda a: torch.as_tensor(padded(a.astype(np.float32), pitch), device=d)
+    d_eps, d_sig = t(eps), t(sig)
+    d_m = [torch.zeros((nz, pitch), device=d) for _ in range(4)]
+    ws = torch.empty(gprfwi_update_workspace_bytes(nz, pitch), dtype=torch.uint8, device=d)
+    for step in (1, 2, 3):
+        ge = rng.standard_normal((nz, nx)) * 1e-3; gs = rng.standard_normal((nz, nx)) * 2.0
+        d_ge, d_gs = t(ge), t(gs)
+        u = make_update_params(step=step, lr_eps_r=0.05, lr_sigma=2e-4, tv_iters=10, tv_lambda=0.01,
+                               mask_rows=wl.npml + 6, eps_r_min=1.0, sigma_min=0.0)
+        gprfwi_update(nz, nx, pitch, u, d_eps, d_sig, d_ge, d_gs, d_m[0], d_m[1], d_m[2], d_m[3], ws)
+        torch.cuda.synchronize()
+        eps, sig, ge_tv, gs_tv = ep.update(eps, sig, ge, gs, st, step, 0.05, 2e-4, tv_iters=10, tv_lambda=0.01,
+                                           mask_rows=wl.npml + 6)
+        for name, got, want, x in (("eps", d_ge, ge_tv, eps), ("sig", d_gs, gs_tv, sig)):
+            err = np.abs(got.cpu().numpy()[:, :nx] - want).max()
+            assert err <= 1e-5 * np.abs(x).max() + 1e-6 * np.abs(want).max(), (name, step, err)
+        assert rel_l2(d_eps.cpu().numpy()[:, :nx], eps) <= 1e-5
+        assert rel_l2(d_sig.cpu().numpy()[:, :nx], sig) <= 1e-5
+        assert d_eps.cpu().numpy()[:, :nx].min() >= 1.0 and d_sig.cpu().numpy()[:, :nx].min() >= 0.0
+        assert torch.all(d_eps[:, nx:] == 0)                       # pitch padding untouched

@@ -329,3 +329,64 @@ def test_geometry_on_ring_rejected():
         oracle.forward(problem(wl, src_zx=np.array([[0, 5]])), wl.eps_r, wl.sigma)
     with pytest.raises(ValueError):
         oracle.forward(problem(wl, rec_zx=np.array([[[5, wl.nx - 1]]])), wl.eps_r, wl.sigma)
+
+
+# ------------------------------------------------------------------------------------------------
+# iteration epilogue (a7): oracle/epilogue.py
+# ------------------------------------------------------------------------------------------------
+def test_epilogue_adam_first_step_closed_form_mask_and_clamp():
+    """Eqs. (14)-(15), at t = 1: m_hat = g, v_hat = g^2, so the step is
+    -lr g / (|g| + eps); masked rows do not move; clamps hold."""
+    from oracle import epilogue as ep
+    rng = np.random.default_rng(3)
+    x = rng.uniform(1.0, 9.0, (12, 17)); g = rng.standard_normal((12, 17)) * 3.0
+    xn, m, v = ep.adam_step(x, g, np.zeros_like(x), np.zeros_like(x), 1, lr=0.05, eps=1e-8, mask_rows=4, xmin=1.0)
+    want = x - 0.05 * g / (np.abs(g) + 1e-8)
+    assert np.array_equal(xn[:4], x[:4])
+    assert np.allclose(xn[4:], np.maximum(want[4:], 1.0), rtol=0, atol=1e-12)
+    assert xn.min() >= 1.0
+    # second step against the recursion written out
+    g2 = rng.standard_normal(x.shape)
+    xn2, m2, v2 = ep.adam_step(xn, g2, m, v, 2, lr=0.05)
+    mm = 0.9 * (0.1 * np.where(np.arange(12)[:, None] < 4, 0, g)) + 0.1 * g2
+    vv = 0.999 * (0.001 * np.where(np.arange(12)[:, None] < 4, 0, g) ** 2) + 0.001 * g2 ** 2
+    assert np.allclose(xn2, xn - 0.05 * (mm / (1 - 0.81)) / (np.sqrt(vv / (1 - 0.999 ** 2)) + 1e-8), atol=1e-12)
+
+
+def test_epilogue_tv_invariants():
+    """Eq. (17) shrink; constant model => zero TV term; the Jacobi sweeps converge to the solution of
+    (I + rho D^T D) U = U0 + rho D^T (Z - B) (dense solve on a tiny periodic grid, Z = B = 0 so U -> the
+    screened-Poisson smoothing of U0); TV term is small and acts against roughness."""
+    from oracle import epilogue as ep
+    vx, vz = ep.shrink(np.array([3.0, 0.1, 0.0]), np.array([4.0, 0.1, 0.0]), 1.0)
+    assert np.allclose(vx, [3.0 * 0.8, 0.0, 0.0]) and np.allclose(vz, [4.0 * 0.8, 0.0, 0.0])
+    assert np.all(ep.tv_gradient(np.full((9, 11), 7.5)) == 0.0)
+    rng = np.random.default_rng(5)
+    nz, nx, rho = 6, 7, 1.0
+    x = rng.uniform(1, 2, (nz, nx))
+    # dense periodic operator I + rho D^T D  (D^T D = 4 I - neighbours)
+    n = nz * nx
+    A = np.zeros((n, n))
+    for j in range(nz):
+        for i in range(nx):
+            k = j * nx + i
+            A[k, k] = 1 + 4 * rho
+            for (jj, ii) in ((j, (i + 1) % nx), (j, (i - 1) % nx), ((j + 1) % nz, i), ((j - 1) % nz, i)):
+                A[k, jj * nx + ii] -= rho
+    s = np.abs(x).max()
+    u_exact = np.linalg.solve(A, (x / s).ravel()).reshape(nz, nx)
+    # lambda so large that Z stays 0 (everything shrunk away) and B only accumulates G; one iteration = one sweep
+    g1 = ep.tv_gradient(x, iters=1, rho=rho, lam=1e9, alpha=1.0)
+    u1 = (x - g1) / s
+    nb = np.roll(x / s, 1, 0) + np.roll(x / s, -1, 0) + np.roll(x / s, 1, 1) + np.roll(x / s, -1, 1)
+    assert np.allclose(u1, (x / s + rho * nb) / (1 + 4 * rho), atol=1e-14)            # the sweep itself
+    # fixed point of the sweep with Z = B = 0 frozen is the dense solution
+    u = x / s
+    for _ in range(200):
+        nbu = np.roll(u, 1, 0) + np.roll(u, -1, 0) + np.roll(u, 1, 1) + np.roll(u, -1, 1)
+        u = (x / s + rho * nbu) / (1 + 4 * rho)
+    assert np.allclose(u, u_exact, atol=1e-10)
+    # roughness: TV term correlates positively with (x - local mean)
+    g = ep.tv_gradient(x)
+    loc = x - 0.25 * (np.roll(x, 1, 0) + np.roll(x, -1, 0) + np.roll(x, 1, 1) + np.roll(x, -1, 1))
+    assert np.sum(g * loc) > 0
