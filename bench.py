@@ -159,6 +159,7 @@ def main():
     from paper_2506_20513_b200 import (Simulation, build, gprfwi_gradient_host, gprfwi_residual, gprfwi_update,
                                        gprfwi_update_workspace_bytes, gprfwi_workspace_bytes,
                                        gprfwi_workspace_bytes_host, make_params, make_update_params)
+    from paper_2506_20513_b200.dist import allreduce_gradients
     build.build()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
@@ -199,8 +200,7 @@ def main():
         gprfwi_residual(tr, d_obs, res, misfit)
         if ev: ev[2].record(stream)
         ge, gs = sim.adjoint(res)
-        if world > 1:                      # shots are sharded over ranks: sum the gradients
-            dist.all_reduce(ge); dist.all_reduce(gs)
+        allreduce_gradients(ge, gs)        # shots are sharded over ranks: sum the gradients (no-op at N = 1)
         if ev: ev[3].record(stream)
         gprfwi_update(wl.nz, wl.nx, wl.nx, upd, eps_it, sig_it, ge, gs, adam[0], adam[1], adam[2], adam[3], ws_up)
         if ev:
