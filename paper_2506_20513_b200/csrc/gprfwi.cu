@@ -71,8 +71,10 @@ static Shape adj_shape()
   return {R, NW, MINB, (const void*)adj_kernel<R, NW, MINB>, RegTile<R, NW, 3>::smem_bytes(true),
           RegTile<R, NW, 3>::smem_bytes(false)};
 }
-static const Shape kFwdShapes[] = {fwd_shape<3, 8, 2>(), fwd_shape<4, 8, 2>(), fwd_shape<3, 12, 1>(), fwd_shape<2, 16, 2>()};
-static const Shape kAdjShapes[] = {adj_shape<3, 12, 1>(), adj_shape<3, 8, 2>(), adj_shape<4, 8, 1>(), adj_shape<2, 16, 2>()};
+static const Shape kFwdShapes[] = {fwd_shape<3, 12, 1>(), fwd_shape<3, 8, 2>(), fwd_shape<4, 12, 1>(), fwd_shape<4, 8, 1>(),
+                                   fwd_shape<5, 8, 1>(),  fwd_shape<6, 8, 1>(), fwd_shape<3, 16, 1>()};
+static const Shape kAdjShapes[] = {adj_shape<3, 12, 1>(), adj_shape<3, 8, 2>(), adj_shape<4, 12, 1>(), adj_shape<4, 8, 1>(),
+                                   adj_shape<5, 8, 1>(),  adj_shape<3, 16, 1>()};
 #endif
 static int shape_index(const char* env, int count)
 {
@@ -456,6 +458,25 @@ static int kernels_init(const gprfwi_params* p, const Layout& L)
   return GPRFWI_OK;
 }
 
+// every tile-kernel launch allows programmatic dependent launch (the kernels call griddepcontrol.wait
+// before they read the previous launch's output)
+static int launch_pdl(const Shape& sh, dim3 grid, void* arg, bool pml, cudaStream_t st)
+{
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(sh.threads());
+  cfg.dynamicSmemBytes = sh.smem(pml);
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = env_int("GPRFWI_PDL", 1) ? 1 : 0;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  void* args[] = {arg};
+  GPR_CUDA(cudaLaunchKernelExC(&cfg, sh.func, args));
+  return GPRFWI_OK;
+}
+
 static int lanes_init(gprfwi_handle* h)
 {
   if (!h->lanes.empty()) return GPRFWI_OK;
@@ -523,9 +544,8 @@ static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, 
   a.hz = L.T;
   a.oz = L.f.oz;
   const Shape& sh = kFwdShapes[L.fv];
-  dim3 grid(L.f.tiles_x, L.f.tiles_y, (ns + L.fgroup - 1) / L.fgroup), block(sh.threads());
-  void* args[] = {&a};
-  GPR_CUDA(cudaLaunchKernel(sh.func, grid, block, args, sh.smem(p.npml > 0), st));
+  dim3 grid(L.f.tiles_x, L.f.tiles_y, (ns + L.fgroup - 1) / L.fgroup);
+  if (int rc = launch_pdl(sh, grid, &a, p.npml > 0, st)) return rc;
   h->launches++;
   return GPRFWI_OK;
 }
@@ -564,9 +584,8 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   a.oz = L.a.oz;
   a.shot_base = shot0;
   const Shape& sh = kAdjShapes[L.av];
-  dim3 grid(L.a.tiles_x, L.a.tiles_y, ngrp), block(sh.threads());
-  void* args[] = {&a};
-  GPR_CUDA(cudaLaunchKernel(sh.func, grid, block, args, sh.smem(p.npml > 0), st));
+  dim3 grid(L.a.tiles_x, L.a.tiles_y, ngrp);
+  if (int rc = launch_pdl(sh, grid, &a, p.npml > 0, st)) return rc;
   h->launches++;
   return GPRFWI_OK;
 }

@@ -241,6 +241,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   TileCtx<R, NW, 3> c;
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
   const int grp = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
+  pdl_launch_dependents();
   c.template stage_tables<false>(g);
   c.zero_psi(g);
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
@@ -257,6 +258,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
     }
   }
 
+  pdl_wait();                          // everything below reads what the previous launch wrote
   const int s_end = min((grp + 1) * a.group, a.nshots);
   for (int s = grp * a.group; s < s_end; ++s) {
     // ---- everything this shot needs from global memory, issued together ----------------------------

@@ -210,9 +210,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
   const int s0 = blockIdx.z * a.group, s1 = min(s0 + a.group, a.nshots);
   const int tid = threadIdx.x;
 
-  // once per CTA: first shot's fields and scalars on their way, CPML tables -> shared memory,
-  // Ca / Cb of the region -> registers
-  fwd_fetch<R, NW>(a, c, s0);
+  // once per CTA, overlapping the previous launch's tail: CPML tables -> shared memory, Ca / Cb of the
+  // region -> registers; then, once the previous launch's state is complete, the first shot's fields
+  pdl_launch_dependents();
   if (tid < 7) c.meta_()[tid] = fwd_meta_word(a, s0, tile, ntile, tid);
   c.template stage_tables<true>(g);
   c.zero_psi(g);
@@ -226,6 +226,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
       ldg4a(a.cb + o, cb[r]);
     }
   }
+  pdl_wait();
+  fwd_fetch<R, NW>(a, c, s0);
   __syncthreads();
   // the receiver this thread records (receivers of the tile are dealt out one per thread)
   int2 ent_next = make_int2(-1, 0);

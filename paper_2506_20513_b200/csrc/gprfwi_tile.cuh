@@ -88,6 +88,11 @@ __device__ __forceinline__ void cp_async16(float* smem, const float* gmem)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+// Programmatic dependent launch: the next launch on the stream may start its prologue (everything that
+// does not read the previous launch's output) while this grid drains; pdl_wait() blocks until the
+// previous grid has completed and its writes are visible.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void zero4(float* v) { v[0] = v[1] = v[2] = v[3] = 0.f; }
 
 // Per-thread view of the region: where this lane's 4 columns and this warp's R rows sit in the grid,
