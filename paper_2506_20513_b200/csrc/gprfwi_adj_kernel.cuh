@@ -5,7 +5,7 @@
 //
 // Reverse step n, lamE written mu (masked: Ca = Cb = 0 on the PEC ring), q = Cb*mu:
 //   [A]  mu[rec] += residual[n+1]                          transpose of recording (staged in rowbuf)
-//        gCa += mu*E^n,  gCb += mu*(E^{n+1} - Ca*E^n)/Cb   owned cells; the /Cb is applied at the flush
+//        gCa += mu*E^n,  gCb += mu*(E^{n+1} - Ca*E^n)/Cb   owned cells; the /Cb is applied in grad_finalize
 //   [B]  tx = q/kex + cex*(psiEx + q),  psiEx <- bex*(psiEx + q)       (tx = q off the CPML)
 //        tz = -q/kez + cez*(psiEz - q), psiEz <- bez*(psiEz - q)       (tz = -q)
 //        lamHy += (tx[i] - tx[i+1])/dx,  lamHx += (tz[j] - tz[j+1])/dx,  mu <- Ca*mu
@@ -318,21 +318,15 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   }
 
   // ---- once per CTA: add the register partial sums to this group's gCa / gCb planes --------------------
+  // Fire-and-forget vector reductions (no CTA ever shares a cell of a group plane, so they are
+  // uncontended and the result does not depend on their order).  gb holds sum mu (E^{n+1} - Ca E^n);
+  // its division by Cb is done once per cell in grad_finalize_kernel.
 #pragma unroll
   for (int r = 0; r < R; ++r) {
     if (!((c.own >> r) & 1u)) continue;
     const long long o = grp * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-    float va[4], vb[4];
-    lds4a(a.gca + o, va);
-    lds4a(a.gcb + o, vb);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      if (cb[r][q] == 0.f) continue;                   // PEC cells and the ring: no dependence on Ca, Cb
-      va[q] += ga[r][q];
-      vb[q] += gb[r][q] / cb[r][q];
-    }
-    st4a(a.gca + o, va);
-    st4a(a.gcb + o, vb);
+    atomicAdd(reinterpret_cast<float4*>(a.gca + o), make_float4(ga[r][0], ga[r][1], ga[r][2], ga[r][3]));
+    atomicAdd(reinterpret_cast<float4*>(a.gcb + o), make_float4(gb[r][0], gb[r][1], gb[r][2], gb[r][3]));
   }
 }
 #endif

@@ -18,12 +18,14 @@ GPR_HD void coef_cell(float er, float sg, float rdt, float& ca, float& cb)
   cb = 1.0f / EA;
 }
 
-// chain rule Ca, Cb -> eps_r, sigma
-GPR_HD void grad_cell(float er, float sg, float rdt, float gca, float gcb, float& ge, float& gs)
+// chain rule Ca, Cb -> eps_r, sigma.  gcb_cb is the adjoint kernel's sum
+// mu (E^{n+1} - Ca E^n), i.e. Cb * dJ/dCb; with Cb = 1/EA the division by Cb is a multiplication by EA.
+GPR_HD void grad_cell(float er, float sg, float rdt, float gca, float gcb_cb, float& ge, float& gs)
 {
   if (sg > kPecSigma) { ge = 0.f; gs = 0.f; return; }
   const float a = kEps0 * er * rdt;
   const float EA = a + 0.5f * sg;
+  const float gcb = gcb_cb * EA;
   const float r2 = 1.0f / (EA * EA);
   ge = kEps0 * rdt * (gca * sg - gcb) * r2;
   gs = -(gca * a + 0.5f * gcb) * r2;
@@ -58,8 +60,9 @@ __global__ void grad_finalize_kernel(const float* __restrict__ eps_r, const floa
     sa += gca[g * plane + (long long)j * pitch + i];
     sb += gcb[g * plane + (long long)j * pitch + i];
   }
-  float ge, gs;
-  grad_cell(eps_r[(long long)j * upitch + i], sigma[(long long)j * upitch + i], rdt, sa, sb, ge, gs);
+  float ge = 0.f, gs = 0.f;                                  // the PEC ring does not depend on the model
+  if (i >= 1 && i <= nx - 2 && j >= 1 && j <= nz - 2)
+    grad_cell(eps_r[(long long)j * upitch + i], sigma[(long long)j * upitch + i], rdt, sa, sb, ge, gs);
   grad_eps[(long long)j * upitch + i] = ge;
   grad_sig[(long long)j * upitch + i] = gs;
 }
