@@ -71,10 +71,8 @@ static Shape adj_shape()
   return {R, NW, MINB, (const void*)adj_kernel<R, NW, MINB>, RegTile<R, NW, 3>::smem_bytes(true),
           RegTile<R, NW, 3>::smem_bytes(false)};
 }
-static const Shape kFwdShapes[] = {fwd_shape<3, 12, 1>(), fwd_shape<3, 8, 2>(), fwd_shape<4, 12, 1>(), fwd_shape<4, 8, 1>(),
-                                   fwd_shape<5, 8, 1>(),  fwd_shape<6, 8, 1>(), fwd_shape<3, 16, 1>()};
-static const Shape kAdjShapes[] = {adj_shape<3, 12, 1>(), adj_shape<3, 8, 2>(), adj_shape<4, 12, 1>(), adj_shape<4, 8, 1>(),
-                                   adj_shape<5, 8, 1>(),  adj_shape<3, 16, 1>()};
+static const Shape kFwdShapes[] = {fwd_shape<3, 12, 1>(), fwd_shape<3, 8, 2>(), fwd_shape<4, 12, 1>(), fwd_shape<2, 16, 1>()};
+static const Shape kAdjShapes[] = {adj_shape<3, 12, 1>(), adj_shape<3, 8, 2>(), adj_shape<4, 12, 1>(), adj_shape<2, 16, 1>()};
 #endif
 static int shape_index(const char* env, int count)
 {
