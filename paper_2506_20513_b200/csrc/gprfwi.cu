@@ -140,8 +140,6 @@ static void base_layout(const gprfwi_params* p, Layout& L)
     t.tiles_y = (p->nz + t.oz - 1) / t.oz;
   };
   L.fv = shape_index("GPRFWI_FWD_SHAPE", (int)(sizeof(kFwdShapes) / sizeof(Shape)));
-  // large grids: the taller forward tile (48 rows, 40 owned) wastes less on the halo (measured on config 3)
-  if (!std::getenv("GPRFWI_FWD_SHAPE") && (long long)p->nz * p->nx >= 500000) L.fv = 2;
   L.av = shape_index("GPRFWI_ADJ_SHAPE", (int)(sizeof(kAdjShapes) / sizeof(Shape)));
   tiling(kFwdShapes[L.fv].rows(), L.f);
   tiling(kAdjShapes[L.av].rows(), L.a);
