@@ -291,3 +291,35 @@ def test_epilogue_update_matches_numpy_oracle():
         assert rel_l2(d_sig.cpu().numpy()[:, :nx], sig) <= 1e-5
         assert d_eps.cpu().numpy()[:, :nx].min() >= 1.0 and d_sig.cpu().numpy()[:, :nx].min() >= 0.0
         assert torch.all(d_eps[:, nx:] == 0)                       # pitch padding untouched
+
+
+def test_many_receivers_per_tile_and_per_shot_wavelets():
+    """More receivers in one tile than the CTA has threads (the per-thread receiver entries overflow
+    into the strided loops), receivers on every region row (both words of the row mask), and one
+    wavelet per shot (wavelet_per_shot = 1)."""
+    wl = gi.small_random(nz=60, nx=100, nt=90, npml=8, nshots=2, nrec=900, seed=41)
+    rng = np.random.default_rng(2)
+    wav = np.stack([wl.wavelet, 0.5 * np.roll(wl.wavelet, 7)]).astype(np.float32)
+    wav[1, :7] = 0.0
+    pb = problem(wl, wavelet=wav.astype(np.float64))
+    tr_o = oracle.forward(pb, wl.eps_r, wl.sigma)["traces"]
+    res = (rng.standard_normal(tr_o.shape) * np.sqrt(np.mean(tr_o ** 2))).astype(np.float32)
+    ge_o, gs_o = oracle.gradient(pb, wl.eps_r, wl.sigma, res)
+    p = params_of(wl, wavelet_per_shot=1)
+    sim = Simulation(p, wl.src_zx, wl.rec_zx, wav, dev())
+    tr = sim.forward(torch.as_tensor(wl.eps_r, device=dev()), torch.as_tensor(wl.sigma, device=dev())).cpu().numpy().copy()
+    ge, gs = [t.cpu().numpy().copy() for t in sim.adjoint(torch.as_tensor(res, device=dev()))]
+    sim.close()
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o), " 900 receivers, per-shot wavelets")
+
+
+def test_no_receivers_forward_only():
+    """nrec = 0: nothing to record or inject; forward and adjoint must still run (zero gradient)."""
+    wl = gi.small_random(nz=40, nx=50, nt=30, npml=6, nshots=2, nrec=1, seed=8)
+    p = params_of(wl, nrec=0)
+    sim = Simulation(p, wl.src_zx, np.zeros((2, 0, 2), np.int32), wl.wavelet, dev())
+    sim.forward(torch.as_tensor(wl.eps_r, device=dev()), torch.as_tensor(wl.sigma, device=dev()))
+    ge, gs = sim.adjoint(torch.zeros((2, 30, 0), device=dev()))
+    torch.cuda.synchronize()
+    assert float(ge.abs().max()) == 0.0 and float(gs.abs().max()) == 0.0
+    sim.close()
