@@ -6,6 +6,8 @@ the expectations are an analytic solution (Hankel function via SciPy), conservat
 (reciprocity), the adjoint identity against complex-step derivatives of the forward code, finite
 differences of the misfit, closed-form special cases and brute force on tiny inputs.
 """
+import os
+
 import numpy as np
 import pytest
 from scipy.special import hankel2
@@ -390,3 +392,19 @@ def test_epilogue_tv_invariants():
     g = ep.tv_gradient(x)
     loc = x - 0.25 * (np.roll(x, 1, 0) + np.roll(x, -1, 0) + np.roll(x, 1, 1) + np.roll(x, -1, 1))
     assert np.sum(g * loc) > 0
+
+
+def test_golden_config1_oracle_values_unchanged():
+    """tests/golden/config1_oracle.txt (written by tests/golden/make_golden.py from the oracle alone):
+    the oracle and the input generator still give the frozen numbers."""
+    import importlib.util
+    here = os.path.dirname(os.path.abspath(__file__))
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "golden", "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec); spec.loader.exec_module(mg)
+    now = mg.values()
+    with open(os.path.join(here, "golden", "config1_oracle.txt")) as f:
+        for line in f:
+            if line.startswith("#"):
+                continue
+            k, v = line.rsplit(" ", 1)
+            assert abs(now[k] - float(v)) <= 1e-9 * max(abs(float(v)), 1e-30), k
