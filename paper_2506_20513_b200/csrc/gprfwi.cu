@@ -166,7 +166,7 @@ static void set_groups(const gprfwi_params* p, Layout& L)
 {
   const int fslots = 148 * std::max(1, kFwdShapes[L.fv].minb), aslots = 148 * std::max(1, kAdjShapes[L.av].minb);
   pick_groups(L.f.tiles(), p->nshots, fslots, 2, L.fgroup, L.fngroups);
-  pick_groups(L.a.tiles(), L.Sb, aslots, 3, L.group, L.ngroups);
+  pick_groups(L.a.tiles(), L.Sb, aslots, 2, L.group, L.ngroups);
   if (int g = env_int("GPRFWI_FWD_GROUP", 0)) { L.fgroup = std::min(g, p->nshots); L.fngroups = (p->nshots + L.fgroup - 1) / L.fgroup; }
   if (int g = env_int("GPRFWI_ADJ_GROUP", 0)) { L.group = std::min(g, L.Sb); L.ngroups = (L.Sb + L.group - 1) / L.group; }
 }

@@ -138,7 +138,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
         }
         st4a(c.pez_() + r * kRegW, p);
       }
-      if (XP && c.xslot >= 0) {          // lanes off the x CPML keep tx = q
+      if (XP) {                          // (all lanes: trivial coefficients off the CPML give tx = q exactly)
         float p[4], b[4], cc[4], ik[4];
         lds4a(c.pex_() + r * kRegW, p);
         lds4a(c.tabx_() + 3 * kRegW + c.l4, b); lds4a(c.tabx_() + 4 * kRegW + c.l4, cc); lds4a(c.tabx_() + 5 * kRegW + c.l4, ik);
@@ -193,7 +193,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
         }
         st4a(c.phz_() + r * kRegW, p);
       }
-      if (XP && c.xslot >= 0) {          // lanes off the x CPML keep sx = Db lamHy
+      if (XP) {                          // (all lanes: trivial coefficients off the CPML give sx = Db lamHy)
         float p[4], b[4], cc[4], ik[4];
         lds4a(c.phx_() + r * kRegW, p);
         lds4a(c.tabx_() + 0 * kRegW + c.l4, b); lds4a(c.tabx_() + 1 * kRegW + c.l4, cc); lds4a(c.tabx_() + 2 * kRegW + c.l4, ik);

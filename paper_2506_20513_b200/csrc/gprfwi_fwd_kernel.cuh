@@ -62,10 +62,11 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
     }
 
     // ---- stages 2-3: H update + H CPML -------------------------------------------------------------
-    // x tables of this lane's columns (XP only; lanes off the CPML use the trivial coefficients
-    // and a psi of zero without touching shared memory)
+    // x tables of this lane's columns (XP only; every lane of an XP warp runs the psi form -- lanes off
+    // the CPML have the trivial coefficients and a psi of zero; predicating them off costs more in
+    // divergent branches than the shared-memory traffic it saves: measured)
     float xb[4] = {0.f, 0.f, 0.f, 0.f}, xc[4] = {0.f, 0.f, 0.f, 0.f}, xk[4] = {kap, kap, kap, kap};
-    const bool xl = XP && c.xslot >= 0;
+    const bool xl = XP;
     if (xl) { lds4a(c.tabx_() + 0 * kRegW + c.l4, xb); lds4a(c.tabx_() + 1 * kRegW + c.l4, xc); lds4a(c.tabx_() + 2 * kRegW + c.l4, xk); }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -266,7 +267,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
 #pragma unroll
     for (int r = 0; r < R; ++r) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
     // ---- next shot: fields into the (now free) landing slots, scalars into the other meta slot ------
-    cp_async_wait<0>();                // psi landed
+    if (s + 1 >= s1) cp_async_commit();   // (keeps the group count uniform: psi is always the second newest)
     if (s + 1 < s1) {
       fwd_fetch<R, NW>(a, c, s + 1);
       if (tid < 7) c.meta_()[(((s - s0) & 1) ^ 1) * 8 + tid] = fwd_meta_word(a, s + 1, tile, ntile, tid);
@@ -284,6 +285,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
     }
     __syncthreads();
     const unsigned rflags = c.row_flags();
+    cp_async_wait<1>();                // psi landed (the next shot's fields may still be in flight)
 
     if (c.zp && c.xp) fwd_steps<R, NW, true, true>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
     else if (c.zp) fwd_steps<R, NW, true, false>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
