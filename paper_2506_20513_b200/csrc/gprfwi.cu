@@ -368,7 +368,7 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
       const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
       const int ty = rz / L.f.oz, tx = rx / kOwnW;
       const size_t k = (size_t)s * R + fill[tile_of[r]]++;
-      h->h_blk_ent[2 * k] = (rz - (ty * L.f.oz - L.T)) * kRegW + (rx - (tx * kOwnW - 4));
+      h->h_blk_ent[2 * k] = (rz - (ty * L.f.oz - L.T)) * kRegW + col_pos(rx - (tx * kOwnW - 4));   // internal column order
       h->h_blk_ent[2 * k + 1] = r;
     }
   }
@@ -393,7 +393,7 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
       const int ty = t / L.a.tiles_x, tx = t % L.a.tiles_x;
       for (int r : bucket[t]) {
         const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
-        h->h_reg_ent.push_back((rz - (ty * L.a.oz - L.T)) * kRegW + (rx - (tx * kOwnW - 4)));
+        h->h_reg_ent.push_back((rz - (ty * L.a.oz - L.T)) * kRegW + col_pos(rx - (tx * kOwnW - 4)));
         h->h_reg_ent.push_back(r);
       }
       h->h_reg_start[(size_t)s * natile + t + 1] = (int)(h->h_reg_ent.size() / 2);

@@ -75,17 +75,17 @@ __device__ __forceinline__ void adj_fetch(const AdjArgs& a, const TileCtx<R, NW,
 
 // The T reverse steps of one warp for one shot; ZP / XP as in fwd_steps (the psi forms below give
 // exactly tx = q, tz = -q, sx, sz = +-Db lamH with the trivial coefficients outside the CPML).
+// Packed pairs as in the forward kernel: P = (c0, c2), Q = (c1, c3).
 template <int R, int NW, bool ZP, bool XP>
 __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
-                                          int2 ent, const float (&rv)[kMaxT], unsigned iflags, float (&le)[R][4], float (&lhx)[R][4], float (&lhy)[R][4],
-                                          const float (&ca)[R][4], const float (&cb)[R][4],
-                                          float (&ga)[R][4], float (&gb)[R][4])
+                                          int2 ent, const float (&rv)[kMaxT], unsigned iflags,
+                                          P2 (&le)[R], P2 (&lhx)[R], P2 (&lhy)[R], const P2 (&ca)[R], const P2 (&cb)[R],
+                                          P2 (&ga)[R], P2 (&gb)[R])
 {
   using L = RegTile<R, NW, 3>;
-  const Geo& g = a.g;
   const unsigned full = 0xffffffffu;
-  const float rdx = g.rdx, Db = g.Db;
-  #pragma unroll 1
+  const u64 rdx2 = bc2(a.g.rdx), Db2 = bc2(a.g.Db), nDb2 = bc2(-a.g.Db);
+#pragma unroll 1
   for (int t = 0; t < a.nsub; ++t) {
     // ---- [A] adjoint source, gradient terms ------------------------------------------------------
     adj_fetch<R, NW>(a, c, s, t + 2);                   // two steps ahead; planes t and t+1 have landed after the wait
@@ -95,141 +95,105 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       if ((iflags >> r) & 1u) {
-        float v[4];
         float* rb = c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4;
-        lds4a(rb, v);
-        le[r][0] = FA(le[r][0], v[0]); le[r][1] = FA(le[r][1], v[1]);
-        le[r][2] = FA(le[r][2], v[2]); le[r][3] = FA(le[r][3], v[3]);
-        zero4(v);
-        st4a(rb, v);
+        const P2 v = ld2(rb);
+        le[r].p = add2(le[r].p, v.p); le[r].q = add2(le[r].q, v.q);
+        st2(rb, zero2());
       }
       if ((c.own >> r) & 1u) {
-        float e0[4], e1[4];
-        lds4a(h0 + r * kRegW, e0);                     // E^n
-        lds4a(h1 + r * kRegW, e1);                     // E^{n+1}
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          ga[r][q] = FF(le[r][q], e0[q], ga[r][q]);
-          gb[r][q] = FF(le[r][q], FF(-ca[r][q], e0[q], e1[q]), gb[r][q]);
-        }
+        const P2 e0 = ld2(h0 + r * kRegW), e1 = ld2(h1 + r * kRegW);      // E^n, E^{n+1}
+        ga[r].p = fma2(le[r].p, e0.p, ga[r].p); ga[r].q = fma2(le[r].q, e0.q, ga[r].q);
+        gb[r].p = fma2(le[r].p, fma2(neg2(ca[r].p), e0.p, e1.p), gb[r].p);
+        gb[r].q = fma2(le[r].q, fma2(neg2(ca[r].q), e0.q, e1.q), gb[r].q);
       }
     }
     // ---- [B] transpose of the E update + E CPML ----------------------------------------------------
-    float tzp[4], tz0[4];                             // tz of the previous row; of the warp's row R-1
+    P2 xb = zero2(), xc = zero2(), xk = zero2();
+    if (XP) { xb = ld2(c.tabx_() + 3 * kRegW + c.l4); xc = ld2(c.tabx_() + 4 * kRegW + c.l4); xk = ld2(c.tabx_() + 5 * kRegW + c.l4); }
+    P2 tzp = zero2();                                   // tz of the previous row; after the loop: of row R-1
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      float tx[4], tz[4];
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const float qv = FM(cb[r][q], le[r][q]);
-        tx[q] = qv; tz[q] = -qv;
-        le[r][q] = FM(ca[r][q], le[r][q]);
-      }
+      P2 tx, tz;
+      tx.p = mul2(cb[r].p, le[r].p); tx.q = mul2(cb[r].q, le[r].q);       // q = Cb mu
+      tz.p = neg2(tx.p); tz.q = neg2(tx.q);
+      le[r].p = mul2(ca[r].p, le[r].p); le[r].q = mul2(ca[r].q, le[r].q);
       if (ZP) {
-        float p[4];
-        lds4a(c.pez_() + r * kRegW, p);
-        const float b = c.tabz_()[3 * L::ROWS + c.lr0 + r], cc = c.tabz_()[4 * L::ROWS + c.lr0 + r],
-                    ik = c.tabz_()[5 * L::ROWS + c.lr0 + r];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const float T_ = FA(p[q], tz[q]);           // psiEz - q
-          tz[q] = FF(cc, T_, FM(tz[q], ik));
-          p[q] = FM(b, T_);
-        }
-        st4a(c.pez_() + r * kRegW, p);
+        P2 p = ld2(c.pez_() + r * kRegW);
+        const u64 b = bc2(c.tabz_()[3 * L::ROWS + c.lr0 + r]), cc = bc2(c.tabz_()[4 * L::ROWS + c.lr0 + r]),
+                  ik = bc2(c.tabz_()[5 * L::ROWS + c.lr0 + r]);
+        const u64 Tp = add2(p.p, tz.p), Tq = add2(p.q, tz.q);             // psiEz - q
+        tz.p = fma2(cc, Tp, mul2(tz.p, ik)); tz.q = fma2(cc, Tq, mul2(tz.q, ik));
+        p.p = mul2(b, Tp); p.q = mul2(b, Tq);
+        st2(c.pez_() + r * kRegW, p);
       }
-      if (XP) {                          // (all lanes: trivial coefficients off the CPML give tx = q exactly)
-        float p[4], b[4], cc[4], ik[4];
-        lds4a(c.pex_() + r * kRegW, p);
-        lds4a(c.tabx_() + 3 * kRegW + c.l4, b); lds4a(c.tabx_() + 4 * kRegW + c.l4, cc); lds4a(c.tabx_() + 5 * kRegW + c.l4, ik);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          {
-            const float T_ = FA(p[q], tx[q]);         // psiEx + q
-            tx[q] = FF(cc[q], T_, FM(tx[q], ik[q]));
-            p[q] = FM(b[q], T_);
-          }
-        }
-        st4a(c.pex_() + r * kRegW, p);
+      if (XP) {                                         // (all lanes: trivial coefficients off the CPML give tx = q exactly)
+        P2 p = ld2(c.pex_() + r * kRegW);
+        const u64 Tp = add2(p.p, tx.p), Tq = add2(p.q, tx.q);             // psiEx + q
+        tx.p = fma2(xc.p, Tp, mul2(tx.p, xk.p)); tx.q = fma2(xc.q, Tq, mul2(tx.q, xk.q));
+        p.p = mul2(xb.p, Tp); p.q = mul2(xb.q, Tq);
+        st2(c.pex_() + r * kRegW, p);
       }
-      const float txn[4] = {tx[1], tx[2], tx[3], __shfl_down_sync(full, tx[0], 1)};     // tx to the right
-#pragma unroll
-      for (int q = 0; q < 4; ++q) lhy[r][q] = FF(rdx, FS(tx[q], txn[q]), lhy[r][q]);
-      if (r == 0) st4a(c.xe_() + c.w * kRegW + c.l4, tz);
+      // tx to the right of (c0, c2) is Q; to the right of (c1, c3) it is (c2, c0 of the next lane)
+      const u64 txnq = pk(hi2(tx.p), __shfl_down_sync(full, lo2(tx.p), 1));
+      lhy[r].p = fma2(rdx2, sub2(tx.p, tx.q), lhy[r].p);
+      lhy[r].q = fma2(rdx2, sub2(tx.q, txnq), lhy[r].q);
+      if (r == 0) st2(c.xe_() + c.w * kRegW + c.l4, tz);
       else {
-#pragma unroll
-        for (int q = 0; q < 4; ++q) lhx[r - 1][q] = FF(rdx, FS(tzp[q], tz[q]), lhx[r - 1][q]);
+        lhx[r - 1].p = fma2(rdx2, sub2(tzp.p, tz.p), lhx[r - 1].p);
+        lhx[r - 1].q = fma2(rdx2, sub2(tzp.q, tz.q), lhx[r - 1].q);
       }
-#pragma unroll
-      for (int q = 0; q < 4; ++q) tzp[q] = tz[q];
+      tzp = tz;
     }
-#pragma unroll
-    for (int q = 0; q < 4; ++q) tz0[q] = tzp[q];
     __syncthreads();
     if (t + 1 < a.nsub) adj_stage<R, NW>(a, c, s, rk0, rk1, ent, rv, t + 1);
     {
-      float tzb[4];                                   // tz of the row below the warp's last row
-      lds4a(c.xe_() + (c.w + 1) * kRegW + c.l4, tzb);
-#pragma unroll
-      for (int q = 0; q < 4; ++q) lhx[R - 1][q] = FF(rdx, FS(tz0[q], tzb[q]), lhx[R - 1][q]);
+      const P2 tzb = ld2(c.xe_() + (c.w + 1) * kRegW + c.l4);             // tz of the row below the warp's last row
+      lhx[R - 1].p = fma2(rdx2, sub2(tzp.p, tzb.p), lhx[R - 1].p);
+      lhx[R - 1].q = fma2(rdx2, sub2(tzp.q, tzb.q), lhx[R - 1].q);
     }
     // ---- [C] transpose of the H update + H CPML ----------------------------------------------------
-    float szp[4], sz0[4];
+    if (XP) { xb = ld2(c.tabx_() + 0 * kRegW + c.l4); xc = ld2(c.tabx_() + 1 * kRegW + c.l4); xk = ld2(c.tabx_() + 2 * kRegW + c.l4); }
+    P2 szp = zero2(), sz0 = zero2();
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      float sx[4], sz[4];
-#pragma unroll
-      for (int q = 0; q < 4; ++q) { sz[q] = FM(-Db, lhx[r][q]); sx[q] = FM(Db, lhy[r][q]); }
+      P2 sx, sz;
+      sz.p = mul2(nDb2, lhx[r].p); sz.q = mul2(nDb2, lhx[r].q);
+      sx.p = mul2(Db2, lhy[r].p); sx.q = mul2(Db2, lhy[r].q);
       if (ZP) {
-        float p[4];
-        lds4a(c.phz_() + r * kRegW, p);
-        const float b = c.tabz_()[0 * L::ROWS + c.lr0 + r], cc = c.tabz_()[1 * L::ROWS + c.lr0 + r],
-                    ik = c.tabz_()[2 * L::ROWS + c.lr0 + r];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const float T_ = FA(p[q], sz[q]);
-          sz[q] = FF(cc, T_, FM(sz[q], ik));
-          p[q] = FM(b, T_);
-        }
-        st4a(c.phz_() + r * kRegW, p);
+        P2 p = ld2(c.phz_() + r * kRegW);
+        const u64 b = bc2(c.tabz_()[0 * L::ROWS + c.lr0 + r]), cc = bc2(c.tabz_()[1 * L::ROWS + c.lr0 + r]),
+                  ik = bc2(c.tabz_()[2 * L::ROWS + c.lr0 + r]);
+        const u64 Tp = add2(p.p, sz.p), Tq = add2(p.q, sz.q);
+        sz.p = fma2(cc, Tp, mul2(sz.p, ik)); sz.q = fma2(cc, Tq, mul2(sz.q, ik));
+        p.p = mul2(b, Tp); p.q = mul2(b, Tq);
+        st2(c.phz_() + r * kRegW, p);
       }
-      if (XP) {                          // (all lanes: trivial coefficients off the CPML give sx = Db lamHy)
-        float p[4], b[4], cc[4], ik[4];
-        lds4a(c.phx_() + r * kRegW, p);
-        lds4a(c.tabx_() + 0 * kRegW + c.l4, b); lds4a(c.tabx_() + 1 * kRegW + c.l4, cc); lds4a(c.tabx_() + 2 * kRegW + c.l4, ik);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          {
-            const float T_ = FA(p[q], sx[q]);
-            sx[q] = FF(cc[q], T_, FM(sx[q], ik[q]));
-            p[q] = FM(b[q], T_);
-          }
-        }
-        st4a(c.phx_() + r * kRegW, p);
+      if (XP) {                                         // (all lanes: trivial coefficients off the CPML give sx = Db lamHy)
+        P2 p = ld2(c.phx_() + r * kRegW);
+        const u64 Tp = add2(p.p, sx.p), Tq = add2(p.q, sx.q);
+        sx.p = fma2(xc.p, Tp, mul2(sx.p, xk.p)); sx.q = fma2(xc.q, Tq, mul2(sx.q, xk.q));
+        p.p = mul2(xb.p, Tp); p.q = mul2(xb.q, Tq);
+        st2(c.phx_() + r * kRegW, p);
       }
-      const float sxl[4] = {__shfl_up_sync(full, sx[3], 1), sx[0], sx[1], sx[2]};       // sx to the left
-#pragma unroll
-      for (int q = 0; q < 4; ++q) le[r][q] = FF(rdx, FS(sxl[q], sx[q]), le[r][q]);
-      if (r == 0) {
-#pragma unroll
-        for (int q = 0; q < 4; ++q) sz0[q] = sz[q];
-      } else {
-#pragma unroll
-        for (int q = 0; q < 4; ++q) le[r][q] = FF(rdx, FS(szp[q], sz[q]), le[r][q]);
+      // sx to the left of (c0, c2) is (c3 of the previous lane, c1); to the left of (c1, c3) it is P
+      const u64 sxlp = pk(__shfl_up_sync(full, hi2(sx.q), 1), lo2(sx.q));
+      le[r].p = fma2(rdx2, sub2(sxlp, sx.p), le[r].p);
+      le[r].q = fma2(rdx2, sub2(sx.p, sx.q), le[r].q);
+      if (r == 0) sz0 = sz;
+      else {
+        le[r].p = fma2(rdx2, sub2(szp.p, sz.p), le[r].p);
+        le[r].q = fma2(rdx2, sub2(szp.q, sz.q), le[r].q);
       }
-      if (r == R - 1) st4a(c.xh_() + (c.w + 1) * kRegW + c.l4, sz);
-#pragma unroll
-      for (int q = 0; q < 4; ++q) szp[q] = sz[q];
+      if (r == R - 1) st2(c.xh_() + (c.w + 1) * kRegW + c.l4, sz);
+      szp = sz;
     }
     __syncthreads();
     {
-      float sza[4];                                   // sz of the row above the warp's first row
-      lds4a(c.xh_() + c.w * kRegW + c.l4, sza);
-#pragma unroll
-      for (int q = 0; q < 4; ++q) le[0][q] = FF(rdx, FS(sza[q], sz0[q]), le[0][q]);
+      const P2 sza = ld2(c.xh_() + c.w * kRegW + c.l4);                   // sz of the row above the warp's first row
+      le[0].p = fma2(rdx2, sub2(sza.p, sz0.p), le[0].p);
+      le[0].q = fma2(rdx2, sub2(sza.q, sz0.q), le[0].q);
     }
   }
-
 }
 
 template <int R, int NW, int MINB>
@@ -247,14 +211,14 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
     reinterpret_cast<float4*>(c.rowbuf_())[k] = make_float4(0.f, 0.f, 0.f, 0.f);
 
-  float ca[R][4], cb[R][4], ga[R][4], gb[R][4];
+  P2 ca[R], cb[R], ga[R], gb[R];
 #pragma unroll
   for (int r = 0; r < R; ++r) {
-    zero4(ca[r]); zero4(cb[r]); zero4(ga[r]); zero4(gb[r]);
+    ca[r] = zero2(); cb[r] = zero2(); ga[r] = zero2(); gb[r] = zero2();
     if (c.colin && ((c.rin >> r) & 1u)) {
       const long long o = (long long)(c.gj0 + r) * g.pitch + c.gi;
-      ldg4a(a.ca + o, ca[r]);
-      ldg4a(a.cb + o, cb[r]);
+      ca[r] = ldg2(a.ca + o);
+      cb[r] = ldg2(a.cb + o);
     }
   }
 
@@ -264,15 +228,15 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
     // ---- everything this shot needs from global memory, issued together ----------------------------
     const long long row = (long long)(a.shot_base + s) * (a.tiles_x * a.tiles_y) + tile;
     const int rk0 = a.reg_start[row], rk1 = a.reg_start[row + 1];
-    float le[R][4], lhx[R][4], lhy[R][4];
+    P2 le[R], lhx[R], lhy[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      zero4(le[r]); zero4(lhx[r]); zero4(lhy[r]);
+      le[r] = zero2(); lhx[r] = zero2(); lhy[r] = zero2();
       if (c.colin && ((c.rin >> r) & 1u)) {
         const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-        ldg4a(a.in.ez + o, le[r]);
-        ldg4a(a.in.hx + o, lhx[r]);
-        ldg4a(a.in.hy + o, lhy[r]);
+        le[r] = ldg2(a.in.ez + o);
+        lhx[r] = ldg2(a.in.hx + o);
+        lhy[r] = ldg2(a.in.hy + o);
       }
     }
     adj_fetch<R, NW>(a, c, s, 0);
@@ -310,9 +274,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
     for (int r = 0; r < R; ++r) {
       if (!((c.own >> r) & 1u)) continue;
       const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-      st4a(a.out.ez + o, le[r]);
-      st4a(a.out.hx + o, lhx[r]);
-      st4a(a.out.hy + o, lhy[r]);
+      st2(a.out.ez + o, le[r]);
+      st2(a.out.hx + o, lhx[r]);
+      st2(a.out.hy + o, lhy[r]);
     }
     if (c.zp || c.xp) c.store_psi(g, a.out, s);
   }
@@ -325,8 +289,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   for (int r = 0; r < R; ++r) {
     if (!((c.own >> r) & 1u)) continue;
     const long long o = grp * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-    atomicAdd(reinterpret_cast<float4*>(a.gca + o), make_float4(ga[r][0], ga[r][1], ga[r][2], ga[r][3]));
-    atomicAdd(reinterpret_cast<float4*>(a.gcb + o), make_float4(gb[r][0], gb[r][1], gb[r][2], gb[r][3]));
+    // (memory order inside a unit is c0 c2 c1 c3 = P.lo P.hi Q.lo Q.hi, like every internal plane)
+    atomicAdd(reinterpret_cast<float4*>(a.gca + o), make_float4(lo2(ga[r].p), hi2(ga[r].p), lo2(ga[r].q), hi2(ga[r].q)));
+    atomicAdd(reinterpret_cast<float4*>(a.gcb + o), make_float4(lo2(gb[r].p), hi2(gb[r].p), lo2(gb[r].q), hi2(gb[r].q)));
   }
 }
 #endif

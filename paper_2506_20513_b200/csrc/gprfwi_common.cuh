@@ -62,6 +62,13 @@ GPR_HD int xstrip_slot(int u, int xnl, int xur, int pitch)
   return u < 0 ? -1 : (u < xnl ? 4 * u : ((u >= xur && 4 * u < pitch) ? 4 * (xnl + u - xur) : -1));
 }
 
+// INTERNAL column order (every [..][pitch] array the library owns: fields, psi, Ca, Cb, history, gCa, gCb):
+// inside each aligned group of four columns (c0 c1 c2 c3) the floats are stored as (c0 c2 c1 c3), so that a
+// 128-bit load yields two packed pairs P = (c0, c2), Q = (c1, c3) for the sm_100 FFMA2 / FADD2 / FMUL2
+// instructions with every x-neighbour difference (c1 - c0, c3 - c2) a plain pair operation.
+GPR_HD int unit_perm(int c) { return c == 1 ? 2 : (c == 2 ? 1 : c); }
+GPR_HD int col_pos(int i) { return (i & ~3) | unit_perm(i & 3); }
+
 GPR_HD float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
 GPR_HD void st4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
 GPR_HD float4 mk4(float a, float b, float c, float d) { float4 v; v.x = a; v.y = b; v.z = c; v.w = d; return v; }

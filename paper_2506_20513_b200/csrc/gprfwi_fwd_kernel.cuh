@@ -14,6 +14,8 @@
 //   Ez  = Ca Ez + Cb (((Hy - Hy[i-1])/kx - (Hx - Hx[j-1])/kz)/dx + (psix - psiz))
 // A warp whose rows (ZP) / whose CTA's columns (XP) touch the CPML runs the psi form on all its
 // cells, every other warp the plain form; a cell's value does not depend on which form computed it.
+// All arithmetic is packed fp32 pairs (FFMA2 / FADD2 / FMUL2, gprfwi_tile.cuh): each component is
+// rounded exactly like the scalar operation, at half the issue slots.
 #pragma once
 #include "gprfwi_tile.cuh"
 
@@ -39,17 +41,18 @@ struct FwdArgs {
 
 #if defined(__CUDACC__)
 // The T-step loop of one warp.  All variants hit the same barriers, so the warps of one CTA may run
-// different variants.
+// different variants.  Every field row of the thread is two packed pairs P = (c0, c2), Q = (c1, c3):
+// differences to the right / left neighbour are Q - P resp. P - Q for half the cells and need one
+// repacked pair (with the lane shuffle) for the other half.
 template <int R, int NW, bool ZP, bool XP>
 __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
                                           int2 ent, unsigned rflags, int src_r, int src_c, const float (&wv)[kMaxT],
-                                          float (&e)[R][4], float (&hx)[R][4], float (&hy)[R][4],
-                                          const float (&ca)[R][4], const float (&cb)[R][4])
+                                          P2 (&e)[R], P2 (&hx)[R], P2 (&hy)[R], const P2 (&ca)[R], const P2 (&cb)[R])
 {
   using L = RegTile<R, NW, 3>;
   const Geo& g = a.g;
   const unsigned full = 0xffffffffu;
-  const float rdx = g.rdx, Db = g.Db, kap = g.kap;
+  const u64 rdx2 = bc2(g.rdx), Db2 = bc2(g.Db), nDb2 = bc2(-g.Db), kap2 = bc2(g.kap), nkap2 = bc2(-g.kap);
   const long long hoff = s * g.plane + (long long)c.gj0 * g.pitch + c.gi;     // this thread's row 0 in a plane of shot s
   float* const trp = a.traces + (s * a.trace_stride + ent.y);                 // this thread's receiver, sample n
 #pragma unroll 1
@@ -65,83 +68,78 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
     // x tables of this lane's columns (XP only; every lane of an XP warp runs the psi form -- lanes off
     // the CPML have the trivial coefficients and a psi of zero; predicating them off costs more in
     // divergent branches than the shared-memory traffic it saves: measured)
-    float xb[4] = {0.f, 0.f, 0.f, 0.f}, xc[4] = {0.f, 0.f, 0.f, 0.f}, xk[4] = {kap, kap, kap, kap};
-    const bool xl = XP;
-    if (xl) { lds4a(c.tabx_() + 0 * kRegW + c.l4, xb); lds4a(c.tabx_() + 1 * kRegW + c.l4, xc); lds4a(c.tabx_() + 2 * kRegW + c.l4, xk); }
+    P2 xb = zero2(), xc = zero2(), xk = zero2();
+    if (XP) { xb = ld2(c.tabx_() + 0 * kRegW + c.l4); xc = ld2(c.tabx_() + 1 * kRegW + c.l4); xk = ld2(c.tabx_() + 2 * kRegW + c.l4); }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      float eb[4];                                      // Ez of the row below
-      if (r + 1 < R) { eb[0] = e[r + 1][0]; eb[1] = e[r + 1][1]; eb[2] = e[r + 1][2]; eb[3] = e[r + 1][3]; }
-      else lds4a(c.xe_() + (c.w + 1) * kRegW + c.l4, eb);
-      const float en[4] = {e[r][1], e[r][2], e[r][3], __shfl_down_sync(full, e[r][0], 1)};   // Ez to the right
+      const P2 eb = (r + 1 < R) ? e[r + 1] : ld2(c.xe_() + (c.w + 1) * kRegW + c.l4);     // Ez of the row below
+      // Ez to the right of (c1, c3) is (c2, c0 of the next lane); to the right of (c0, c2) it is Q itself
+      const u64 enq = pk(hi2(e[r].p), __shfl_down_sync(full, lo2(e[r].p), 1));
       if (ZP) {
-        float p[4];
-        lds4a(c.phz_() + r * kRegW, p);
-        const float b = c.tabz_()[0 * L::ROWS + c.lr0 + r], cr = c.tabz_()[1 * L::ROWS + c.lr0 + r],
-                    kk = c.tabz_()[2 * L::ROWS + c.lr0 + r];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const float d = FS(eb[q], e[r][q]);
-          p[q] = FF(b, p[q], FM(cr, d));
-          hx[r][q] = FF(-Db, p[q], FF(-kk, d, hx[r][q]));
-        }
-        st4a(c.phz_() + r * kRegW, p);
+        P2 p = ld2(c.phz_() + r * kRegW);
+        const u64 b = bc2(c.tabz_()[0 * L::ROWS + c.lr0 + r]), cr = bc2(c.tabz_()[1 * L::ROWS + c.lr0 + r]),
+                  nkk = bc2(-c.tabz_()[2 * L::ROWS + c.lr0 + r]);
+        const u64 dp = sub2(eb.p, e[r].p), dq = sub2(eb.q, e[r].q);
+        p.p = fma2(b, p.p, mul2(cr, dp)); p.q = fma2(b, p.q, mul2(cr, dq));
+        hx[r].p = fma2(nDb2, p.p, fma2(nkk, dp, hx[r].p)); hx[r].q = fma2(nDb2, p.q, fma2(nkk, dq, hx[r].q));
+        st2(c.phz_() + r * kRegW, p);
       } else {
-#pragma unroll
-        for (int q = 0; q < 4; ++q) hx[r][q] = FF(-kap, FS(eb[q], e[r][q]), hx[r][q]);
+        hx[r].p = fma2(nkap2, sub2(eb.p, e[r].p), hx[r].p);
+        hx[r].q = fma2(nkap2, sub2(eb.q, e[r].q), hx[r].q);
       }
       if (XP) {
-        float p[4] = {0.f, 0.f, 0.f, 0.f};
-        if (xl) lds4a(c.phx_() + r * kRegW, p);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const float d = FS(en[q], e[r][q]);
-          p[q] = FF(xb[q], p[q], FM(xc[q], d));
-          hy[r][q] = FF(Db, p[q], FF(xk[q], d, hy[r][q]));
-        }
-        if (xl) st4a(c.phx_() + r * kRegW, p);
+        P2 p = ld2(c.phx_() + r * kRegW);
+        const u64 dp = sub2(e[r].q, e[r].p), dq = sub2(enq, e[r].q);
+        p.p = fma2(xb.p, p.p, mul2(xc.p, dp)); p.q = fma2(xb.q, p.q, mul2(xc.q, dq));
+        hy[r].p = fma2(Db2, p.p, fma2(xk.p, dp, hy[r].p)); hy[r].q = fma2(Db2, p.q, fma2(xk.q, dq, hy[r].q));
+        st2(c.phx_() + r * kRegW, p);
       } else {
-#pragma unroll
-        for (int q = 0; q < 4; ++q) hy[r][q] = FF(kap, FS(en[q], e[r][q]), hy[r][q]);
+        hy[r].p = fma2(kap2, sub2(e[r].q, e[r].p), hy[r].p);
+        hy[r].q = fma2(kap2, sub2(enq, e[r].q), hy[r].q);
       }
     }
-    st4a(c.xh_() + (c.w + 1) * kRegW + c.l4, hx[R - 1]);
+    st2(c.xh_() + (c.w + 1) * kRegW + c.l4, hx[R - 1]);
     __syncthreads();
 
     // ---- stages 4-7: E update + E CPML, source, save wavefield --------------------------------------
-    if (XP) { xk[0] = xk[1] = xk[2] = xk[3] = 1.f; }
-    if (xl) { lds4a(c.tabx_() + 3 * kRegW + c.l4, xb); lds4a(c.tabx_() + 4 * kRegW + c.l4, xc); lds4a(c.tabx_() + 5 * kRegW + c.l4, xk); }
+    if (XP) { xb = ld2(c.tabx_() + 3 * kRegW + c.l4); xc = ld2(c.tabx_() + 4 * kRegW + c.l4); xk = ld2(c.tabx_() + 5 * kRegW + c.l4); }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      float ha[4];                                      // Hx of the row above
-      if (r > 0) { ha[0] = hx[r - 1][0]; ha[1] = hx[r - 1][1]; ha[2] = hx[r - 1][2]; ha[3] = hx[r - 1][3]; }
-      else lds4a(c.xh_() + c.w * kRegW + c.l4, ha);
-      const float hl[4] = {__shfl_up_sync(full, hy[r][3], 1), hy[r][0], hy[r][1], hy[r][2]};  // Hy to the left
+      const P2 ha = (r > 0) ? hx[r - 1] : ld2(c.xh_() + c.w * kRegW + c.l4);              // Hx of the row above
+      // Hy to the left of (c0, c2) is (c3 of the previous lane, c1); to the left of (c1, c3) it is P itself
+      const u64 hlp = pk(__shfl_up_sync(full, hi2(hy[r].q), 1), lo2(hy[r].q));
+      const u64 txp = sub2(hy[r].p, hlp), txq = sub2(hy[r].q, hy[r].p);
+      const u64 tzp = sub2(hx[r].p, ha.p), tzq = sub2(hx[r].q, ha.q);
       if (ZP || XP) {
-        float pz[4], px[4] = {0.f, 0.f, 0.f, 0.f};
-        float bz = 0.f, cz = 0.f, kz = 1.f;
+        P2 pz = zero2(), px = zero2();
+        u64 bz = 0ULL, cz = 0ULL, kz = 0ULL;
         if (ZP) {
-          lds4a(c.pez_() + r * kRegW, pz);
-          bz = c.tabz_()[3 * L::ROWS + c.lr0 + r]; cz = c.tabz_()[4 * L::ROWS + c.lr0 + r]; kz = c.tabz_()[5 * L::ROWS + c.lr0 + r];
+          pz = ld2(c.pez_() + r * kRegW);
+          bz = bc2(c.tabz_()[3 * L::ROWS + c.lr0 + r]); cz = bc2(c.tabz_()[4 * L::ROWS + c.lr0 + r]); kz = bc2(c.tabz_()[5 * L::ROWS + c.lr0 + r]);
+          pz.p = fma2(bz, pz.p, mul2(cz, tzp)); pz.q = fma2(bz, pz.q, mul2(cz, tzq));
         }
-        if (xl) lds4a(c.pex_() + r * kRegW, px);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const float tx = FS(hy[r][q], hl[q]), tz = FS(hx[r][q], ha[q]);
-          float dd, pp;                                 // (tx/kx - tz/kz) and (psix - psiz)
-          if (ZP) pz[q] = FF(bz, pz[q], FM(cz, tz));
-          if (XP) px[q] = FF(xb[q], px[q], FM(xc[q], tx));
-          if (ZP && XP) { dd = FF(tx, xk[q], -FM(tz, kz)); pp = FS(px[q], pz[q]); }
-          else if (ZP)  { dd = FS(tx, FM(tz, kz));         pp = -pz[q]; }
-          else          { dd = FF(tx, xk[q], -tz);         pp = px[q]; }
-          e[r][q] = FF(cb[r][q], FF(dd, rdx, pp), FM(ca[r][q], e[r][q]));
+        if (XP) {
+          px = ld2(c.pex_() + r * kRegW);
+          px.p = fma2(xb.p, px.p, mul2(xc.p, txp)); px.q = fma2(xb.q, px.q, mul2(xc.q, txq));
         }
-        if (ZP) st4a(c.pez_() + r * kRegW, pz);
-        if (xl) st4a(c.pex_() + r * kRegW, px);
+        u64 ddp, ddq, ppp, ppq;                         // (tx/kx - tz/kz) and (psix - psiz)
+        if (ZP && XP) {
+          ddp = fma2(txp, xk.p, neg2(mul2(tzp, kz))); ddq = fma2(txq, xk.q, neg2(mul2(tzq, kz)));
+          ppp = sub2(px.p, pz.p); ppq = sub2(px.q, pz.q);
+        } else if (ZP) {
+          ddp = sub2(txp, mul2(tzp, kz)); ddq = sub2(txq, mul2(tzq, kz));
+          ppp = neg2(pz.p); ppq = neg2(pz.q);
+        } else {
+          ddp = fma2(txp, xk.p, neg2(tzp)); ddq = fma2(txq, xk.q, neg2(tzq));
+          ppp = px.p; ppq = px.q;
+        }
+        e[r].p = fma2(cb[r].p, fma2(ddp, rdx2, ppp), mul2(ca[r].p, e[r].p));
+        e[r].q = fma2(cb[r].q, fma2(ddq, rdx2, ppq), mul2(ca[r].q, e[r].q));
+        if (ZP) st2(c.pez_() + r * kRegW, pz);
+        if (XP) st2(c.pex_() + r * kRegW, px);
       } else {
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-          e[r][q] = FF(cb[r][q], FM(FS(FS(hy[r][q], hl[q]), FS(hx[r][q], ha[q])), rdx), FM(ca[r][q], e[r][q]));
+        e[r].p = fma2(cb[r].p, mul2(sub2(txp, tzp), rdx2), mul2(ca[r].p, e[r].p));
+        e[r].q = fma2(cb[r].q, mul2(sub2(txq, tzq), rdx2), mul2(ca[r].q, e[r].q));
       }
     }
     if (src_r >= 0) {                                   // every CTA whose region holds the source injects
@@ -150,25 +148,30 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
       for (int k = 1; k < kMaxT; ++k) wn = t == k ? wv[k] : wn;
 #pragma unroll
       for (int r = 0; r < R; ++r)
+        if (r == src_r) {                               // src_c: 0 -> P.lo, 1 -> Q.lo, 2 -> P.hi, 3 -> Q.hi
+          float v[4] = {lo2(e[r].p), lo2(e[r].q), hi2(e[r].p), hi2(e[r].q)};
+          const float k4[4] = {lo2(cb[r].p), lo2(cb[r].q), hi2(cb[r].p), hi2(cb[r].q)};
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-          if (r == src_r && q == src_c) e[r][q] = FF(-cb[r][q], wn, e[r][q]);
+          for (int q = 0; q < 4; ++q)
+            if (q == src_c) v[q] = FF(-k4[q], wn, v[q]);
+          e[r].p = pk(v[0], v[2]); e[r].q = pk(v[1], v[3]);
+        }
     }
     float* ez_out = (t + 1 == a.nsub) ? a.out.ez : a.ez_hist[t + 1];
     if (ez_out) {
       float* dst = ez_out + hoff;
 #pragma unroll
       for (int r = 0; r < R; ++r) {
-        if ((c.own >> r) & 1u) st4a(dst, e[r]);
+        if ((c.own >> r) & 1u) st2(dst, e[r]);
         dst += g.pitch;
       }
     }
     if (rflags) {
 #pragma unroll
       for (int r = 0; r < R; ++r)
-        if ((rflags >> r) & 1u) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
+        if ((rflags >> r) & 1u) st2(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
     }
-    st4a(c.xe_() + c.w * kRegW + c.l4, e[0]);
+    st2(c.xe_() + c.w * kRegW + c.l4, e[0]);
     __syncthreads();
   }
 }
@@ -217,14 +220,14 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
   if (tid < 7) c.meta_()[tid] = fwd_meta_word(a, s0, tile, ntile, tid);
   c.template stage_tables<true>(g);
   c.zero_psi(g);
-  float ca[R][4], cb[R][4];
+  P2 ca[R], cb[R];
 #pragma unroll
   for (int r = 0; r < R; ++r) {
-    zero4(ca[r]); zero4(cb[r]);
+    ca[r] = zero2(); cb[r] = zero2();
     if (c.colin && ((c.rin >> r) & 1u)) {
       const long long o = (long long)(c.gj0 + r) * g.pitch + c.gi;
-      ldg4a(a.ca + o, ca[r]);
-      ldg4a(a.cb + o, cb[r]);
+      ca[r] = ldg2(a.ca + o);
+      cb[r] = ldg2(a.cb + o);
     }
   }
   pdl_wait();
@@ -249,23 +252,23 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
       if (dj >= 0 && dj < R && di >= 0 && di < 4) { src_r = dj; src_c = di; }
     }
     // ---- this shot's fields have landed in the thread's slots: move them to registers ---------------
-    float e[R][4], hx[R][4], hy[R][4];
+    P2 e[R], hx[R], hy[R];
     c.fetch_psi(g, a.in, s);           // (the previous shot's psi went out in its store_psi)
     cp_async_wait<1>();                // fields: landed; psi: on its way
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      zero4(e[r]); zero4(hx[r]); zero4(hy[r]);
+      e[r] = zero2(); hx[r] = zero2(); hy[r] = zero2();
       if (c.colin && ((c.rin >> r) & 1u)) {
-        lds4a(c.hist_() + 0 * L::ROWS * kRegW + r * kRegW, e[r]);
-        lds4a(c.hist_() + 1 * L::ROWS * kRegW + r * kRegW, hx[r]);
-        lds4a(c.hist_() + 2 * L::ROWS * kRegW + r * kRegW, hy[r]);
+        e[r] = ld2(c.hist_() + 0 * L::ROWS * kRegW + r * kRegW);
+        hx[r] = ld2(c.hist_() + 1 * L::ROWS * kRegW + r * kRegW);
+        hy[r] = ld2(c.hist_() + 2 * L::ROWS * kRegW + r * kRegW);
       }
     }
     if (tid < 2) c.mask_()[tid] = 0u;
     // publish: row 0 for the warp above, all rows for the first trace sample
-    st4a(c.xe_() + c.w * kRegW + c.l4, e[0]);
+    st2(c.xe_() + c.w * kRegW + c.l4, e[0]);
 #pragma unroll
-    for (int r = 0; r < R; ++r) st4a(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
+    for (int r = 0; r < R; ++r) st2(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
     // ---- next shot: fields into the (now free) landing slots, scalars into the other meta slot ------
     if (s + 1 >= s1) cp_async_commit();   // (keeps the group count uniform: psi is always the second newest)
     if (s + 1 < s1) {
@@ -297,8 +300,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
     for (int r = 0; r < R; ++r) {
       if (!((c.own >> r) & 1u)) continue;
       const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-      st4a(a.out.hx + o, hx[r]);
-      st4a(a.out.hy + o, hy[r]);
+      st2(a.out.hx + o, hx[r]);
+      st2(a.out.hy + o, hy[r]);
     }
     if (c.zp || c.xp) c.store_psi(g, a.out, s);
   }

@@ -43,8 +43,8 @@ __global__ void coef_kernel(const float* __restrict__ eps_r, const float* __rest
   // kernels then keep those nodes at zero without any bounds test
   if (i >= 1 && i <= nx - 2 && j >= 1 && j <= nz - 2)
     coef_cell(eps_r[(long long)j * upitch + i], sigma[(long long)j * upitch + i], rdt, a, b);
-  ca[(long long)j * pitch + i] = a;
-  cb[(long long)j * pitch + i] = b;
+  ca[(long long)j * pitch + col_pos(i)] = a;          // internal column order: gprfwi_common.cuh
+  cb[(long long)j * pitch + col_pos(i)] = b;
 }
 
 __global__ void grad_finalize_kernel(const float* __restrict__ eps_r, const float* __restrict__ sigma, int upitch,
@@ -57,8 +57,8 @@ __global__ void grad_finalize_kernel(const float* __restrict__ eps_r, const floa
   if (i >= nx || j >= nz) return;
   float sa = 0.f, sb = 0.f;
   for (int g = 0; g < ngroups; ++g) {
-    sa += gca[g * plane + (long long)j * pitch + i];
-    sb += gcb[g * plane + (long long)j * pitch + i];
+    sa += gca[g * plane + (long long)j * pitch + col_pos(i)];      // internal column order
+    sb += gcb[g * plane + (long long)j * pitch + col_pos(i)];
   }
   float ge = 0.f, gs = 0.f;                                  // the PEC ring does not depend on the model
   if (i >= 1 && i <= nx - 2 && j >= 1 && j <= nz - 2)

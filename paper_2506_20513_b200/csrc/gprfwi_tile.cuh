@@ -57,6 +57,34 @@ __device__ __forceinline__ float FS(float a, float b) { return __fsub_rn(a, b); 
 __device__ __forceinline__ float FA(float a, float b) { return __fadd_rn(a, b); }
 __device__ __forceinline__ float FF(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 
+// ---- packed pairs of fp32 (sm_100: one FFMA2 / FADD2 / FMUL2 does two IEEE-rounded operations in one
+// issue slot; the kernels are issue-bound, not FP-pipe-bound).  A float4 unit of a row is held as
+// P = (c0, c2), Q = (c1, c3): see gprfwi_common.cuh.
+typedef unsigned long long u64;
+struct P2 { u64 p, q; };
+__device__ __forceinline__ u64 pk(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float lo2(u64 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
+__device__ __forceinline__ float hi2(u64 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
+__device__ __forceinline__ u64 bc2(float v) { return pk(v, v); }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 neg2(u64 a) { return a ^ 0x8000000080000000ULL; }
+__device__ __forceinline__ P2 zero2() { P2 v; v.p = 0ULL; v.q = 0ULL; return v; }
+__device__ __forceinline__ P2 ldg2(const float* p)          // read-only global, 128 bit
+{
+  const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2*>(p));
+  P2 r; r.p = v.x; r.q = v.y; return r;
+}
+__device__ __forceinline__ P2 ld2(const float* p)           // shared / generic, 128 bit
+{
+  const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(p);
+  P2 r; r.p = v.x; r.q = v.y; return r;
+}
+__device__ __forceinline__ void st2(float* p, P2 v) { *reinterpret_cast<ulonglong2*>(p) = make_ulonglong2(v.p, v.q); }
+__device__ __forceinline__ void stcs2(float* p, P2 v) { __stcs(reinterpret_cast<ulonglong2*>(p), make_ulonglong2(v.p, v.q)); }
+
 __device__ __forceinline__ void ldg4a(const float* p, float* o)
 {
   const float4 v = __ldg(reinterpret_cast<const float4*>(p));
@@ -166,12 +194,12 @@ struct TileCtx {
       for (int c = 0; c < 4; ++c) {
         const int i = gi + c;
         const bool in = i >= 0 && i < g.nx;
-        tabx_()[0 * kRegW + l4 + c] = in ? g.thx[i] : 0.f;
-        tabx_()[1 * kRegW + l4 + c] = in ? g.thx[r1 * g.nx + i] : 0.f;
-        tabx_()[2 * kRegW + l4 + c] = in ? g.thx[r2h * g.nx + i] : k0;
-        tabx_()[3 * kRegW + l4 + c] = in ? g.tex[i] : 0.f;
-        tabx_()[4 * kRegW + l4 + c] = in ? g.tex[r1 * g.nx + i] : 0.f;
-        tabx_()[5 * kRegW + l4 + c] = in ? g.tex[2 * g.nx + i] : 1.f;
+        tabx_()[0 * kRegW + l4 + unit_perm(c)] = in ? g.thx[i] : 0.f;
+        tabx_()[1 * kRegW + l4 + unit_perm(c)] = in ? g.thx[r1 * g.nx + i] : 0.f;
+        tabx_()[2 * kRegW + l4 + unit_perm(c)] = in ? g.thx[r2h * g.nx + i] : k0;
+        tabx_()[3 * kRegW + l4 + unit_perm(c)] = in ? g.tex[i] : 0.f;
+        tabx_()[4 * kRegW + l4 + unit_perm(c)] = in ? g.tex[r1 * g.nx + i] : 0.f;
+        tabx_()[5 * kRegW + l4 + unit_perm(c)] = in ? g.tex[2 * g.nx + i] : 1.f;
       }
     }
     for (int k = threadIdx.x; k < L::ROWS; k += L::THREADS) {
