@@ -30,6 +30,13 @@
 
 namespace gprfwi {
 
+// Offset (floats) of the thread-private landing / psi arrays from a 128-byte boundary.  Measured on
+// config 2 (B200): odd multiples of 4 floats (16 B) give 256-257 Gcell-updates/s, multiples of 8 floats
+// (32 B, including the "natural" 128-byte alignment) 248-250 -- the cp.async landing rows and the
+// exchange rows then collide in the shared-memory pipe.  28 was the best of 0, 4, ..., 28.
+#ifndef GPRFWI_SMEM_PAD
+#define GPRFWI_SMEM_PAD 28
+#endif
 constexpr int kMaxT = 4;       // fused steps per launch <= x halo (4 columns = one float4)
 constexpr int kRegW = 128;     // region width  = 32 lanes x float4
 constexpr int kOwnW = 120;     // owned width   = lanes 1..30
@@ -45,7 +52,7 @@ struct RegTile {
   static constexpr int TABZ = TABX + 6 * kRegW;
   static constexpr int MASK = TABZ + 6 * ROWS;                 // 2 words: rows of the region that hold receivers
   static constexpr int META = MASK + 2;                        // 2 x 8 words: per-shot scalars, fetched one shot ahead
-  static constexpr int HIST = (META + 16 + 3) / 4 * 4;
+  static constexpr int HIST = (META + 16 + 31) / 32 * 32 + GPRFWI_SMEM_PAD;
   static constexpr int PSI = HIST + NH * ROWS * kRegW;
   GPR_HD static size_t smem_bytes(bool pml) { return sizeof(float) * (size_t)(PSI + (pml ? 4 * ROWS * kRegW : 0)); }
 };
