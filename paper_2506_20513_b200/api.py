@@ -190,3 +190,35 @@ class Simulation:
             self.close()
         except Exception:
             pass
+
+
+def invert(sim: "Simulation", eps_r: torch.Tensor, sigma: torch.Tensor, d_obs: torch.Tensor, *, iterations: int,
+           lr_eps_r: float, lr_sigma: float, mask_rows: int = 0, tv_iters: int = 10, tv_lambda: float = 0.01,
+           tv_alpha: float = 1.0, eps_r_min: float = 1.0, sigma_min: float = 0.0, callback=None):
+    """The paper's inversion loop as a sequence of C-ABI calls, nothing computed here:
+    per iteration gprfwi_forward -> gprfwi_residual (+ misfit) -> gprfwi_adjoint -> gprfwi_update
+    (TV term, source mask, Adam with one learning rate per parameter, clamps).  `eps_r` and `sigma`
+    are updated in place; returns the list of misfits 0.5*||d_syn - d_obs||^2 (one per iteration,
+    evaluated BEFORE that iteration's update)."""
+    p = sim.p
+    if p.pitch != p.nx:
+        raise ValueError("invert() expects unpadded models (pitch == nx)")
+    dev = sim.device
+    res = torch.empty_like(d_obs)
+    misfit = torch.zeros(1, dtype=torch.float64, device=dev)
+    state = [torch.zeros_like(eps_r) for _ in range(4)]
+    ws = torch.empty(gprfwi_update_workspace_bytes(p.nz, p.pitch), dtype=torch.uint8, device=dev)
+    history = []
+    for it in range(1, iterations + 1):
+        traces = sim.forward(eps_r, sigma)
+        misfit.zero_()
+        gprfwi_residual(traces, d_obs, res, misfit)
+        ge, gs = sim.adjoint(res)
+        u = make_update_params(step=it, lr_eps_r=lr_eps_r, lr_sigma=lr_sigma, tv_iters=tv_iters,
+                               tv_lambda=tv_lambda, tv_alpha=tv_alpha, mask_rows=mask_rows,
+                               eps_r_min=eps_r_min, sigma_min=sigma_min)
+        gprfwi_update(p.nz, p.nx, p.pitch, u, eps_r, sigma, ge, gs, state[0], state[1], state[2], state[3], ws)
+        history.append(float(misfit.item()))
+        if callback is not None:
+            callback(it, history[-1])
+    return history
