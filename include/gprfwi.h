@@ -166,6 +166,15 @@ int gprfwi_update(int32_t nz, int32_t nx, int32_t pitch, const gprfwi_update_par
                   float* m_eps_r, float* v_eps_r, float* m_sigma, float* v_sigma,
                   void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Multiscale (frequency-staged) inversion: zero-phase FIR along time applied to
+ * traces or wavelets before a low-frequency stage.
+ *   in, out  device [nseries][nt][nrec] (nrec = 1 for wavelets), out != in
+ *   taps     device [ntaps], ntaps odd; out[n] = sum_k taps[k] in[n + k - (ntaps-1)/2], zero outside [0, nt)
+ * The filter design (cut-off, window) is the caller's: any symmetric taps give zero phase.
+ * Errors: EINVAL (null pointer, in == out, nt/nrec/nseries < 1, ntaps even or < 1), ECUDA. */
+int gprfwi_lowpass(const float* in, float* out, int32_t nseries, int32_t nt, int32_t nrec,
+                   const float* taps, int32_t ntaps, void* cuda_stream);
+
 /* Number of kernel launches enqueued by the last forward / adjoint on this handle. */
 int64_t gprfwi_launch_count(const gprfwi_handle* h);
 

@@ -68,3 +68,20 @@ def update(eps_r, sigma, g_eps, g_sig, state, step, lr_eps, lr_sig, beta1=0.9, b
         out[name] = (xn, g)
         state["m_" + name], state["v_" + name] = m, v
     return out["eps"][0], out["sig"][0], out["eps"][1], out["sig"][1]
+
+
+def lowpass(x, taps):
+    """Zero-phase FIR along axis 1 of x[nseries][nt][...] (multiscale stages):
+    out[n] = sum_k taps[k] x[n + k - (ntaps-1)/2], zero outside.  Pin: equals np.convolve(..., 'same')
+    for symmetric taps; a constant series keeps its value away from the ends when sum(taps) = 1."""
+    x = np.asarray(x, dtype=np.float64)
+    taps = np.asarray(taps, dtype=np.float64)
+    half = (len(taps) - 1) // 2
+    out = np.zeros_like(x)
+    nt = x.shape[1]
+    for k, h in enumerate(taps):
+        sh = k - half
+        lo, hi = max(0, -sh), min(nt, nt - sh)
+        if lo < hi:                                   # (taps may be longer than the series)
+            out[:, lo:hi] += h * x[:, lo + sh:hi + sh]
+    return out

@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "OK", -1: "EINVAL", -2: "ECFL", -3: "EGEOM", -4: "ENOMEM", -5
 EXPORTS = (
     "gprfwi_workspace_bytes", "gprfwi_forward", "gprfwi_adjoint", "gprfwi_gradient_host",
     "gprfwi_workspace_bytes_host", "gprfwi_residual", "gprfwi_launch_count", "gprfwi_get_plan",
-    "gprfwi_release", "gprfwi_strerror", "gprfwi_version", "gprfwi_update", "gprfwi_update_workspace_bytes",
+    "gprfwi_release", "gprfwi_strerror", "gprfwi_version", "gprfwi_update", "gprfwi_update_workspace_bytes", "gprfwi_lowpass",
 )
 
 
@@ -95,6 +95,8 @@ def _declare(lib):
     lib.gprfwi_update.restype = ctypes.c_int
     lib.gprfwi_update.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(UpdateParams),
                                   fp, fp, fp, fp, fp, fp, fp, fp, vp, sz, vp]
+    lib.gprfwi_lowpass.restype = ctypes.c_int
+    lib.gprfwi_lowpass.argtypes = [fp, fp, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, fp, ctypes.c_int32, vp]
     lib.gprfwi_version.restype = ctypes.c_int
     return lib
 

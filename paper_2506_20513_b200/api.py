@@ -149,6 +149,26 @@ def gprfwi_update(nz, nx, pitch, u: UpdateParams, eps_r, sigma, grad_eps_r, grad
                                     workspace.numel(), _stream_ptr(stream)))
 
 
+def gprfwi_lowpass(x: torch.Tensor, out: torch.Tensor, taps: torch.Tensor, stream=None):
+    """Zero-phase FIR along time of x[nseries][nt][nrec] (or [nseries][nt]) into `out` (multiscale stages)."""
+    if x.dim() == 2:
+        nseries, nt, nrec = x.shape[0], x.shape[1], 1
+    else:
+        nseries, nt, nrec = x.shape
+    check(_lib.load().gprfwi_lowpass(_dev(x, "x"), _dev(out, "out", x.numel()), int(nseries), int(nt), int(nrec),
+                                     _dev(taps, "taps"), int(taps.numel()), _stream_ptr(stream)))
+    return out
+
+
+def lowpass_taps(dt: float, f_cut: float, ntaps: int = 0) -> np.ndarray:
+    """Hamming-windowed sinc, unit DC gain (harness-side filter design; the ABI takes any taps)."""
+    if ntaps <= 0:
+        ntaps = int(4.0 / (f_cut * dt)) | 1
+    k = np.arange(ntaps) - (ntaps - 1) / 2
+    h = np.sinc(2.0 * f_cut * dt * k) * np.hamming(ntaps)
+    return (h / h.sum()).astype(np.float32)
+
+
 class Simulation:
     """Owns the device buffers (torch) and the library handle for one problem."""
 

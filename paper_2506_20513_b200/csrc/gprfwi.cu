@@ -967,4 +967,16 @@ int gprfwi_update(int32_t nz, int32_t nx, int32_t pitch, const gprfwi_update_par
   return GPRFWI_OK;
 }
 
+int gprfwi_lowpass(const float* in, float* out, int32_t nseries, int32_t nt, int32_t nrec, const float* taps,
+                   int32_t ntaps, void* cuda_stream)
+{
+  if (!in || !out || !taps || in == out) return GPRFWI_EINVAL;
+  if (nseries < 1 || nt < 1 || nrec < 1 || ntaps < 1 || (ntaps & 1) == 0) return GPRFWI_EINVAL;
+  const long long n = (long long)nt * nrec;
+  dim3 grid((unsigned)std::min<long long>((n + 255) / 256, 4 * 148), (unsigned)nseries);
+  GPR_LAUNCH(lowpass_kernel, grid, dim3(256), (cudaStream_t)cuda_stream, in, out, nt, nrec, taps, ntaps);
+  GPR_CUDA(cudaGetLastError());
+  return GPRFWI_OK;
+}
+
 }  // extern "C"

@@ -99,6 +99,26 @@ __global__ void adam_kernel(int nz, int nx, int pitch, int mask_rows, float lr, 
   const float xn = x[o] - lr * (mn * c1) / (sqrtf(vn * c2) + eps);        // c1 = 1/(1-b1^t), c2 = 1/(1-b2^t)
   x[o] = fmaxf(xn, xmin);
 }
+
+// Zero-phase FIR along time for the multiscale (frequency-staged) strategy, PAPER.md:529-531:
+// out[s][n][r] = sum_k taps[k] * in[s][n + k - (ntaps-1)/2][r], samples outside [0, nt) taken as 0.
+// Thread = one (n, r) of one shot; r fastest, so reads and writes are coalesced along receivers.
+__global__ void lowpass_kernel(const float* __restrict__ in, float* __restrict__ out, int nt, int nrec,
+                               const float* __restrict__ taps, int ntaps)
+{
+  const long long base = (long long)blockIdx.y * nt * nrec;
+  const int half = (ntaps - 1) / 2;
+  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < (long long)nt * nrec;
+       k += (long long)gridDim.x * blockDim.x) {
+    const int n = (int)(k / nrec), r = (int)(k % nrec);
+    float acc = 0.f;
+    for (int q = 0; q < ntaps; ++q) {
+      const int m = n + q - half;
+      if (m >= 0 && m < nt) acc = fmaf(taps[q], in[base + (long long)m * nrec + r], acc);
+    }
+    out[base + k] = acc;
+  }
+}
 #endif
 
 }  // namespace gprfwi

@@ -363,3 +363,21 @@ def test_inversion_loop_reduces_misfit_and_recovers_anomaly():
     d = eps.cpu().numpy() - wl.eps_r
     assert np.all(d[:wl.npml + 8] == 0.0) and np.abs(d[wl.npml + 8:]).max() > 0.0
     assert eps.min().item() >= 1.0 and torch.equal(sig.cpu(), torch.as_tensor(wl.sigma))      # lr_sigma = 0
+
+
+def test_lowpass_matches_oracle():
+    """Multiscale stage filter: zero-phase FIR along time of traces and of a wavelet."""
+    from oracle import epilogue as ep
+    from paper_2506_20513_b200 import gprfwi_lowpass, lowpass_taps
+    rng = np.random.default_rng(4)
+    x = rng.standard_normal((3, 517, 11)).astype(np.float32)
+    taps = lowpass_taps(2e-11, 150e6)
+    assert len(taps) % 2 == 1
+    d_x = torch.as_tensor(x, device=dev()); d_t = torch.as_tensor(taps, device=dev())
+    y = gprfwi_lowpass(d_x, torch.empty_like(d_x), d_t).cpu().numpy()
+    assert rel_l2(y, ep.lowpass(x, taps)) <= 1e-6
+    w = gi.ricker(800, 2e-11, 400e6)[None, :]
+    d_w = torch.as_tensor(w, device=dev())
+    yw = gprfwi_lowpass(d_w, torch.empty_like(d_w), d_t).cpu().numpy()
+    assert rel_l2(yw, ep.lowpass(w[:, :, None], taps)[:, :, 0]) <= 1e-6
+    assert np.abs(np.fft.rfft(yw[0]))[60:].max() < 0.2 * np.abs(np.fft.rfft(w[0])).max()      # highs are gone

@@ -408,3 +408,16 @@ def test_golden_config1_oracle_values_unchanged():
                 continue
             k, v = line.rsplit(" ", 1)
             assert abs(now[k] - float(v)) <= 1e-9 * max(abs(float(v)), 1e-30), k
+
+
+def test_lowpass_oracle_equals_numpy_convolve():
+    from oracle import epilogue as ep
+    rng = np.random.default_rng(1)
+    x = rng.standard_normal((2, 200, 3))
+    k = np.arange(31) - 15
+    taps = np.sinc(0.2 * k) * np.hamming(31); taps /= taps.sum()
+    y = ep.lowpass(x, taps)
+    for s in range(2):
+        for r in range(3):
+            assert np.allclose(y[s, :, r], np.convolve(x[s, :, r], taps, mode="same"), atol=1e-13)
+    assert np.allclose(ep.lowpass(np.ones((1, 100, 1)), taps)[0, 20:80, 0], 1.0, atol=1e-13)
