@@ -401,3 +401,27 @@ def test_random_shapes_fuzz():
             continue
         tr, ge, gs, _ = run_gpu(wl, res, checkpoint_stride=min(K, nt))
         assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o), f" fuzz {case}: {nz}x{nx} npml {npml} nt {nt} S {S} R {R} K {K}")
+
+
+def test_config3_full_launch_configuration_properties():
+    """Config 3 exactly as bench.py launches it (60 shots, nt = 4000, checkpoint-and-recompute chosen by
+    the plan): shot 0's traces against the oracle, shots 0 and 59 bit-identical to a two-shot run, and
+    the full-batch gradient equal to the sum of the gradients of the two half batches."""
+    wl = gi.config3()
+    free, _ = torch.cuda.mem_get_info(dev())
+    budget = int(free * 0.9)
+    res = gi.random_residual(wl, 1.0, seed=5)
+    tr, ge, gs, plan = run_gpu(wl, res, budget=budget)
+    assert plan["full_history"] == 0
+    one = wl.subset([0])
+    tr_o = oracle.forward(problem(one), one.eps_r, one.sigma)["traces"]
+    assert rel_l2(tr[:1], tr_o) <= TOL_TRACE
+    sub = wl.subset([0, 59])
+    t2, _, _, _ = run_gpu(sub, budget=budget)
+    assert np.array_equal(t2, tr[[0, 59]])
+    ga, gb = np.zeros_like(ge, dtype=np.float64), np.zeros_like(gs, dtype=np.float64)
+    for lo, hi in ((0, 30), (30, 60)):
+        half = wl.subset(list(range(lo, hi)))
+        _, a, b, _ = run_gpu(half, res[lo:hi], budget=budget)
+        ga += a; gb += b
+    assert rel_l2(ge, ga) <= 1e-5 and rel_l2(gs, gb) <= 1e-5
