@@ -322,7 +322,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         oracle.build()
-        shots = sorted({(k * wl.nshots) // 6 for k in range(6)}) if args.config <= 2 else [0]
+        shots = sorted({(k * wl.nshots) // 8 for k in range(8)}) if args.config <= 2 else [0]
         sub = wl if args.config <= 2 else wl.subset(list(range(wl.nshots)), nt=min(wl.nt, 400))
         secs, w = oracle_sample(sub, shots)
         cpu = {"value": w / secs / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
