@@ -106,6 +106,32 @@ def line_geometry(nz_int: int, nx_int: int, npml: int, nshots: int, nrec: int, d
     return src, rec
 
 
+def acquisition(src0_zx, src_step_zx, steps: int, rec0_zx, rec_step_zx, nrx: int,
+                fixed_receiver: bool = False):
+    """Acquisition of PAPER.md:184-199 (Table 1: source_location, source_step, step, receiver_location,
+    receiver_step, nrx, Fixedreceiver) in grid cells.  Shot k fires at src0 + k*src_step; its receivers
+    sit at rec0 + j*rec_step (j < nrx), shifted by k*src_step as well unless `fixed_receiver`
+    (a moving source-receiver array; nrx = 1 gives a common-offset profile)."""
+    k = np.arange(steps, dtype=np.int64)[:, None]
+    j = np.arange(nrx, dtype=np.int64)[:, None]
+    src = np.asarray(src0_zx, dtype=np.int64)[None, :] + k * np.asarray(src_step_zx, dtype=np.int64)[None, :]
+    rec1 = np.asarray(rec0_zx, dtype=np.int64)[None, :] + j * np.asarray(rec_step_zx, dtype=np.int64)[None, :]
+    rec = np.broadcast_to(rec1, (steps, nrx, 2)).copy()
+    if not fixed_receiver:
+        rec += (src - src[:1])[:, None, :]
+    return src.astype(np.int32), rec.astype(np.int32)
+
+
+def with_geometry(wl: "Workload", src_zx, rec_zx, name: str | None = None) -> "Workload":
+    """Same models and wavelet, other acquisition (positions must lie inside the PEC ring)."""
+    src = np.ascontiguousarray(src_zx, dtype=np.int32)
+    rec = np.ascontiguousarray(rec_zx, dtype=np.int32)
+    assert src.ndim == 2 and rec.ndim == 3 and rec.shape[0] == src.shape[0]
+    for a, n in ((src[:, 0], wl.nz), (src[:, 1], wl.nx), (rec[..., 0], wl.nz), (rec[..., 1], wl.nx)):
+        assert a.min() >= 1 and a.max() <= n - 2, "position on or outside the PEC ring"
+    return replace(wl, name=name or wl.name + "+geometry", src_zx=src, rec_zx=rec)
+
+
 def _gauss2d(nz, nx, cz, cx, std):
     z = np.arange(nz, dtype=np.float64)[:, None]
     x = np.arange(nx, dtype=np.float64)[None, :]
@@ -217,6 +243,33 @@ def config4(nshots: int = 100, nrec: int = 400, nt: int = 6000) -> Workload:
     eps_o, sig_o = _inclusions(np.random.Generator(np.random.PCG64(seed + 1000)), nz, nx, eps0, sig0)
     return _finish("config4-high-frequency", eps, sig, eps_o, sig_o, npml, 0.005, 1e-11, nt, 1.2e9,
                    nshots, nrec, seed)
+
+
+def crosshole(nt: int = 1000, nrec: int = 200) -> Workload:
+    """Shapes of the paper's cross-hole experiment (section 4.1): 120 x 220 cells incl. a
+    10-cell CPML, dx = 0.05 m, dt = 1e-10 s, 1e-7 s window, one 100 MHz source in one hole and `nrec`
+    receivers down a line 5 m away.  The models are a seeded stand-in (three layers, three anomalies and
+    a thin channel with eps_r and sigma placed differently), not the paper's landfill model."""
+    seed = BASE_SEED + 6
+    npml, nz, nx = 10, 200, 100                      # interior; z is the long (depth) axis
+    rng = np.random.Generator(np.random.PCG64(seed))
+    layer = np.minimum(np.arange(nz) // 70, 2)[:, None] * np.ones((1, nx), dtype=np.int64)
+    eps = np.array([5.0, 8.0, 11.0])[layer]
+    sig = np.array([1e-3, 3e-3, 6e-3])[layer]
+    eps_o, sig_o = eps.copy(), sig.copy()
+    z = np.arange(nz)[:, None]; x = np.arange(nx)[None, :]
+    for k in range(3):
+        cz, cx, r = int(rng.integers(30, nz - 30)), int(rng.integers(30, nx - 30)), int(rng.integers(6, 12))
+        m = (z - cz) ** 2 + (x - cx) ** 2 <= r * r
+        eps_o = np.where(m, rng.uniform(3.0, 16.0), eps_o)
+        m2 = (z - cz - 8) ** 2 + (x - cx + 5) ** 2 <= r * r          # sigma anomaly displaced
+        sig_o = np.where(m2, float(np.exp(rng.uniform(np.log(5e-3), np.log(3e-2)))), sig_o)
+    chan = (np.abs(z - (60 + x // 3)) <= 1) & (x > 25) & (x < 80)
+    eps_o = np.where(chan, 14.0, eps_o); sig_o = np.where(chan, 2e-2, sig_o)
+    src, rec = acquisition((npml + 10, npml + 10), (0, 0), 1, (npml, npml + 89), (1, 0), min(nrec, nz),
+                           fixed_receiver=True)
+    return _finish("crosshole-4.1-shapes", eps, sig, eps_o, sig_o, npml, 0.05, 1e-10, nt, 100e6, 1, nrec,
+                   seed, geometry=(src, rec))
 
 
 def config5(n: int = 512, batch: int = 1, nt: int = 1000, nrec: int = 64) -> Workload:

@@ -6,6 +6,7 @@ entry points take NumPy arrays); nothing is computed here.
 from __future__ import annotations
 
 import ctypes
+from dataclasses import dataclass
 
 import numpy as np
 import torch
@@ -242,3 +243,42 @@ def invert(sim: "Simulation", eps_r: torch.Tensor, sigma: torch.Tensor, d_obs: t
         if callback is not None:
             callback(it, history[-1])
     return history
+
+
+@dataclass
+class Stage:
+    """One stage of a staged inversion: the two-stage learning-rate strategy of PAPER.md:547 (eps_r first,
+    then both: set lr_sigma = 0 in the first stage) and / or one band of the multiscale strategy of
+    PAPER.md:529-531 (`f_cut` = low-pass corner in Hz applied to the wavelet and the observed data;
+    None = full band)."""
+    iterations: int
+    lr_eps_r: float
+    lr_sigma: float
+    f_cut: float | None = None
+    ntaps: int = 0
+
+
+def invert_staged(sim: "Simulation", eps_r: torch.Tensor, sigma: torch.Tensor, d_obs: torch.Tensor, stages,
+                  callback=None, **update_kw):
+    """Stage driver (reading R21): per stage, low-pass the source wavelet and
+    d_obs with gprfwi_lowpass when the stage has a corner frequency, then run invert() with the stage's
+    learning rates.  Adam's moments and step counter restart at every stage; a parameter whose learning
+    rate is 0 does not move.  Returns one misfit list per stage; `callback(stage, iteration, misfit)`."""
+    full = sim.wavelet
+    dev = sim.device
+    out = []
+    try:
+        for k, st in enumerate(stages):
+            w, d = full, d_obs
+            if st.f_cut is not None:
+                taps = torch.as_tensor(lowpass_taps(sim.p.dt, st.f_cut, st.ntaps), device=dev)
+                w2 = full.reshape(-1, sim.p.nt)
+                w = gprfwi_lowpass(w2, torch.empty_like(w2), taps).reshape(full.shape)
+                d = gprfwi_lowpass(d_obs, torch.empty_like(d_obs), taps)
+            sim.wavelet = w
+            cb = None if callback is None else (lambda it, mf, k=k: callback(k, it, mf))
+            out.append(invert(sim, eps_r, sigma, d, iterations=st.iterations, lr_eps_r=st.lr_eps_r,
+                              lr_sigma=st.lr_sigma, callback=cb, **update_kw))
+    finally:
+        sim.wavelet = full
+    return out

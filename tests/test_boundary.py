@@ -99,3 +99,19 @@ def test_forced_stride(lib):
     wl = gi.config1(nt=100)
     nb, plan = gprfwi_workspace_bytes(params_of(wl, checkpoint_stride=7), 0)
     assert plan["full_history"] == 0 and plan["checkpoint_stride"] == 7
+
+
+def test_acquisition_presets_match_table_1_semantics():
+    """step / source_step / receiver_step / Fixedreceiver as integer-cell positions."""
+    import gpr_inputs as gi
+    src, rec = gi.acquisition((15, 20), (0, 4), 5, (15, 22), (0, 1), 3)
+    assert src.tolist() == [[15, 20 + 4 * k] for k in range(5)]
+    assert rec[:, :, 1].tolist() == [[22 + 4 * k + j for j in range(3)] for k in range(5)]      # array moves along
+    assert np.all(rec[:, :, 0] == 15)
+    _, rec_f = gi.acquisition((15, 20), (0, 4), 5, (15, 22), (0, 1), 3, fixed_receiver=True)
+    assert np.all(rec_f == rec[:1])
+    wl = gi.crosshole()
+    assert (wl.nz, wl.nx, wl.nshots, wl.nrec, wl.nt) == (220, 120, 1, 200, 1000)           # PAPER.md:547
+    assert np.all(np.diff(wl.rec_zx[0, :, 0]) == 1) and np.all(wl.rec_zx[0, :, 1] == wl.rec_zx[0, 0, 1])
+    with pytest.raises(AssertionError):
+        gi.with_geometry(wl, [[0, 5]], [[[5, 5]]])                                          # on the PEC ring

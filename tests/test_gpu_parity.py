@@ -383,6 +383,65 @@ def test_lowpass_matches_oracle():
     assert np.abs(np.fft.rfft(yw[0]))[60:].max() < 0.2 * np.abs(np.fft.rfft(w[0])).max()      # highs are gone
 
 
+def test_crosshole_and_moving_array_acquisitions():
+    """the acquisition variants of Table 1 are per-shot receiver lists.
+    Cross-hole shapes of section 4.1 (120 x 220 grid, one source, 200 receivers down the
+    other hole, so every tile row holds receivers), a moving source-receiver array, and a
+    common-offset profile (one receiver per shot)."""
+    wl = gi.crosshole(nt=700)
+    tr_o, res, ge_o, gs_o = oracle_all(wl, with_obs=True)
+    tr, ge, gs, _ = run_gpu(wl, res)
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
+    base = gi.small_random(nz=64, nx=170, nt=150, npml=8, nshots=1, nrec=1, seed=77)
+    for tag, (src, rec) in (("moving array", gi.acquisition((12, 14), (1, 23), 6, (12, 20), (0, 7), 5)),
+                            ("common offset", gi.acquisition((11, 12), (0, 15), 10, (11, 18), (0, 0), 1)),
+                            ("fixed receivers", gi.acquisition((50, 15), (-3, 28), 5, (10, 10), (2, 9), 16,
+                                                               fixed_receiver=True))):
+        wl2 = gi.with_geometry(base, src, rec, name="small-random " + tag)
+        tr_o, res, ge_o, gs_o = oracle_all(wl2)
+        tr, ge, gs, _ = run_gpu(wl2, res)
+        assert_parity(wl2, (tr, ge, gs), (tr_o, ge_o, gs_o))
+
+
+def test_staged_inversion_driver():
+    """SURVEY 8(f)-1/-2, reading R21: two-stage learning-rate strategy (eps_r only, then both) with a
+    low-passed first stage, on the cross-hole shapes.  Checked against the oracle where the result is
+    fixed: the first misfit of each stage equals the oracle's misfit at that stage's starting models
+    with that stage's (filtered) wavelet and data; sigma does not move while its rate is 0; the
+    filtered stage leaves the full-band wavelet in place afterwards; each stage lowers its misfit."""
+    from oracle import epilogue as ep
+    from paper_2506_20513_b200 import Stage, invert_staged, lowpass_taps
+    wl = gi.crosshole(nt=600)
+    pb = problem(wl)
+    d_obs64 = oracle.forward(pb, wl.eps_r_obs, wl.sigma_obs)["traces"]
+    d_obs = torch.as_tensor(d_obs64.astype(np.float32), device=dev())
+    sim = Simulation(params_of(wl), wl.src_zx, wl.rec_zx, wl.wavelet, dev())
+    eps = torch.as_tensor(wl.eps_r.copy(), device=dev()); sig = torch.as_tensor(wl.sigma.copy(), device=dev())
+    stages = [Stage(4, 0.05, 0.0, f_cut=80e6), Stage(4, 0.05, 2e-4)]
+    snap = {}
+
+    def cb(k, it, mf):
+        if it == stages[k].iterations:
+            snap[k] = (eps.cpu().numpy().copy(), sig.cpu().numpy().copy())
+
+    hist = invert_staged(sim, eps, sig, d_obs, stages, callback=cb, mask_rows=0, tv_iters=3, tv_lambda=0.002,
+                         tv_alpha=0.0)
+    assert torch.equal(sim.wavelet.cpu(), torch.as_tensor(wl.wavelet))
+    sim.close()
+    print("[staged]", [" ".join(f"{h:.3e}" for h in hs) for hs in hist])
+    assert [len(h) for h in hist] == [4, 4]
+    assert np.array_equal(snap[0][1], wl.sigma) and not np.array_equal(snap[0][0], wl.eps_r)
+    assert not np.array_equal(snap[1][1], wl.sigma)
+    assert hist[0][-1] < hist[0][0] and hist[1][-1] < hist[1][0]
+    taps = lowpass_taps(wl.dt, 80e6)
+    w_lp = ep.lowpass(wl.wavelet[None, :, None], taps)[0, :, 0]
+    d_lp = ep.lowpass(d_obs.cpu().numpy(), taps)
+    r0 = oracle.forward(problem(wl, wavelet=w_lp), wl.eps_r, wl.sigma)["traces"] - d_lp
+    assert abs(hist[0][0] - 0.5 * np.sum(r0 * r0)) <= 1e-3 * hist[0][0]
+    r1 = oracle.forward(pb, snap[0][0], snap[0][1])["traces"] - d_obs.cpu().numpy()
+    assert abs(hist[1][0] - 0.5 * np.sum(r1 * r1)) <= 1e-3 * hist[1][0]
+
+
 def test_random_shapes_fuzz():
     """Seeded random grids (ragged tiles, nx a multiple of the tile width or one past it, CPML
     thickness 0 / 3 / 4 / 7 / 10 / 13), shot counts, receiver counts and checkpoint strides against the
