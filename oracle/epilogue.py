@@ -9,8 +9,12 @@ definition of `*_tv_grad`; the reading below is the one both sides implement.
 Pins (tests/test_oracle_pins.py): Adam's first step equals -lr g/(|g| + eps) (closed form of
 Eqs. (14)-(15) at t = 1), masked rows do not move, clamps hold; shrink(v, t) = v max(1 - t/|v|, 0)
 (Eq. (17)); a constant X gives tv_grad = 0; the U update solves (I + rho D^T D) U = U0 + rho D^T (Z - B)
-in the limit of many sweeps (checked with one dense solve on a tiny grid).  Beyond those invariants
-the TV term is PARITY UNPINNED: the paper gives no value to compare with.
+in the limit of many sweeps (checked with one dense solve on a tiny grid); run to convergence the
+iteration reaches the minimiser of 1/2 |U - U0|^2 + lambda TV(U), checked against its closed form for a
+two-level periodic stripe along either axis (plateaus approach by 2 lambda / L, and merge at the mean
+for large lambda).  What the paper does not fix -- the constants, the scaling by max|X|, one Jacobi
+sweep per iteration, stopping after n_it iterations -- stays a reading (R20): at the default n_it the
+TV term is PARITY UNPINNED against the paper, which prints no value to compare with.
 """
 import numpy as np
 

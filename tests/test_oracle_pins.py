@@ -355,6 +355,29 @@ def test_epilogue_adam_first_step_closed_form_mask_and_clamp():
     assert np.allclose(xn2, xn - 0.05 * (mm / (1 - 0.81)) / (np.sqrt(vv / (1 - 0.999 ** 2)) + 1e-8), atol=1e-12)
 
 
+def test_epilogue_tv_converges_to_the_rof_minimiser_closed_form():
+    """Algorithm 3 is a split-variable solver of min_U 1/2 |U - U0|^2 + lambda TV(U):
+    run long enough it must reach that minimiser, which has a closed form for a two-level periodic
+    stripe (plateau lengths L1, L2, two jumps per period): the plateaus move towards each other by
+    2 lambda / L1 and 2 lambda / L2.  So tv_grad = alpha (X - s U) -> +alpha s 2 lambda / L1 on the high
+    plateau and -alpha s 2 lambda / L2 on the low one.  Checked along x and along z (pins the forward /
+    backward differences, the sign of the B update and the shrink threshold lambda / rho in each axis)
+    and for two values of rho (the limit does not depend on rho)."""
+    from oracle import epilogue as ep
+    L1, L2, hi, lo, lam, alpha = 10, 14, 8.0, 2.0, 0.01, 0.7
+    x = np.empty((4, L1 + L2)); x[:, :L1] = hi; x[:, L1:] = lo
+    for rho in (1.0, 0.5):
+        for img in (x, x.T.copy()):
+            g = ep.tv_gradient(img, iters=1500, rho=rho, lam=lam, alpha=alpha)
+            g = g if img is x else g.T
+            assert np.allclose(g[:, :L1], alpha * hi * 2 * lam / L1, rtol=1e-9, atol=0)
+            assert np.allclose(g[:, L1:], -alpha * hi * 2 * lam / L2, rtol=1e-9, atol=0)
+    # lambda beyond the crossing point (0.75 / (2/L1 + 2/L2) = 2.19 for U0 = X / 8): the minimiser is the
+    # mean, tv_grad = alpha (X - mean)
+    g = ep.tv_gradient(x, iters=1500, rho=1.0, lam=5.0, alpha=1.0)
+    assert np.allclose(g, x - x.mean(), atol=1e-8)
+
+
 def test_epilogue_tv_invariants():
     """Eq. (17) shrink; constant model => zero TV term; the Jacobi sweeps converge to the solution of
     (I + rho D^T D) U = U0 + rho D^T (Z - B) (dense solve on a tiny periodic grid, Z = B = 0 so U -> the
