@@ -293,6 +293,32 @@ def test_epilogue_update_matches_numpy_oracle():
         assert torch.all(d_eps[:, nx:] == 0)                       # pitch padding untouched
 
 
+def test_epilogue_tv_long_run_reaches_rof_closed_form():
+    """The CUDA TV term against mathematics rather than the oracle: run to convergence on a two-level
+    periodic stripe it must give +alpha s 2 lambda / L1 and -alpha s 2 lambda / L2 (the ROF minimiser's
+    closed form, see tests/test_oracle_pins.py), along x (eps_r plane) and along z (sigma plane)."""
+    from paper_2506_20513_b200 import gprfwi_update, gprfwi_update_workspace_bytes, make_update_params
+    L1, L2, lam, alpha = 10, 14, 0.01, 0.7
+    n = L1 + L2
+    ex = np.empty((n, n), np.float32); ex[:, :L1] = 8.0; ex[:, L1:] = 2.0           # stripe along x
+    sz = np.empty((n, n), np.float32); sz[:L1, :] = 0.04; sz[L1:, :] = 0.01         # stripe along z
+    d = dev()
+    d_e, d_s = torch.as_tensor(ex.copy(), device=d), torch.as_tensor(sz.copy(), device=d)
+    g_e, g_s = torch.zeros((n, n), device=d), torch.zeros((n, n), device=d)
+    st = [torch.zeros((n, n), device=d) for _ in range(4)]
+    ws = torch.empty(gprfwi_update_workspace_bytes(n, n), dtype=torch.uint8, device=d)
+    u = make_update_params(step=1, lr_eps_r=0.0, lr_sigma=0.0, tv_iters=1500, tv_rho=1.0, tv_lambda=lam,
+                           tv_alpha=alpha, mask_rows=0)
+    gprfwi_update(n, n, n, u, d_e, d_s, g_e, g_s, st[0], st[1], st[2], st[3], ws)
+    torch.cuda.synchronize()
+    ge, gs = g_e.cpu().numpy(), g_s.cpu().numpy()
+    assert np.array_equal(d_e.cpu().numpy(), ex) and np.array_equal(d_s.cpu().numpy(), sz)      # lr = 0
+    assert np.allclose(ge[:, :L1], alpha * 8.0 * 2 * lam / L1, rtol=2e-3)
+    assert np.allclose(ge[:, L1:], -alpha * 8.0 * 2 * lam / L2, rtol=2e-3)
+    assert np.allclose(gs[:L1, :], alpha * 0.04 * 2 * lam / L1, rtol=2e-3)
+    assert np.allclose(gs[L1:, :], -alpha * 0.04 * 2 * lam / L2, rtol=2e-3)
+
+
 def test_many_receivers_per_tile_and_per_shot_wavelets():
     """More receivers in one tile than the CTA has threads (the per-thread receiver entries overflow
     into the strided loops), receivers on every region row (both words of the row mask), and one
