@@ -124,13 +124,13 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
         }
         u64 ddp, ddq, ppp, ppq;                         // (tx/kx - tz/kz) and (psix - psiz)
         if (ZP && XP) {
-          ddp = fma2(txp, xk.p, neg2(mul2(tzp, kz))); ddq = fma2(txq, xk.q, neg2(mul2(tzq, kz)));
+          ddp = sub2(mul2(txp, xk.p), mul2(tzp, kz)); ddq = sub2(mul2(txq, xk.q), mul2(tzq, kz));
           ppp = sub2(px.p, pz.p); ppq = sub2(px.q, pz.q);
         } else if (ZP) {
           ddp = sub2(txp, mul2(tzp, kz)); ddq = sub2(txq, mul2(tzq, kz));
           ppp = neg2(pz.p); ppq = neg2(pz.q);
         } else {
-          ddp = fma2(txp, xk.p, neg2(tzp)); ddq = fma2(txq, xk.q, neg2(tzq));
+          ddp = sub2(mul2(txp, xk.p), tzp); ddq = sub2(mul2(txq, xk.q), tzq);
           ppp = px.p; ppq = px.q;
         }
         e[r].p = fma2(cb[r].p, fma2(ddp, rdx2, ppp), mul2(ca[r].p, e[r].p));
