@@ -156,7 +156,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2506_20513_b200 import (Simulation, build, gprfwi_gradient_host, gprfwi_residual, gprfwi_update,
+    from paper_2506_20513_b200 import (Simulation, build, split_batch, gprfwi_gradient_host, gprfwi_residual, gprfwi_update,
                                        gprfwi_update_workspace_bytes, gprfwi_workspace_bytes,
                                        gprfwi_workspace_bytes_host, make_params, make_update_params)
     from paper_2506_20513_b200.dist import allreduce_gradients
@@ -174,20 +174,14 @@ def main():
     free, _total = torch.cuda.mem_get_info(dev)
     ntr = wl.nshots * wl.nt * wl.nrec
     budget = int(args.budget_gb * 1e9) if args.budget_gb > 0 else int(free * 0.92) - 3 * ntr * 4
-    # A batch whose states do not fit one call (config 5's largest cells) is split into equal chunks of
-    # shots that are swept one after the other through the same workspace; gradients are summed.
-    nchunks = 1
-    while True:
-        if wl.nshots % nchunks == 0:
-            p.nshots = wl.nshots // nchunks
-            try:
-                sim = Simulation(p, wl.src_zx[:p.nshots], wl.rec_zx[:p.nshots], wl.wavelet, dev, budget_bytes=budget)
-                break
-            except ValueError:
-                pass
-        nchunks += 1
-        if nchunks > wl.nshots:
-            raise SystemExit("the problem does not fit this GPU even one shot at a time")
+    # A batch whose states do not fit one call, or fit only with single-shot adjoint passes (config 5's
+    # largest cells), is split into equal chunks of shots that are swept one after the other through the
+    # same workspace; gradients are summed (paper_2506_20513_b200.split_batch picks the split).
+    try:
+        nchunks, p.nshots, _ = split_batch(p, budget)
+    except ValueError:
+        raise SystemExit("the problem does not fit this GPU even one shot at a time")
+    sim = Simulation(p, wl.src_zx[:p.nshots], wl.rec_zx[:p.nshots], wl.wavelet, dev, budget_bytes=budget)
     cs = p.nshots
     eps = torch.as_tensor(wl.eps_r, device=dev)
     sig = torch.as_tensor(wl.sigma, device=dev)

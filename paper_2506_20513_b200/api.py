@@ -57,6 +57,33 @@ def gprfwi_workspace_bytes_host(p: Params, budget_bytes: int = 0) -> int:
     return int(_lib.load().gprfwi_workspace_bytes_host(ctypes.byref(p), int(budget_bytes)))
 
 
+def split_batch(p: Params, budget_bytes: int = 0, min_shots_per_pass: int = 3):
+    """How many equal calls to split p.nshots shots into so that the library's memory plan is a good one
+    (host-side planning only, gprfwi_workspace_bytes per candidate): the fewest calls whose plan keeps
+    the full history or sends at least `min_shots_per_pass` shots down each adjoint pass (single-shot
+    passes leave the launch lanes empty); failing that, the fewest calls that fit at all.
+    -> (ncalls, shots per call, plan dict).  Gradients of the calls add; traces concatenate."""
+    S = int(p.nshots)
+    first = None
+    try:
+        for ncalls in range(1, S + 1):
+            if S % ncalls:
+                continue
+            p.nshots = S // ncalls
+            nbytes, plan = gprfwi_workspace_bytes(p, budget_bytes)
+            if nbytes == 0:
+                continue
+            if first is None:
+                first = (ncalls, p.nshots, plan)
+            if plan["full_history"] or plan["shots_per_pass"] >= min(min_shots_per_pass, p.nshots):
+                return ncalls, p.nshots, plan
+    finally:
+        p.nshots = S
+    if first is None:
+        raise ValueError("invalid parameters, or the problem does not fit the budget even one shot at a time")
+    return first
+
+
 def gprfwi_forward(p: Params, eps_r, sigma, wavelet, src_zx, rec_zx, workspace, traces, handle=None,
                    stream=None):
     """Enqueue Algorithm 1 on `stream`; returns the (new or reused) handle (an int)."""

@@ -115,3 +115,20 @@ def test_acquisition_presets_match_table_1_semantics():
     assert np.all(np.diff(wl.rec_zx[0, :, 0]) == 1) and np.all(wl.rec_zx[0, :, 1] == wl.rec_zx[0, 0, 1])
     with pytest.raises(AssertionError):
         gi.with_geometry(wl, [[0, 5]], [[[5, 5]]])                                          # on the PEC ring
+
+
+def test_split_batch_prefers_plans_with_several_shots_per_pass():
+    """Host-side planning only: a batch that fits one call only with single-shot adjoint passes is split."""
+    from paper_2506_20513_b200 import split_batch
+    mk = lambda n, b: make_params(nz=n, nx=n, dx=0.01, dt=2e-11, nt=1000, npml=10, pml_order=3, pml_sigma_max=1.0,
+                                  pml_kappa_max=1.0, pml_alpha_max=0.1, nshots=b, nrec=64)
+    budget = int(165e9)
+    p = mk(4096, 128)
+    nbytes, plan1 = gprfwi_workspace_bytes(p, budget)
+    assert nbytes == 0 or plan1["shots_per_pass"] < 3                     # one call: does not fit, or barely
+    ncalls, per_call, plan = split_batch(p, budget)
+    assert ncalls * per_call == 128 and ncalls > 1 and plan["shots_per_pass"] >= 3
+    assert p.nshots == 128                                                # params restored
+    assert split_batch(mk(512, 8), budget)[:2] == (1, 8)                  # fits with full history: no split
+    with pytest.raises(ValueError):
+        split_batch(mk(8192, 4), int(1e9))                                # one shot does not fit 1 GB
