@@ -148,10 +148,12 @@ static void base_layout(const gprfwi_params* p, Layout& L)
 // A CTA owns one tile and sweeps a GROUP of shots one after the other (the adjoint keeps their
 // gradient sum in registers; per-CTA set-up is paid once per group).  Small grids get small groups
 // so that a launch still has a few CTAs per SM slot; once the tiles alone fill the machine `fill`
-// times over, one CTA per tile sweeps all the shots.
+// times over, the shots are dealt into three groups, one per launch lane.
 static void pick_groups(int tiles, int shots, int slots, int fill, int& group, int& ngroups)
 {
-  const int want = std::max(1, std::min(shots, (fill * slots + tiles - 1) / tiles));
+  // never fewer groups than launch lanes: a single group means a single lane, and then every launch
+  // drains before the next one can start (measured: -20 % on config 4, -30 % on 1024^2 x 32 shots)
+  const int want = std::max(1, std::min(shots, std::max(3, (fill * slots + tiles - 1) / tiles)));
   group = (shots + want - 1) / want;
   ngroups = (shots + group - 1) / group;
 }
