@@ -148,12 +148,17 @@ static void base_layout(const gprfwi_params* p, Layout& L)
 // A CTA owns one tile and sweeps a GROUP of shots one after the other (the adjoint keeps their
 // gradient sum in registers; per-CTA set-up is paid once per group).  Small grids get small groups
 // so that a launch still has a few CTAs per SM slot; once the tiles alone fill the machine `fill`
-// times over, the shots are dealt into three groups, one per launch lane.
+// times over, the shots are dealt into two or three groups, one per launch lane.
 static void pick_groups(int tiles, int shots, int slots, int fill, int& group, int& ngroups)
 {
-  // never fewer groups than launch lanes: a single group means a single lane, and then every launch
-  // drains before the next one can start (measured: -20 % on config 4, -30 % on 1024^2 x 32 shots)
-  const int want = std::max(1, std::min(shots, std::max(3, (fill * slots + tiles - 1) / tiles)));
+  // Avoid a single group on mid-sized grids: it means a single launch lane, and a lone lane drains
+  // before the next launch can start (measured: -20 % on config 4, -30 % on 1024^2 x 32 shots).  Two
+  // lanes are enough once one group's launch fills the machine twice over (larger groups amortise the
+  // CTA set-up: config 4, 1024^2 and 2048^2 batches measured 1-5 % better with 2 than with 3), three
+  // below that (config 3); from about 24 waves per launch the drain no longer matters and splitting
+  // the few shots of a pass only costs (4096^2: -3 %, 8192^2: -7 % with two groups).
+  const int floor_groups = tiles >= 24 * slots ? 1 : (tiles >= 2 * slots ? 2 : 3);
+  const int want = std::max(1, std::min(shots, std::max(floor_groups, (fill * slots + tiles - 1) / tiles)));
   group = (shots + want - 1) / want;
   ngroups = (shots + group - 1) / group;
 }
