@@ -270,8 +270,9 @@ def main():
     fwd_launch_us = fwd_ms * 1e3 / nlaunch
     # dram__bytes_read.sum + dram__bytes_write.sum of the adjoint kernel per time block, from the
     # `ncu --set full` capture summarised in profiles/r01_v4_README.md (one lane launch of 6 shots moved
-    # 24.8 MB; scaled to the 20 shots of a block).  Only config 2 has been captured.
-    traffic = {2: 82.7e6}.get(args.config) if not (args.nt or args.shots) else None
+    # 24.8 MB; scaled to the 20 shots of a block).  Config 3: adjoint 521.5 MB + recompute sweep 265.7 MB per
+    # lane launch of 20 shots, three lanes per block (same README).  Config 4 has not been captured.
+    traffic = {2: 82.7e6, 3: 2361.6e6}.get(args.config) if not (args.nt or args.shots) else None
     pair_gbs = (fwd_bytes + adj_bytes + (cells * BYTES_RECOMPUTE * wl.nt / nlaunch if recompute else 0.0)) \
         * nlaunch / ((fwd_ms + adj_ms) * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "adj_kernel (+recompute fwd_kernel)" if recompute else "adj_kernel",
