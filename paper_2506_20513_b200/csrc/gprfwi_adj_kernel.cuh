@@ -100,7 +100,8 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
         le[r].p = add2(le[r].p, v.p); le[r].q = add2(le[r].q, v.q);
         st2(rb, zero2());
       }
-      if ((c.own >> r) & 1u) {
+      {                                                 // (every thread: the ring slots of cells the tile does not own
+                                                        //  are never fetched into and stay zero, so they add nothing)
         const P2 e0 = ld2(h0 + r * kRegW), e1 = ld2(h1 + r * kRegW);      // E^n, E^{n+1}
         ga[r].p = fma2(le[r].p, e0.p, ga[r].p); ga[r].q = fma2(le[r].q, e0.q, ga[r].q);
         gb[r].p = fma2(le[r].p, fma2(neg2(ca[r].p), e0.p, e1.p), gb[r].p);
@@ -210,6 +211,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   c.zero_psi(g);
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
     reinterpret_cast<float4*>(c.rowbuf_())[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+  for (int k = 0; k < 3 * R; ++k)      // the thread's own slots of the Ez-history ring (see [A])
+    st2(c.hist_() + (k / R) * (L::ROWS * kRegW) + (k % R) * kRegW, zero2());
 
   P2 ca[R], cb[R], ga[R], gb[R];
 #pragma unroll
