@@ -246,6 +246,26 @@ def test_config4_grid_subset_against_oracle():
     assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
 
 
+def test_config5_4096_grid_short_run_against_oracle():
+    """Config 5's 4096 x 4096 grid (5145 tiles: the one-group / one-lane launch regime; plane offsets of
+    the second shot beyond 2^24 cells) for 16 steps, one source in the top-left CPML corner tile and one
+    near the bottom-right corner, six receivers within four cells of each source so that 16 steps reach
+    them.  Everything the wave has not reached must stay exactly zero."""
+    import dataclasses
+    wl = gi.config5(n=4096, batch=2, nt=16)
+    off = np.array([(2, 0), (0, 3), (-3, -1), (4, 4), (-2, 2), (1, -4)])
+    src = np.array([(25, 30), (4060, 4070)])
+    wl = gi.with_geometry(wl, src, src[:, None, :] + off[None, :, :], name="config5-4096-short")
+    wl = dataclasses.replace(wl, wavelet=np.sin(0.6 * np.arange(16)).astype(np.float32))
+    tr_o, res, ge_o, gs_o = oracle_all(wl)
+    tr, ge, gs, plan = run_gpu(wl, res)
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o))
+    far = np.ones((wl.nz, wl.nx), bool)
+    for (j, i) in src:
+        far[max(j - 40, 0):j + 41, max(i - 40, 0):i + 41] = False
+    assert np.all(ge[far] == 0.0) and np.all(gs[far] == 0.0) and np.all(ge_o[far] == 0.0)
+
+
 def test_config5_per_shot_receivers_batched():
     """Config 5 (512^2, uniform random eps_r / sigma per cell, every shot its own 64 receivers): a
     batch of 8 in one call, shots 0 and 7 against the oracle, and batched == per-shot bit for bit."""
