@@ -271,8 +271,9 @@ def main():
     # dram__bytes_read.sum + dram__bytes_write.sum of the adjoint kernel per time block, from the
     # `ncu --set full` capture summarised in profiles/r01_v4_README.md (one lane launch of 6 shots moved
     # 24.8 MB; scaled to the 20 shots of a block).  Config 3: adjoint 521.5 MB + recompute sweep 265.7 MB per
-    # lane launch of 20 shots, three lanes per block (same README).  Config 4 has not been captured.
-    traffic = {2: 82.7e6, 3: 2361.6e6}.get(args.config) if not (args.nt or args.shots) else None
+    # lane launch of 20 shots, three lanes per block (same README).  Config 4 (profiles/r01_v5_README.md):
+    # adjoint 1771 MB + recompute sweep 1411 MB per lane launch of 17 shots, scaled to the 100 shots of a block.
+    traffic = {2: 82.7e6, 3: 2361.6e6, 4: 18.72e9}.get(args.config) if not (args.nt or args.shots) else None
     pair_gbs = (fwd_bytes + adj_bytes + (cells * BYTES_RECOMPUTE * wl.nt / nlaunch if recompute else 0.0)) \
         * nlaunch / ((fwd_ms + adj_ms) * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "adj_kernel (+recompute fwd_kernel)" if recompute else "adj_kernel",
