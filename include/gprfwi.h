@@ -70,11 +70,17 @@ typedef struct {
   int32_t  checkpoint_stride;/* K (= nt when full_history)                                       */
   int32_t  shots_per_pass;   /* shots swept together in the adjoint (sub-batch size)             */
   int32_t  time_block;       /* time steps fused per kernel launch                               */
+  int32_t  stored_segments;  /* checkpoint segments (the last ones) whose Ez planes the forward pass
+                                keeps in spare workspace, so the adjoint does not recompute them    */
+  int32_t  reserved;
 } gprfwi_plan;
 
 /* Smallest workspace (bytes) with which gprfwi_forward/adjoint can run `p` when allowed to use
  * at most budget_bytes (0 = no limit): the full Ez history if it fits,
- * otherwise checkpoint-and-recompute with a stride and a shot sub-batch chosen to fit.
+ * otherwise checkpoint-and-recompute with a stride and a shot sub-batch chosen to fit; what the
+ * budget leaves beyond that plan's minimum then holds the Ez planes of the last checkpoint segments
+ * (plan->stored_segments of them), which the adjoint sweeps without recomputing.  The returned size
+ * includes those planes and never exceeds budget_bytes.
  * Returns 0 if `p` is invalid or nothing fits.  If plan != NULL it is filled in. */
 size_t gprfwi_workspace_bytes(const gprfwi_params* p, size_t budget_bytes, gprfwi_plan* plan);
 

@@ -39,7 +39,7 @@ class Plan(ctypes.Structure):
     _fields_ = [
         ("workspace_bytes", ctypes.c_uint64), ("full_history", ctypes.c_int32),
         ("checkpoint_stride", ctypes.c_int32), ("shots_per_pass", ctypes.c_int32),
-        ("time_block", ctypes.c_int32),
+        ("time_block", ctypes.c_int32), ("stored_segments", ctypes.c_int32), ("reserved", ctypes.c_int32),
     ]
 
     def as_dict(self):

@@ -100,6 +100,7 @@ struct Layout {
   int K = 0;               // checkpoint stride (nt when full history)
   int ncheck = 0;          // checkpoints at n = 0, K, 2K, ... (< nt); slot ncheck = state at nt
   int Sb = 0;              // shots per adjoint pass
+  int Mtail = 0;           // last Mtail segments: Ez planes stored by the forward pass (no recompute sweep)
   int group = 1, ngroups = 1;      // adjoint: shots per CTA, CTAs per tile
   int fgroup = 1, fngroups = 1;    // forward
   size_t bytes = 0;
@@ -186,6 +187,7 @@ struct Carve {
   float* hist = nullptr;      // full history: (nt+1) * S planes
   float* ckpt = nullptr;      // (ncheck+1) * S full states
   float* seg = nullptr;       // (K-1) * Sb planes: Ez^{cK+1 .. cK+K-1}
+  float* tail = nullptr;      // Mtail * (K-1) * S planes: the same planes of the last Mtail segments, all shots
   float* fscratch = nullptr;  // 2 * S full states (forward ping-pong; reused by the recompute)
   float* lam = nullptr;       // 2 * Sb full states (adjoint ping-pong)
 };
@@ -220,6 +222,7 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
   } else {
     o.ckpt = (float*)take((size_t)(L.ncheck + 1) * S * L.full * f);
     o.seg = (float*)take(std::max<size_t>((size_t)(L.K - 1) * L.Sb * L.plane, 1) * f);
+    if (L.Mtail > 0) o.tail = (float*)take((size_t)L.Mtail * (L.K - 1) * S * L.plane * f);
   }
   return off;
 }
@@ -239,6 +242,7 @@ static bool make_plan(const gprfwi_params* p, size_t budget, Layout& L)
     if (budget == 0 || L.bytes <= budget) return true;
   }
   L.full_history = false;
+  L.Mtail = 0;
   const int S = p->nshots;
   int prev_sb = -1;
   for (int div = 1; div <= S; ++div) {
@@ -268,7 +272,17 @@ static bool make_plan(const gprfwi_params* p, size_t budget, Layout& L)
     L.K = bestK;
     L.ncheck = (p->nt + L.K - 1) / L.K;
     L.bytes = best;
-    if (budget == 0 || L.bytes <= budget) return true;
+    if (budget == 0 || L.bytes <= budget) {
+      // Memory the plan leaves unused holds the Ez planes of the LAST segments, written by the forward
+      // pass itself: the adjoint meets those segments first and sweeps them without recomputing.
+      const size_t per = (size_t)(L.K - 1) * S * L.plane * sizeof(float);
+      if (budget > L.bytes && per > 0 && env_int("GPRFWI_TAIL", 1)) {
+        L.Mtail = (int)std::min<size_t>((size_t)L.ncheck, (budget - L.bytes) / per);
+        while (L.Mtail > 0 && (L.bytes = carve(p, L, nullptr, nullptr)) > budget) --L.Mtail;
+        if (L.Mtail == 0) L.bytes = best;
+      }
+      return true;
+    }
   }
   return false;
 }
@@ -629,6 +643,8 @@ size_t gprfwi_workspace_bytes(const gprfwi_params* p, size_t budget_bytes, gprfw
     plan->checkpoint_stride = L.K;
     plan->shots_per_pass = L.Sb;
     plan->time_block = L.T;
+    plan->stored_segments = L.full_history ? 1 : L.Mtail;
+    plan->reserved = 0;
   }
   return L.bytes;
 }
@@ -641,6 +657,8 @@ int gprfwi_get_plan(const gprfwi_handle* h, gprfwi_plan* plan)
   plan->checkpoint_stride = h->L.K;
   plan->shots_per_pass = h->L.Sb;
   plan->time_block = h->L.T;
+  plan->stored_segments = h->L.full_history ? 1 : h->L.Mtail;
+  plan->reserved = 0;
   return GPRFWI_OK;
 }
 
@@ -717,8 +735,19 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
         float* src = (n % L.K == 0) ? h->c.ckpt + (size_t)(n / L.K) * S * L.full : slot[idx & 1];
         float* dst = (m == p->nt) ? h->c.ckpt + (size_t)L.ncheck * S * L.full
                    : (m % L.K == 0) ? h->c.ckpt + (size_t)(m / L.K) * S * L.full : slot[(idx + 1) & 1];
-        rc = launch_fwd_block(h, h->lanes[k], n, nsub, sh0, ns, state_at(L, src, S, sh0), state_at(L, dst, S, sh0),
-                              traces, [](int) -> float* { return nullptr; });
+        State in = state_at(L, src, S, sh0), out = state_at(L, dst, S, sh0);
+        const int c = n / L.K, c0 = L.ncheck - L.Mtail;
+        if (c >= c0) {
+          // a stored segment: Ez^{n0+1 .. n1-1} go to (and are stepped from) the tail planes, as in the
+          // recompute sweep; Ez^{n0} and Ez^{n1} are the checkpoints' own planes
+          const int n0 = c * L.K, n1 = std::min(n0 + L.K, p->nt);
+          auto plane = [=](int q) { return h->c.tail + (((size_t)(c - c0) * (L.K - 1) + (q - n0 - 1)) * S + sh0) * L.plane; };
+          if (n != n0) in.ez = plane(n);
+          if (m != n1) out.ez = plane(m);
+          rc = launch_fwd_block(h, h->lanes[k], n, nsub, sh0, ns, in, out, traces, plane);
+        } else {
+          rc = launch_fwd_block(h, h->lanes[k], n, nsub, sh0, ns, in, out, traces, [](int) -> float* { return nullptr; });
+        }
       }
     }
     if (rc != GPRFWI_OK) return rc;
@@ -771,10 +800,12 @@ int gprfwi_adjoint(gprfwi_handle* h, const float* residual, float* grad_eps_r, f
             const size_t slot = (m == p->nt) ? (size_t)L.ncheck : (size_t)(m / L.K);
             return h->c.ckpt + slot * S * L.full + (size_t)g0 * L.plane;
           }
+          if (c >= L.ncheck - L.Mtail)
+            return h->c.tail + (((size_t)(c - (L.ncheck - L.Mtail)) * (L.K - 1) + (m - n0 - 1)) * S + g0) * L.plane;
           return h->c.seg + ((size_t)(m - n0 - 1) * L.Sb + l0) * L.plane;
         };
       };
-      if (!L.full_history) {
+      if (!L.full_history && c < L.ncheck - L.Mtail) {
         // recompute Ez^{n0+1 .. n1-1} from checkpoint c with the same kernel (Ez^{n1} is a checkpoint)
         int idx = 0;
         for (int n = n0; n < n1 - 1; ++idx) {

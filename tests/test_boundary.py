@@ -39,7 +39,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_struct_layout_matches_header():
     assert ctypes.sizeof(_lib.Params) == 15 * 4
-    assert ctypes.sizeof(_lib.Plan) == 8 + 4 * 4
+    assert ctypes.sizeof(_lib.Plan) == 8 + 6 * 4
 
 
 def test_strerror(lib):
@@ -87,6 +87,14 @@ def test_plan_full_history_when_it_fits_else_checkpoints(lib):
                      pml_kappa_max=1.0, pml_alpha_max=0.0, nshots=60, nrec=200)
     nb3, plan3 = gprfwi_workspace_bytes(p3, budget)
     assert 0 < nb3 <= budget and plan3["full_history"] == 0 and plan3["shots_per_pass"] == 60
+    # spare budget holds the Ez planes of the last segments; none of it when the budget is the bare minimum
+    nseg3 = -(-p3.nt // plan3["checkpoint_stride"])
+    assert 0 < plan3["stored_segments"] < nseg3
+    per3 = (plan3["checkpoint_stride"] - 1) * 60 * 540 * 1056 * 4
+    bare = nb3 - plan3["stored_segments"] * per3
+    nb3b, plan3b = gprfwi_workspace_bytes(p3, bare + 1024)
+    assert plan3b["stored_segments"] == 0 and plan3b["checkpoint_stride"] == plan3["checkpoint_stride"]
+    assert abs(nb3b - bare) < 4096
     p4 = make_params(nz=1060, nx=2060, dx=0.005, dt=1e-11, nt=6000, npml=30, pml_order=3, pml_sigma_max=1.0,
                      pml_kappa_max=1.0, pml_alpha_max=0.0, nshots=100, nrec=400)
     nb4, plan4 = gprfwi_workspace_bytes(p4, budget)

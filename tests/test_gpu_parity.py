@@ -142,6 +142,57 @@ def test_checkpoint_recompute_matches_stored_history_and_subbatched():
     assert_parity(wl, ck[:3], (tr_o, ge_o, gs_o), " small-budget")
 
 
+def test_stored_tail_segments_equal_recompute_bit_for_bit(monkeypatch):
+    """a6, hybrid plan: workspace the checkpoint plan leaves unused holds the Ez planes of the last
+    segments (written by the forward pass), and the adjoint sweeps those without a recompute sweep.
+    Same stride and shot grouping as the pure recompute plan, so traces AND gradients must be
+    bit-identical to it; checked with some, all and (sub-batched budgets) whatever segments fit."""
+    wl = gi.small_random(nz=64, nx=140, nt=101, npml=10, nshots=5, nrec=6, seed=78)
+    tr_o, res, ge_o, gs_o = oracle_all(wl)
+    K = 12
+    p = params_of(wl, checkpoint_stride=K)
+    monkeypatch.setenv("GPRFWI_TAIL", "0")
+    nb0, plan0 = gprfwi_workspace_bytes(p, 1 << 40)
+    assert plan0["stored_segments"] == 0 and plan0["shots_per_pass"] == wl.nshots
+    pure = run_gpu(wl, res, budget=nb0, checkpoint_stride=K)
+    assert pure[3]["stored_segments"] == 0
+    assert_parity(wl, pure[:3], (tr_o, ge_o, gs_o), " pure recompute")
+    monkeypatch.setenv("GPRFWI_TAIL", "1")
+    per = (K - 1) * wl.nshots * wl.nz * 160 * 4          # one segment's planes (internal pitch 160)
+    nseg = -(-wl.nt // K)
+    for want, budget in ((3, nb0 + int(3.5 * per)), (nseg, 1 << 40)):
+        hy = run_gpu(wl, res, budget=budget, checkpoint_stride=K)
+        print("[plan] stored tail:", hy[3])
+        assert hy[3]["full_history"] == 0 and hy[3]["stored_segments"] == want
+        assert hy[3]["workspace_bytes"] <= budget
+        for a, b in zip(hy[:3], pure[:3]):
+            assert np.array_equal(a, b)
+    # sub-batched adjoint passes together with stored segments (stride 2: one segment's planes cost
+    # less than one more shot in the pass, so budgets exist where both happen)
+    p2 = params_of(wl, checkpoint_stride=2)
+    monkeypatch.setenv("GPRFWI_TAIL", "0")
+    nb2 = gprfwi_workspace_bytes(p2, 1 << 40)[0]
+    monkeypatch.setenv("GPRFWI_TAIL", "1")
+    seen = 0
+    for b in np.linspace(0.3, 0.99, 70) * nb2:
+        nb, plan = gprfwi_workspace_bytes(p2, int(b))
+        if nb == 0 or plan["shots_per_pass"] == wl.nshots or plan["stored_segments"] == 0:
+            continue
+        seen += 1
+        hy = run_gpu(wl, res, budget=int(b), checkpoint_stride=2)
+        monkeypatch.setenv("GPRFWI_TAIL", "0")
+        ref = run_gpu(wl, res, budget=int(b), checkpoint_stride=2)
+        monkeypatch.setenv("GPRFWI_TAIL", "1")
+        print("[plan] sub-batched + stored:", hy[3])
+        assert ref[3]["stored_segments"] == 0 and ref[3]["shots_per_pass"] == hy[3]["shots_per_pass"] < wl.nshots
+        for a, c in zip(hy[:3], ref[:3]):
+            assert np.array_equal(a, c)
+        if seen == 2:
+            break
+    assert seen > 0
+    print("[plan] sub-batched plans with stored segments checked:", seen)
+
+
 def test_batched_equals_per_shot_and_adjoint_reusable():
     wl = gi.small_random(nz=60, nx=136, nt=120, npml=8, nshots=4, nrec=5, seed=5)
     tr_o, res, _, _ = oracle_all(wl)
