@@ -263,10 +263,14 @@ def main():
     T = plan["time_block"]
     nlaunch = -(-wl.nt // T)
     recompute = not plan["full_history"]
+    # share of the time steps the adjoint phase recomputes: every segment but the last `stored_segments`,
+    # whose Ez planes the forward pass kept in spare workspace
+    nseg = -(-wl.nt // plan["checkpoint_stride"])
+    refrac = (nseg - plan["stored_segments"]) / nseg if recompute else 0.0
     adj_bytes = cells * BYTES_ADJ * wl.nt / nlaunch
-    adj_launch_us = adj_ms * 1e3 / (nlaunch * (2 if recompute else 1))     # recompute launches interleave
-    achieved = (cells * (BYTES_ADJ + (BYTES_RECOMPUTE if recompute else 0.0)) * wl.nt) / (adj_ms * 1e-3) / 1e9
-    fwd_bytes = cells * (BYTES_FWD if plan["full_history"] else 24.0) * wl.nt / nlaunch
+    adj_launch_us = adj_ms * 1e3 / (nlaunch * (1.0 + refrac))              # recompute launches interleave
+    achieved = (cells * (BYTES_ADJ + BYTES_RECOMPUTE * refrac) * wl.nt) / (adj_ms * 1e-3) / 1e9
+    fwd_bytes = cells * (24.0 + (BYTES_FWD - 24.0) * (1.0 - refrac if recompute else 1.0)) * wl.nt / nlaunch   # + Ez planes kept
     fwd_launch_us = fwd_ms * 1e3 / nlaunch
     # dram__bytes_read.sum + dram__bytes_write.sum of the adjoint kernel per time block, from the
     # `ncu --set full` capture summarised in profiles/r01_v4_README.md (one lane launch of 6 shots moved
@@ -274,13 +278,14 @@ def main():
     # lane launch of 20 shots, three lanes per block (same README).  Config 4 (profiles/r01_v5_README.md):
     # adjoint 1771 MB + recompute sweep 1411 MB per lane launch of 17 shots, scaled to the 100 shots of a block.
     traffic = {2: 82.7e6, 3: 2361.6e6, 4: 18.72e9}.get(args.config) if not (args.nt or args.shots) else None
-    pair_gbs = (fwd_bytes + adj_bytes + (cells * BYTES_RECOMPUTE * wl.nt / nlaunch if recompute else 0.0)) \
+    pair_gbs = (fwd_bytes + adj_bytes + cells * BYTES_RECOMPUTE * refrac * wl.nt / nlaunch) \
         * nlaunch / ((fwd_ms + adj_ms) * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "adj_kernel (+recompute fwd_kernel)" if recompute else "adj_kernel",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": peak_src, "steps_per_launch": T,
                 "launch_is": "one time block of T steps over all shots (issued as up to 3 concurrent lane launches)",
                 "algorithmic_bytes_per_launch": adj_bytes, "avg_launch_us": adj_launch_us,
+                "recomputed_fraction_of_steps": refrac,
                 "note": "algorithmic bytes are the one-step-per-pass figures (32 B adj, 28 B fwd per cell-step); "
                         "the kernels fuse T steps per pass, so frac can exceed what a T=1 sweep could reach",
                 "forward": {"kernel": "fwd_kernel", "achieved": fwd_bytes / (fwd_launch_us * 1e-6) / 1e9,
