@@ -140,7 +140,7 @@ struct TileCtx {
   int lane, w, l4, lr0;
   int gj0, gi;          // grid row of this warp's row 0, grid column of this lane's component 0
   int rj0, ri0;         // grid row / column of the region's origin
-  bool colin;           // the lane's float4 lies inside [0, pitch)
+  bool colin;           // the lane's float4 holds at least one grid column: inside [0, roundup4(nx))
   int xslot;            // float offset of this lane's unit in an x-strip row, -1 if it holds no CPML column
   bool xp, zp;          // the CTA's columns / this warp's rows touch the x / z CPML (warp-uniform)
   unsigned zsH, zsE;    // bit r: row gj0 + r carries H- / E-located z psi (warp-uniform)
@@ -172,7 +172,9 @@ struct TileCtx {
     rj0 = tile_y * oz - hz; ri0 = tile_x * kOwnW - 4;
     gj0 = rj0 + lr0; gi = ri0 + l4;
     sm = sm_; toff = lr0 * kRegW + l4;
-    colin = gi >= 0 && gi < g.pitch;
+    // columns at or beyond roundup4(nx) belong to no tile (lanes 1..30 own columns < 120 * tiles_x only up to
+    // the grid edge's unit): nothing ever writes them, so they are never loaded either
+    colin = gi >= 0 && gi < ((g.nx + 3) & ~3);
     xslot = (g.P > 0 && colin) ? xstrip_slot(gi >> 2, g.xnl, g.xur, g.pitch) : -1;
     zsH = zsE = rin = own = 0u;
     xp = g.P > 0 && (ri0 < g.P || ri0 + kRegW > g.nx - 1 - g.P);

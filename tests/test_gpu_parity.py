@@ -35,7 +35,7 @@ def run_gpu(wl, residual=None, pitch=None, budget=0, checkpoint_stride=0):
     pitch = pitch or wl.nx
     p = params_of(wl, pitch=pitch, checkpoint_stride=checkpoint_stride)
     sim = Simulation(p, wl.src_zx, wl.rec_zx, wl.wavelet, dev(), budget_bytes=budget)
-    sim.workspace.fill_(0xAB)          # the library must not rely on a zeroed workspace
+    sim.workspace.fill_(0xFF)          # NaN everywhere: the library must not rely on a zeroed workspace
     e = torch.as_tensor(padded(wl.eps_r, pitch), device=dev())
     s = torch.as_tensor(padded(wl.sigma, pitch), device=dev())
     tr = sim.forward(e, s).cpu().numpy().copy()
@@ -103,7 +103,8 @@ def test_config1_end_to_end_residual_on_gpu():
     assert ee <= TOL_GRAD and es <= TOL_GRAD
 
 
-@pytest.mark.parametrize("shape", [(44, 52, 8), (70, 150, 10), (97, 263, 12), (40, 40, 0), (33, 129, 5)])
+@pytest.mark.parametrize("shape", [(44, 52, 8), (70, 150, 10), (97, 263, 12), (40, 40, 0), (33, 129, 5),
+                                   (50, 120, 10), (41, 100, 8), (37, 230, 6)])
 def test_small_ragged_grids(shape):
     """Several tiles with ragged tails in x and z, scattered interior sources/receivers
     (incl. receivers inside the CPML), CPML thickness not a multiple of 4, and a PEC box."""
