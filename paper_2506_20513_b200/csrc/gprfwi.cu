@@ -160,7 +160,7 @@ static void pick_groups(int tiles, int shots, int slots, int fill, int& group, i
   // the few shots of a pass only costs (4096^2: -3 %, 8192^2: -7 % with two groups).
   const int floor_groups = tiles >= 24 * slots ? 1 : (tiles >= 2 * slots ? 2 : 3);
   const int want = std::max(1, std::min(shots, std::max(floor_groups, (fill * slots + tiles - 1) / tiles)));
-  group = (shots + want - 1) / want;
+  group = std::min((shots + want - 1) / want, kMaxGroup);     // (the kernels keep a per-shot table of kMaxGroup entries)
   ngroups = (shots + group - 1) / group;
 }
 
@@ -170,20 +170,39 @@ static int env_int(const char* name, int dflt)
   return e ? std::atoi(e) : dflt;
 }
 
+// SMs of the current device (queried once; 148 on a B200 and when no device can be asked, e.g. when the
+// plan is sized on a host without a GPU)
+static int sm_count()
+{
+  static const int n = [] {
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) {
+      cudaGetLastError();
+      return 148;
+    }
+    return v;
+  }();
+  return n;
+}
+
 static void set_groups(const gprfwi_params* p, Layout& L)
 {
-  const int fslots = 148 * std::max(1, kFwdShapes[L.fv].minb), aslots = 148 * std::max(1, kAdjShapes[L.av].minb);
+  const int fslots = sm_count() * std::max(1, kFwdShapes[L.fv].minb), aslots = sm_count() * std::max(1, kAdjShapes[L.av].minb);
   pick_groups(L.f.tiles(), p->nshots, fslots, 2, L.fgroup, L.fngroups);
   pick_groups(L.a.tiles(), L.Sb, aslots, 2, L.group, L.ngroups);
-  if (int g = env_int("GPRFWI_FWD_GROUP", 0)) { L.fgroup = std::min(g, p->nshots); L.fngroups = (p->nshots + L.fgroup - 1) / L.fgroup; }
-  if (int g = env_int("GPRFWI_ADJ_GROUP", 0)) { L.group = std::min(g, L.Sb); L.ngroups = (L.Sb + L.group - 1) / L.group; }
+  if (int g = std::min(env_int("GPRFWI_FWD_GROUP", 0), kMaxGroup)) { L.fgroup = std::min(g, p->nshots); L.fngroups = (p->nshots + L.fgroup - 1) / L.fgroup; }
+  if (int g = std::min(env_int("GPRFWI_ADJ_GROUP", 0), kMaxGroup)) { L.group = std::min(g, L.Sb); L.ngroups = (L.Sb + L.group - 1) / L.group; }
 }
 
 // device pointers carved out of the caller's workspace
 struct Carve {
-  float *ca = nullptr, *cb = nullptr, *tables = nullptr, *gca = nullptr, *gcb = nullptr;
-  int *src_off = nullptr, *blk_start = nullptr, *blk_ent = nullptr;   // receivers by owning tile (forward tiling)
-  int *reg_start = nullptr, *reg_ent = nullptr;   // receivers by region (tile + halo) of the adjoint tiling
+  float *ca = nullptr, *cb = nullptr, *gca = nullptr, *gcb = nullptr;
+  // static block (one contiguous range, uploaded with one copy): CPML tables, source cells, receiver tables
+  char* stat = nullptr;
+  size_t stat_bytes = 0;
+  float* tables = nullptr;
+  int *src_zx = nullptr, *blk_start = nullptr, *blk_ent = nullptr, *blk_mask = nullptr;   // receivers by owning tile (forward tiling)
+  int *reg_start = nullptr, *reg_ent = nullptr, *reg_mask = nullptr;   // receivers by region (tile + halo) of the adjoint tiling
   float* hist = nullptr;      // full history: (nt+1) * S planes
   float* ckpt = nullptr;      // (ncheck+1) * S full states
   float* seg = nullptr;       // (K-1) * Sb planes: Ez^{cK+1 .. cK+K-1}
@@ -207,14 +226,19 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
   Carve& o = c ? *c : tmp;
   o.ca = (float*)take(L.plane * f);
   o.cb = (float*)take(L.plane * f);
-  o.tables = (float*)take((size_t)10 * (p->nx + p->nz) * f);
   o.gca = (float*)take((size_t)L.ngroups * L.plane * f);
   o.gcb = (float*)take((size_t)L.ngroups * L.plane * f);
-  o.src_off = (int*)take(S * sizeof(int));
+  const size_t stat0 = off;
+  o.tables = (float*)take((size_t)10 * (p->nx + p->nz) * f);
+  o.stat = (char*)o.tables;
+  o.src_zx = (int*)take(S * 2 * sizeof(int));
   o.blk_start = (int*)take(S * (ntile + 1) * sizeof(int));
   o.blk_ent = (int*)take(std::max<size_t>(S * R, 1) * 2 * sizeof(int));
+  o.blk_mask = (int*)take(S * ntile * 2 * sizeof(int));
   o.reg_start = (int*)take((S * natile + 1) * sizeof(int));
   o.reg_ent = (int*)take(std::max<size_t>(6 * S * R, 1) * 2 * sizeof(int));
+  o.reg_mask = (int*)take(S * natile * 2 * sizeof(int));
+  o.stat_bytes = off - stat0;
   o.fscratch = (float*)take(2 * S * L.full * f);
   o.lam = (float*)take(2 * (size_t)L.Sb * L.full * f);
   if (L.full_history) {
@@ -326,8 +350,13 @@ struct gprfwi_handle {
   Geo geo;
   const float *eps_r = nullptr, *sigma = nullptr, *wavelet = nullptr;
   void* workspace = nullptr;
-  std::vector<float> h_tables;
-  std::vector<int> h_src_off, h_blk_start, h_blk_ent, h_reg_start, h_reg_ent;
+  // Host copy of the static block (CPML tables, source cells, receiver tables) in PINNED memory, laid out
+  // like Carve::stat so that one asynchronous copy uploads it; rebuilt only when the geometry, the plan or
+  // the workspace changes between forward calls on a reused handle.
+  char* stage = nullptr;
+  size_t stage_bytes = 0;
+  std::vector<int32_t> geo_src, geo_rec;     // the acquisition the block was built for
+  const char* stat_on_device = nullptr;      // where it was uploaded to
   bool forward_done = false;
   int64_t launches = 0;
   // Shots are independent, so the launch sequence is issued as `nlanes` interleaved chains on
@@ -341,7 +370,10 @@ struct gprfwi_handle {
     for (cudaStream_t q : lanes) cudaStreamDestroy(q);
     for (cudaEvent_t e : lane_done) cudaEventDestroy(e);
     if (fork) cudaEventDestroy(fork);
+    if (stage) cudaFreeHost(stage);
   }
+  template <class T>
+  T* staged(const T* dev) const { return reinterpret_cast<T*>(stage + (reinterpret_cast<const char*>(dev) - c.stat)); }
 };
 
 namespace gprfwi {
@@ -366,16 +398,24 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
   const gprfwi_params& p = h->p;
   const Layout& L = h->L;
   const int S = p.nshots, R = p.nrec, ntile = L.f.tiles(), natile = L.a.tiles();
-  h->h_src_off.assign(S, 0);
-  h->h_blk_start.assign((size_t)S * (ntile + 1), 0);
-  h->h_blk_ent.assign((size_t)std::max(S * R, 1) * 2, 0);
+  int* h_src = h->staged(h->c.src_zx);
+  int* h_blk_start = h->staged(h->c.blk_start);
+  int* h_blk_ent = h->staged(h->c.blk_ent);
+  unsigned* h_blk_mask = reinterpret_cast<unsigned*>(h->staged(h->c.blk_mask));
+  int* h_reg_start = h->staged(h->c.reg_start);
+  int* h_reg_ent = h->staged(h->c.reg_ent);
+  unsigned* h_reg_mask = reinterpret_cast<unsigned*>(h->staged(h->c.reg_mask));
+  std::fill(h_blk_start, h_blk_start + (size_t)S * (ntile + 1), 0);
+  std::fill(h_blk_mask, h_blk_mask + (size_t)S * ntile * 2, 0u);
+  std::fill(h_reg_mask, h_reg_mask + (size_t)S * natile * 2, 0u);
   auto ok = [&](int z, int x) { return z >= 1 && z <= p.nz - 2 && x >= 1 && x <= p.nx - 2; };
   // forward: receivers by OWNING tile; entry = (offset inside the tile's region rowbuf, receiver index)
   for (int s = 0; s < S; ++s) {
     const int z = src_zx[2 * s], x = src_zx[2 * s + 1];
     if (!ok(z, x)) return GPRFWI_EGEOM;
-    h->h_src_off[s] = z * L.pitch + x;
-    int* start = h->h_blk_start.data() + (size_t)s * (ntile + 1);
+    h_src[2 * s] = z;
+    h_src[2 * s + 1] = x;
+    int* start = h_blk_start + (size_t)s * (ntile + 1);
     std::vector<int> tile_of(R);
     for (int r = 0; r < R; ++r) {
       const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
@@ -389,14 +429,17 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
       const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
       const int ty = rz / L.f.oz, tx = rx / kOwnW;
       const size_t k = (size_t)s * R + fill[tile_of[r]]++;
-      h->h_blk_ent[2 * k] = (rz - (ty * L.f.oz - L.T)) * kRegW + col_pos(rx - (tx * kOwnW - 4));   // internal column order
-      h->h_blk_ent[2 * k + 1] = r;
+      const int row = rz - (ty * L.f.oz - L.T);
+      h_blk_ent[2 * k] = row * kRegW + col_pos(rx - (tx * kOwnW - 4));   // internal column order
+      h_blk_ent[2 * k + 1] = r;
+      h_blk_mask[((size_t)s * ntile + tile_of[r]) * 2 + (row >> 5)] |= 1u << (row & 31);
     }
   }
   // adjoint: receivers by REGION (a receiver within the halo of a tile is injected there too)
   const int arows = kAdjShapes[L.av].rows();
-  h->h_reg_start.assign((size_t)S * natile + 1, 0);
-  h->h_reg_ent.clear();
+  const size_t cap = (size_t)std::max(6 * S * R, 1);
+  size_t nent = 0;
+  h_reg_start[0] = 0;
   std::vector<std::vector<int>> bucket(natile);
   for (int s = 0; s < S; ++s) {
     for (auto& b : bucket) b.clear();
@@ -414,27 +457,56 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
       const int ty = t / L.a.tiles_x, tx = t % L.a.tiles_x;
       for (int r : bucket[t]) {
         const int rz = rec_zx[((size_t)s * R + r) * 2], rx = rec_zx[((size_t)s * R + r) * 2 + 1];
-        h->h_reg_ent.push_back((rz - (ty * L.a.oz - L.T)) * kRegW + col_pos(rx - (tx * kOwnW - 4)));
-        h->h_reg_ent.push_back(r);
+        if (nent >= cap) return GPRFWI_EINVAL;
+        const int row = rz - (ty * L.a.oz - L.T);
+        h_reg_ent[2 * nent] = row * kRegW + col_pos(rx - (tx * kOwnW - 4));
+        h_reg_ent[2 * nent + 1] = r;
+        h_reg_mask[((size_t)s * natile + t) * 2 + (row >> 5)] |= 1u << (row & 31);
+        ++nent;
       }
-      h->h_reg_start[(size_t)s * natile + t + 1] = (int)(h->h_reg_ent.size() / 2);
+      h_reg_start[(size_t)s * natile + t + 1] = (int)nent;
     }
   }
-  if (h->h_reg_ent.size() / 2 > (size_t)std::max(6 * S * R, 1)) return GPRFWI_EINVAL;
-  if (h->h_reg_ent.empty()) h->h_reg_ent.assign(2, 0);
   return GPRFWI_OK;
 }
 
-static int upload_static(gprfwi_handle* h, cudaStream_t st)
+static void fill_geo(gprfwi_handle* h)
 {
   const gprfwi_params& p = h->p;
   const Layout& L = h->L;
-  const int n = p.nx + p.nz;
-  h->h_tables.assign((size_t)10 * n, 0.f);
-  float* t = h->h_tables.data();
-  const float rdx_f = (float)(1.0 / (double)p.dx), Db_f = (float)((double)p.dt / kMu0);
-  const float kap_f = Db_f * rdx_f;                      // exactly what the kernels compute
+  Geo& g = h->geo;
+  g.nz = p.nz; g.nx = p.nx; g.P = p.npml; g.pitch = L.pitch; g.xw = L.xw; g.xnl = L.xnl; g.xur = L.xur;
+  g.plane = (long long)L.plane; g.zstrip = (long long)L.zstrip; g.xstrip = (long long)L.xstrip;
+  g.rdx = (float)(1.0 / (double)p.dx);
+  g.Db = (float)((double)p.dt / kMu0);
+  g.kap = g.Db * g.rdx;                                   // exactly what the kernels compute
+  g.tex = h->c.tables;       g.tez = g.tex + 5 * p.nx;
+  g.thx = g.tez + 5 * p.nz;  g.thz = g.thx + 5 * p.nx;
+}
+
+// CPML tables + geometry -> the pinned host copy of the static block -> one asynchronous upload.  Skipped
+// when the handle already uploaded the same acquisition to the same place (handle reuse in an inversion
+// loop: the caller must then leave the workspace alone between calls, see include/gprfwi.h).
+static int upload_static(gprfwi_handle* h, const int32_t* src_zx, const int32_t* rec_zx, bool same_plan, cudaStream_t st)
+{
+  const gprfwi_params& p = h->p;
+  fill_geo(h);
+  const size_t ns = (size_t)p.nshots * 2, nr = (size_t)p.nshots * p.nrec * 2;
+  if (same_plan && h->stage && h->stat_on_device == h->c.stat && h->geo_src.size() == ns && h->geo_rec.size() == nr &&
+      std::memcmp(h->geo_src.data(), src_zx, ns * sizeof(int32_t)) == 0 &&
+      (nr == 0 || std::memcmp(h->geo_rec.data(), rec_zx, nr * sizeof(int32_t)) == 0))
+    return GPRFWI_OK;
+  h->stat_on_device = nullptr;
+  if (h->stage_bytes < h->c.stat_bytes) {
+    if (h->stage) cudaFreeHost(h->stage);
+    h->stage = nullptr;
+    h->stage_bytes = 0;
+    GPR_CUDA(cudaMallocHost((void**)&h->stage, h->c.stat_bytes));
+    h->stage_bytes = h->c.stat_bytes;
+  }
   // four sets of [5][len]: ex[nx] ez[nz] hx[nx] hz[nz]; rows b, c, 1/kappa, c/dx, Db/(dx kappa)
+  float* t = h->staged(h->c.tables);
+  const float kap_f = h->geo.kap;
   auto fill = [&](float* set, int len, bool hloc) {
     build_table(&p, len, hloc, set, set + len, set + 2 * len);
     for (int i = 0; i < len; ++i) {
@@ -445,25 +517,11 @@ static int upload_static(gprfwi_handle* h, cudaStream_t st)
   float* ex = t;             float* ez = ex + 5 * p.nx;
   float* hx = ez + 5 * p.nz; float* hz = hx + 5 * p.nx;
   fill(ex, p.nx, false); fill(ez, p.nz, false); fill(hx, p.nx, true); fill(hz, p.nz, true);
-  GPR_CUDA(cudaMemcpyAsync(h->c.tables, t, h->h_tables.size() * sizeof(float), cudaMemcpyHostToDevice, st));
-  GPR_CUDA(cudaMemcpyAsync(h->c.src_off, h->h_src_off.data(), h->h_src_off.size() * sizeof(int),
-                           cudaMemcpyHostToDevice, st));
-  GPR_CUDA(cudaMemcpyAsync(h->c.blk_start, h->h_blk_start.data(), h->h_blk_start.size() * sizeof(int),
-                           cudaMemcpyHostToDevice, st));
-  GPR_CUDA(cudaMemcpyAsync(h->c.blk_ent, h->h_blk_ent.data(), h->h_blk_ent.size() * sizeof(int),
-                           cudaMemcpyHostToDevice, st));
-  GPR_CUDA(cudaMemcpyAsync(h->c.reg_start, h->h_reg_start.data(), h->h_reg_start.size() * sizeof(int),
-                           cudaMemcpyHostToDevice, st));
-  GPR_CUDA(cudaMemcpyAsync(h->c.reg_ent, h->h_reg_ent.data(), h->h_reg_ent.size() * sizeof(int),
-                           cudaMemcpyHostToDevice, st));
-  Geo& g = h->geo;
-  g.nz = p.nz; g.nx = p.nx; g.P = p.npml; g.pitch = L.pitch; g.xw = L.xw; g.xnl = L.xnl; g.xur = L.xur;
-  g.plane = (long long)L.plane; g.zstrip = (long long)L.zstrip; g.xstrip = (long long)L.xstrip;
-  g.rdx = rdx_f;
-  g.Db = Db_f;
-  g.kap = kap_f;
-  g.tex = h->c.tables;       g.tez = g.tex + 5 * p.nx;
-  g.thx = g.tez + 5 * p.nz;  g.thz = g.thx + 5 * p.nx;
+  if (int rc = build_geometry(h, src_zx, rec_zx)) return rc;
+  GPR_CUDA(cudaMemcpyAsync(h->c.stat, h->stage, h->c.stat_bytes, cudaMemcpyHostToDevice, st));
+  h->geo_src.assign(src_zx, src_zx + ns);
+  h->geo_rec.assign(rec_zx, rec_zx + nr);
+  h->stat_on_device = h->c.stat;
   return GPRFWI_OK;
 }
 
@@ -546,12 +604,15 @@ static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, 
   a.out = out;
   a.ca = h->c.ca;
   a.cb = h->c.cb;
-  for (int t = 0; t < kMaxT; ++t) a.ez_hist[t] = (t >= 1 && t < nsub) ? ez_of(n + t) : nullptr;
+  // planes for Ez after steps 1 .. nsub-1 of this launch: consecutive at a fixed stride in every plan
+  a.ez_mid = nsub > 1 ? ez_of(n + 1) : nullptr;
+  a.ez_mid_stride = (a.ez_mid && nsub > 2) ? (long long)(ez_of(n + 2) - ez_of(n + 1)) : 0;
   a.wav_stride = p.wavelet_per_shot ? p.nt : 0;
   a.wavelet = h->wavelet + n + (size_t)shot0 * a.wav_stride;
-  a.src_off = h->c.src_off + shot0;
+  a.src_zx = reinterpret_cast<const int2*>(h->c.src_zx) + shot0;
   a.blk_start = h->c.blk_start + (size_t)shot0 * (L.f.tiles() + 1);
   a.blk_ent = reinterpret_cast<const int2*>(h->c.blk_ent) + (size_t)shot0 * p.nrec;
+  a.blk_mask = reinterpret_cast<const uint2*>(h->c.blk_mask) + (size_t)shot0 * L.f.tiles();
   a.trace_stride = (long long)p.nt * p.nrec;
   a.traces = (traces && p.nrec > 0) ? traces + (size_t)shot0 * a.trace_stride + (size_t)n * p.nrec : nullptr;
   a.nrec = p.nrec;
@@ -591,6 +652,7 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   a.residual = residual ? residual + (size_t)shot0 * tstride + (long long)n_hi * p.nrec : nullptr;
   a.reg_start = h->c.reg_start;
   a.reg_ent = reinterpret_cast<const int2*>(h->c.reg_ent);
+  a.reg_mask = reinterpret_cast<const uint2*>(h->c.reg_mask);
   a.nrec = p.nrec;
   a.nsub = nsub;
   a.n_hi = n_hi;
@@ -685,16 +747,19 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
   } else if (std::memcmp(&h->p, p, sizeof(*p)) != 0) {
     return GPRFWI_EINVAL;
   }
+  const bool same_plan = !fresh && h->workspace == workspace && h->L.bytes == L.bytes && h->L.K == L.K &&
+                         h->L.Sb == L.Sb && h->L.Mtail == L.Mtail && h->L.full_history == L.full_history &&
+                         h->L.group == L.group && h->L.fgroup == L.fgroup && h->L.T == L.T && h->L.fv == L.fv &&
+                         h->L.av == L.av;
   h->p = *p;
   h->L = L;
   h->eps_r = eps_r; h->sigma = sigma; h->wavelet = wavelet; h->workspace = workspace;
   h->forward_done = false;
   h->launches = 0;
   carve(p, L, (char*)workspace, &h->c);
-  rc = build_geometry(h, src_zx, rec_zx);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (rc == GPRFWI_OK) rc = upload_static(h, st);
-  if (rc != GPRFWI_OK) { if (fresh) delete h; return rc; }
+  rc = upload_static(h, src_zx, rec_zx, same_plan, st);
+  if (rc != GPRFWI_OK) { if (fresh) delete h; else h->stat_on_device = nullptr; return rc; }
   *hp = h;
 
   const size_t S = p->nshots, f = sizeof(float);
@@ -856,7 +921,7 @@ int gprfwi_residual(const float* d_syn, const float* d_obs, float* residual, siz
 {
   if (!d_syn || !d_obs || !residual) return GPRFWI_EINVAL;
   if (n == 0) return GPRFWI_OK;
-  const int blocks = (int)std::min<size_t>((n + 255) / 256, 148 * 8);
+  const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)sm_count() * 8);
   GPR_LAUNCH(residual_kernel, dim3(blocks), dim3(256), (cudaStream_t)cuda_stream, d_syn, d_obs, residual, n, misfit);
   GPR_CUDA(cudaGetLastError());
   return GPRFWI_OK;
@@ -936,7 +1001,7 @@ int gprfwi_gradient_host(const gprfwi_params* p, const float* eps_r, const float
   gprfwi_handle* h = nullptr;
   rc = gprfwi_forward(&h, p, hc.eps, hc.sig, hc.wav, src_zx, rec_zx, hc.core, workspace_bytes - hc.head,
                       hc.traces, st);
-  if (rc != GPRFWI_OK) return rc;
+  if (rc != GPRFWI_OK) { gprfwi_release(h); return rc; }      // (forward may fail after it has created the handle)
   rc = gprfwi_residual(hc.traces, hc.dobs, hc.res, ntr, hc.misfit, st);
   if (rc == GPRFWI_OK) rc = gprfwi_adjoint(h, hc.res, hc.ge, hc.gs, st);
   gprfwi_release(h);
@@ -1011,7 +1076,7 @@ int gprfwi_lowpass(const float* in, float* out, int32_t nseries, int32_t nt, int
   if (!in || !out || !taps || in == out) return GPRFWI_EINVAL;
   if (nseries < 1 || nt < 1 || nrec < 1 || ntaps < 1 || (ntaps & 1) == 0) return GPRFWI_EINVAL;
   const long long n = (long long)nt * nrec;
-  dim3 grid((unsigned)std::min<long long>((n + 255) / 256, 4 * 148), (unsigned)nseries);
+  dim3 grid((unsigned)std::min<long long>((n + 255) / 256, 4LL * sm_count()), (unsigned)nseries);
   GPR_LAUNCH(lowpass_kernel, grid, dim3(256), (cudaStream_t)cuda_stream, in, out, nt, nrec, taps, ntaps);
   GPR_CUDA(cudaGetLastError());
   return GPRFWI_OK;

@@ -29,6 +29,7 @@ struct AdjArgs {
   long long trace_stride;             // nt * nrec
   const int* reg_start;               // [S*tiles + 1] CSR of receivers by REGION (tile + halo)
   const int2* reg_ent;                // in CSR order: (row*128 + column inside the region, receiver index)
+  const uint2* reg_mask;              // [S*tiles]: bit j = row j of the region holds a receiver of the shot
   int nrec, nsub, n_hi, nt;
   int nshots, group;
   int tiles_x, tiles_y;
@@ -39,23 +40,20 @@ struct AdjArgs {
 #if defined(__CUDACC__)
 // transpose of recording: residual sample n_hi - t enters lamE at the start of reverse step n_hi-1-t;
 // it is staged in rowbuf (zero between uses) one barrier ahead of its use.  The receivers of the
-// region are dealt out one per thread (entry + its residual samples in registers).
+// region are dealt out one per thread (its residual samples of the launch sit in the thread's private
+// shared-memory slot).
 template <int R, int NW>
 __device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
-                                          int2 ent, const float (&rv)[kMaxT], int t)
+                                          int entx, int t)
 {
   using L = RegTile<R, NW, 3>;
   if (a.n_hi - t >= a.nt) return;
-  if (ent.x >= 0) {
-    float v = rv[0];
-#pragma unroll
-    for (int k = 1; k < kMaxT; ++k) v = t == k ? rv[k] : v;
-    atomicAdd(c.rowbuf_() + ent.x, v);                                 // coincident receivers sum
-  }
-  for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {   // more receivers than threads
-    const int2 e2 = a.reg_ent[k];
-    atomicAdd(c.rowbuf_() + e2.x, a.residual[s * a.trace_stride - (long long)t * a.nrec + e2.y]);
-  }
+  if (entx >= 0) atomicAdd(c.rowbuf_() + entx, c.priv_()[t]);          // coincident receivers sum
+  if (rk1 - rk0 > L::THREADS)                                                // more receivers than threads
+    for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {
+      const int2 e2 = a.reg_ent[k];
+      atomicAdd(c.rowbuf_() + e2.x, a.residual[s * a.trace_stride - (long long)t * a.nrec + e2.y]);
+    }
 }
 
 // owned rows of forward plane Ez^{n_hi - t} -> slot t % 3 of the thread's history ring (one commit group)
@@ -70,7 +68,24 @@ __device__ __forceinline__ void adj_fetch(const AdjArgs& a, const TileCtx<R, NW,
     for (int r = 0; r < R; ++r)
       if ((c.own >> r) & 1u) cp_async16(dst + r * kRegW, src + (long long)r * a.g.pitch);
   }
-  cp_async_commit();
+}
+
+// A warp that touches no CPML never uses its thread-private psi slots: they serve as the landing zone for
+// the NEXT shot's adjoint state (field f: 0 lamE, 1 lamHx, 2 lamHy), fetched while this shot is stepped, so
+// that the next shot does not start with the state loads exposed.
+template <int R, int NW>
+__device__ __forceinline__ float* adj_land(const TileCtx<R, NW, 3>& c, int f)
+{
+  return f == 0 ? c.phz_() : (f == 1 ? c.pez_() : c.phx_());
+}
+template <int R, int NW>
+__device__ __forceinline__ void adj_prefetch_state(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s_next, int f)
+{
+  const float* src = (f == 0 ? a.in.ez : (f == 1 ? a.in.hx : a.in.hy)) + s_next * a.g.plane + (long long)c.gj0 * a.g.pitch + c.gi;
+  float* dst = adj_land<R, NW>(c, f);
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+    if (c.colin && ((c.rin >> r) & 1u)) cp_async16(dst + r * kRegW, src + (long long)r * a.g.pitch);
 }
 
 // The T reverse steps of one warp for one shot; ZP / XP as in fwd_steps (the psi forms below give
@@ -78,7 +93,7 @@ __device__ __forceinline__ void adj_fetch(const AdjArgs& a, const TileCtx<R, NW,
 // Packed pairs as in the forward kernel: P = (c0, c2), Q = (c1, c3).
 template <int R, int NW, bool ZP, bool XP>
 __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
-                                          int2 ent, const float (&rv)[kMaxT], unsigned iflags,
+                                          int entx, unsigned iflags, bool prefetch,
                                           P2 (&le)[R], P2 (&lhx)[R], P2 (&lhy)[R], const P2 (&ca)[R], const P2 (&cb)[R],
                                           P2 (&ga)[R], P2 (&gb)[R])
 {
@@ -89,6 +104,12 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
   for (int t = 0; t < a.nsub; ++t) {
     // ---- [A] adjoint source, gradient terms ------------------------------------------------------
     adj_fetch<R, NW>(a, c, s, t + 2);                   // two steps ahead; planes t and t+1 have landed after the wait
+    if (prefetch) {                                     // next shot's state, one field per step, in the same commit group
+      if (t < 3) adj_prefetch_state<R, NW>(a, c, s + 1, t);
+      if (t + 1 == a.nsub)
+        for (int f = t + 1; f < 3; ++f) adj_prefetch_state<R, NW>(a, c, s + 1, f);
+    }
+    cp_async_commit();
     cp_async_wait<1>();
     const float* h1 = c.hist_() + (t % 3) * (L::ROWS * kRegW);
     const float* h0 = c.hist_() + ((t + 1) % 3) * (L::ROWS * kRegW);
@@ -146,7 +167,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
       tzp = tz;
     }
     __syncthreads();
-    if (t + 1 < a.nsub) adj_stage<R, NW>(a, c, s, rk0, rk1, ent, rv, t + 1);
+    if (t + 1 < a.nsub) adj_stage<R, NW>(a, c, s, rk0, rk1, entx, t + 1);
     {
       const P2 tzb = ld2(c.xe_() + (c.w + 1) * kRegW + c.l4);             // tz of the row below the warp's last row
       lhx[R - 1].p = fma2(rdx2, sub2(tzp.p, tzb.p), lhx[R - 1].p);
@@ -207,6 +228,14 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
   const int grp = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
   pdl_launch_dependents();
+  // per-shot scalars of the whole group (static input: nothing a previous launch writes), word k of 4:
+  // receiver range [rk0, rk1) of the region, 64-bit mask of the region rows that hold a receiver
+  const int s_beg = grp * a.group, s_end = min((grp + 1) * a.group, a.nshots);
+  for (int k = threadIdx.x; k < 4 * (s_end - s_beg); k += L::THREADS) {
+    const long long row = (long long)(a.shot_base + s_beg + (k >> 2)) * (a.tiles_x * a.tiles_y) + tile;
+    const int q = k & 3;
+    c.meta_()[k] = q < 2 ? a.reg_start[row + q] : (q == 2 ? (int)a.reg_mask[row].x : (int)a.reg_mask[row].y);
+  }
   c.template stage_tables<false>(g);
   c.zero_psi(g);
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
@@ -225,53 +254,69 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
       cb[r] = ldg2(a.cb + o);
     }
   }
+  __syncthreads();                     // the group's scalars are visible
+  // the receiver this thread injects (receivers of the region are dealt out one per thread); fetched one
+  // shot ahead into the thread's private slot so that no shot starts with a chain of dependent loads
+  {
+    int2 e0 = make_int2(-1, 0);
+    if (c.meta_()[0] + (int)threadIdx.x < c.meta_()[1]) e0 = a.reg_ent[c.meta_()[0] + threadIdx.x];
+    *reinterpret_cast<int2*>(c.priv_() + 4) = e0;
+  }
 
   pdl_wait();                          // everything below reads what the previous launch wrote
-  const int s_end = min((grp + 1) * a.group, a.nshots);
-  for (int s = grp * a.group; s < s_end; ++s) {
+  const bool can_land = g.P > 0 && !(c.zp || c.xp);     // (warp-uniform; the psi slots exist only when npml > 0)
+  bool landed = false;
+  for (int s = s_beg; s < s_end; ++s) {
     // ---- everything this shot needs from global memory, issued together ----------------------------
-    const long long row = (long long)(a.shot_base + s) * (a.tiles_x * a.tiles_y) + tile;
-    const int rk0 = a.reg_start[row], rk1 = a.reg_start[row + 1];
+    const int* m = c.meta_() + (s - s_beg) * 4;
+    const int rk0 = m[0], rk1 = m[1];
+    const unsigned iflags = (unsigned)((((unsigned long long)(unsigned)m[3] << 32) | (unsigned)m[2]) >> c.lr0) & ((1u << R) - 1u);
+    const int2 ent = *reinterpret_cast<const int2*>(c.priv_() + 4);
     P2 le[R], lhx[R], lhy[R];
+    if (landed) cp_async_wait<0>();    // this shot's state was fetched into the warp's landing slots during the previous one
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       le[r] = zero2(); lhx[r] = zero2(); lhy[r] = zero2();
       if (c.colin && ((c.rin >> r) & 1u)) {
-        const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-        le[r] = ldg2(a.in.ez + o);
-        lhx[r] = ldg2(a.in.hx + o);
-        lhy[r] = ldg2(a.in.hy + o);
+        if (landed) {
+          le[r] = ld2(adj_land<R, NW>(c, 0) + r * kRegW);
+          lhx[r] = ld2(adj_land<R, NW>(c, 1) + r * kRegW);
+          lhy[r] = ld2(adj_land<R, NW>(c, 2) + r * kRegW);
+        } else {
+          const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
+          le[r] = ldcg2(a.in.ez + o);  // (written by the previous launch: not through the read-only path)
+          lhx[r] = ldcg2(a.in.hx + o);
+          lhy[r] = ldcg2(a.in.hy + o);
+        }
       }
     }
+    const bool prefetch = can_land && s + 1 < s_end;
     adj_fetch<R, NW>(a, c, s, 0);
+    cp_async_commit();
     adj_fetch<R, NW>(a, c, s, 1);
-    if (threadIdx.x < 2) c.mask_()[threadIdx.x] = 0u;
+    cp_async_commit();
     c.fetch_psi(g, a.in, s);           // lands with the history planes: step 0 waits for all but the newest group
-    // the receiver this thread injects, with its residual samples of this launch
-    int2 ent = make_int2(-1, 0);
+    // this thread's residual samples of this launch, and the receiver it injects for the next shot
     float rv[kMaxT];
 #pragma unroll
     for (int t = 0; t < kMaxT; ++t) rv[t] = 0.f;
-    if (rk0 + (int)threadIdx.x < rk1) {
-      ent = a.reg_ent[rk0 + threadIdx.x];
+    if (ent.x >= 0) {
 #pragma unroll
       for (int t = 0; t < kMaxT; ++t)
         if (t < a.nsub && a.n_hi - t < a.nt) rv[t] = a.residual[s * a.trace_stride - (long long)t * a.nrec + ent.y];
     }
-    __syncthreads();                   // mask zeroed; the previous shot left rowbuf all zero
-    if (ent.x >= 0) atomicOr(c.mask_() + ((ent.x / kRegW) >> 5), 1u << ((ent.x / kRegW) & 31));
-    for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {
-      const int rw = a.reg_ent[k].x / kRegW;
-      atomicOr(c.mask_() + (rw >> 5), 1u << (rw & 31));
-    }
-    adj_stage<R, NW>(a, c, s, rk0, rk1, ent, rv, 0);
+    int2 ent_next = make_int2(-1, 0);
+    if (s + 1 < s_end && m[4] + (int)threadIdx.x < m[5]) ent_next = a.reg_ent[m[4] + threadIdx.x];
+    *reinterpret_cast<float4*>(c.priv_()) = make_float4(rv[0], rv[1], rv[2], rv[3]);
+    *reinterpret_cast<int2*>(c.priv_() + 4) = ent_next;
+    const int entx = ent.x;
+    adj_stage<R, NW>(a, c, s, rk0, rk1, entx, 0);         // (the previous shot left rowbuf all zero, two barriers ago)
     __syncthreads();
-    const unsigned iflags = c.row_flags();
 
-    if (c.zp && c.xp) adj_steps<R, NW, true, true>(a, c, s, rk0, rk1, ent, rv, iflags, le, lhx, lhy, ca, cb, ga, gb);
-    else if (c.zp) adj_steps<R, NW, true, false>(a, c, s, rk0, rk1, ent, rv, iflags, le, lhx, lhy, ca, cb, ga, gb);
-    else if (c.xp) adj_steps<R, NW, false, true>(a, c, s, rk0, rk1, ent, rv, iflags, le, lhx, lhy, ca, cb, ga, gb);
-    else adj_steps<R, NW, false, false>(a, c, s, rk0, rk1, ent, rv, iflags, le, lhx, lhy, ca, cb, ga, gb);
+    if (c.zp && c.xp) adj_steps<R, NW, true, true>(a, c, s, rk0, rk1, entx, iflags, prefetch, le, lhx, lhy, ca, cb, ga, gb);
+    else if (c.zp) adj_steps<R, NW, true, false>(a, c, s, rk0, rk1, entx, iflags, prefetch, le, lhx, lhy, ca, cb, ga, gb);
+    else if (c.xp) adj_steps<R, NW, false, true>(a, c, s, rk0, rk1, entx, iflags, prefetch, le, lhx, lhy, ca, cb, ga, gb);
+    else adj_steps<R, NW, false, false>(a, c, s, rk0, rk1, entx, iflags, prefetch, le, lhx, lhy, ca, cb, ga, gb);
 
     // ---- write back the owned part of the adjoint state ------------------------------------------------
 #pragma unroll
@@ -283,6 +328,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
       st2(a.out.hy + o, lhy[r]);
     }
     if (c.zp || c.xp) c.store_psi(g, a.out, s);
+    landed = prefetch;
   }
 
   // ---- once per CTA: add the register partial sums to this group's gCa / gCb planes --------------------

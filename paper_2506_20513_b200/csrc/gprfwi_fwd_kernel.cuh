@@ -25,12 +25,14 @@ struct FwdArgs {
   Geo g;
   State in, out;              // out.ez: Ez plane after the last step of this launch
   const float *ca, *cb;       // [nz][pitch], 0 on the PEC ring, in PEC cells and in the pitch padding
-  float* ez_hist[kMaxT];      // [t]: plane for Ez after step t (1 <= t < nsub) or NULL; [0] unused
+  float* ez_mid;              // plane for Ez after step 1 of this launch (local shot 0) or NULL: not kept;
+  long long ez_mid_stride;    //   the planes after steps 2 .. nsub-1 follow at this stride (floats)
   const float* wavelet;       // sample n of local shot 0
   long long wav_stride;       // nt or 0
-  const int* src_off;         // [S] j*pitch + i
+  const int2* src_zx;         // [S] (row, column) of the source cell
   const int* blk_start;       // [S][tiles + 1] CSR of receivers by owning tile
   const int2* blk_ent;        // [S][nrec] in CSR order: (row*128 + column inside the tile's region, receiver index)
+  const uint2* blk_mask;      // [S][tiles]: bit j = row j of the tile's region holds a receiver of the shot
   float* traces;              // sample n of local shot 0 (NULL: do not record)
   long long trace_stride;     // nt * nrec
   int nrec, nsub;             // receivers per shot; steps in this launch (<= hz)
@@ -59,10 +61,11 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
   for (int t = 0; t < a.nsub; ++t) {
     // ---- stage 1: trace sample n + t from the published receiver rows ----------------------------
     if (ent.x >= 0) trp[(long long)t * a.nrec] = c.rowbuf_()[ent.x];
-    for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {      // more receivers than threads
-      const int2 en2 = a.blk_ent[(long long)s * a.nrec + k];
-      a.traces[s * a.trace_stride + (long long)t * a.nrec + en2.y] = c.rowbuf_()[en2.x];
-    }
+    if (rk1 - rk0 > L::THREADS)                                                   // more receivers than threads
+      for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {
+        const int2 en2 = a.blk_ent[(long long)s * a.nrec + k];
+        a.traces[s * a.trace_stride + (long long)t * a.nrec + en2.y] = c.rowbuf_()[en2.x];
+      }
 
     // ---- stages 2-3: H update + H CPML -------------------------------------------------------------
     // x tables of this lane's columns (XP only; every lane of an XP warp runs the psi form -- lanes off
@@ -112,7 +115,7 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
       const u64 tzp = sub2(hx[r].p, ha.p), tzq = sub2(hx[r].q, ha.q);
       if (ZP || XP) {
         P2 pz = zero2(), px = zero2();
-        u64 bz = 0ULL, cz = 0ULL, kz = 0ULL;
+        u64 bz = zf2(), cz = zf2(), kz = zf2();
         if (ZP) {
           pz = ld2(c.pez_() + r * kRegW);
           bz = bc2(c.tabz_()[3 * L::ROWS + c.lr0 + r]); cz = bc2(c.tabz_()[4 * L::ROWS + c.lr0 + r]); kz = bc2(c.tabz_()[5 * L::ROWS + c.lr0 + r]);
@@ -157,9 +160,9 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
           e[r].p = pk(v[0], v[2]); e[r].q = pk(v[1], v[3]);
         }
     }
-    float* ez_out = (t + 1 == a.nsub) ? a.out.ez : a.ez_hist[t + 1];
-    if (ez_out) {
-      float* dst = ez_out + hoff;
+    const bool last = t + 1 == a.nsub;
+    if (last || a.ez_mid) {
+      float* dst = (last ? a.out.ez : a.ez_mid + t * a.ez_mid_stride) + hoff;
 #pragma unroll
       for (int r = 0; r < R; ++r) {
         if ((c.own >> r) & 1u) st2(dst, e[r]);
@@ -176,13 +179,19 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
   }
 }
 
-// per-shot scalars, word k of 8: receiver range [rk0, rk1) of the tile, source offset, 4 wavelet samples
+// per-shot scalars, word k of kMetaW: receiver range [rk0, rk1) of the tile, source row and column, 4 wavelet
+// samples, the 64-bit mask of region rows that hold a receiver.  All of it is static input (nothing a
+// previous launch writes), so the whole group's table is loaded once per CTA in the launch prologue.
 __device__ __forceinline__ int fwd_meta_word(const FwdArgs& a, int s, int tile, int ntile, int k)
 {
   if (k == 0) return a.traces ? a.blk_start[(long long)s * (ntile + 1) + tile] : 0;
   if (k == 1) return a.traces ? a.blk_start[(long long)s * (ntile + 1) + tile + 1] : 0;
-  if (k == 2) return a.src_off[s];
-  return (k - 3 < a.nsub) ? __float_as_int(a.wavelet[s * a.wav_stride + (k - 3)]) : 0;
+  if (k == 2) return a.src_zx[s].x;
+  if (k == 3) return a.src_zx[s].y;
+  if (k < 8) return (k - 4 < a.nsub) ? __float_as_int(a.wavelet[s * a.wav_stride + (k - 4)]) : 0;
+  if (k == 8) return a.traces ? (int)a.blk_mask[(long long)s * ntile + tile].x : 0;
+  if (k == 9) return a.traces ? (int)a.blk_mask[(long long)s * ntile + tile].y : 0;
+  return 0;
 }
 
 // Ez, Hx, Hy of shot s (this thread's cells) -> the thread's landing slots, one commit group
@@ -217,7 +226,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
   // once per CTA, overlapping the previous launch's tail: CPML tables -> shared memory, Ca / Cb of the
   // region -> registers; then, once the previous launch's state is complete, the first shot's fields
   pdl_launch_dependents();
-  if (tid < 7) c.meta_()[tid] = fwd_meta_word(a, s0, tile, ntile, tid);
+  for (int k = tid; k < kMetaW * (s1 - s0); k += L::THREADS)
+    c.meta_()[k] = fwd_meta_word(a, s0 + k / kMetaW, tile, ntile, k % kMetaW);
   c.template stage_tables<true>(g);
   c.zero_psi(g);
   P2 ca[R], cb[R];
@@ -239,16 +249,16 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
 
 #pragma unroll 1
   for (int s = s0; s < s1; ++s) {
-    const int* m = c.meta_() + ((s - s0) & 1) * 8;
-    const int rk0 = m[0], rk1 = m[1], src = m[2];
+    const int* m = c.meta_() + (s - s0) * kMetaW;
+    const int rk0 = m[0], rk1 = m[1];
     float wv[kMaxT];
 #pragma unroll
-    for (int t = 0; t < kMaxT; ++t) wv[t] = __int_as_float(m[3 + t]) * (g.rdx * g.rdx);
+    for (int t = 0; t < kMaxT; ++t) wv[t] = __int_as_float(m[4 + t]) * (g.rdx * g.rdx);
     const int2 ent = ent_next;
     // the source cell, if this thread holds it
     int src_r = -1, src_c = 0;
     {
-      const int dj = src / g.pitch - c.gj0, di = src % g.pitch - c.gi;
+      const int dj = m[2] - c.gj0, di = m[3] - c.gi;
       if (dj >= 0 && dj < R && di >= 0 && di < 4) { src_r = dj; src_c = di; }
     }
     // ---- this shot's fields have landed in the thread's slots: move them to registers ---------------
@@ -264,31 +274,25 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
         hy[r] = ld2(c.hist_() + 2 * L::ROWS * kRegW + r * kRegW);
       }
     }
-    if (tid < 2) c.mask_()[tid] = 0u;
-    // publish: row 0 for the warp above, all rows for the first trace sample
+    // this warp's R bits of the mask of region rows that hold a receiver of this shot
+    const unsigned rflags = (unsigned)((((unsigned long long)(unsigned)m[9] << 32) | (unsigned)m[8]) >> c.lr0) & ((1u << R) - 1u);
+    // publish: row 0 for the warp above, the receiver rows for the first trace sample
     st2(c.xe_() + c.w * kRegW + c.l4, e[0]);
+    if (rflags) {
 #pragma unroll
-    for (int r = 0; r < R; ++r) st2(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
-    // ---- next shot: fields into the (now free) landing slots, scalars into the other meta slot ------
+      for (int r = 0; r < R; ++r)
+        if ((rflags >> r) & 1u) st2(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
+    }
+    // ---- next shot: fields into the (now free) landing slots; the receiver it records -----------------
     if (s + 1 >= s1) cp_async_commit();   // (keeps the group count uniform: psi is always the second newest)
-    if (s + 1 < s1) {
-      fwd_fetch<R, NW>(a, c, s + 1);
-      if (tid < 7) c.meta_()[(((s - s0) & 1) ^ 1) * 8 + tid] = fwd_meta_word(a, s + 1, tile, ntile, tid);
-    }
-    __syncthreads();                   // mask zeroed, next shot's scalars visible
-    if (ent.x >= 0) atomicOr(c.mask_() + ((ent.x / kRegW) >> 5), 1u << ((ent.x / kRegW) & 31));
-    for (int k = rk0 + L::THREADS + tid; k < rk1; k += L::THREADS) {
-      const int row = a.blk_ent[(long long)s * a.nrec + k].x / kRegW;
-      atomicOr(c.mask_() + (row >> 5), 1u << (row & 31));
-    }
     ent_next = make_int2(-1, 0);
     if (s + 1 < s1) {
-      const int* mn = c.meta_() + (((s - s0) & 1) ^ 1) * 8;
+      fwd_fetch<R, NW>(a, c, s + 1);
+      const int* mn = m + kMetaW;
       if (mn[0] + tid < mn[1]) ent_next = a.blk_ent[(long long)(s + 1) * a.nrec + mn[0] + tid];
     }
-    __syncthreads();
-    const unsigned rflags = c.row_flags();
     cp_async_wait<1>();                // psi landed (the next shot's fields may still be in flight)
+    __syncthreads();                   // exchange row and receiver rows published
 
     if (c.zp && c.xp) fwd_steps<R, NW, true, true>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
     else if (c.zp) fwd_steps<R, NW, true, false>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);

@@ -20,8 +20,10 @@
 //                     the adjoint stages the residual there for injection
 //   tabx [6][128]     CPML x tables of the region's columns: bhx chx khx bex cex kex
 //   tabz [6][NW*R]    CPML z tables of the region's rows:    bhz chz khz bez cez kez
-//   mask [2]          bit j: region row j holds a receiver of the current shot
-//   meta [2][8]       per-shot scalars of the current and the next shot (receiver range, source, wavelet)
+//   meta [kMaxGroup][kMetaW] per-shot scalars of the shots of the CTA's group (receiver range, source, wavelet,
+//                     mask of the region rows that hold a receiver), loaded once per CTA
+//   priv [THREADS][8]  thread-private scalars (adjoint: the thread's residual samples of this launch, its receiver
+//                     entry for the next shot)
 //   hist [NH][NW*R][128] thread-private cp.async landing zone: adjoint = ring of forward Ez planes fetched two
 //                     steps ahead; forward = Ez, Hx, Hy of the NEXT shot fetched while this one is stepped
 //   psi  [4][NW*R][128]  CPML psi of the region, thread-private (only when npml > 0): hz ez hx ex
@@ -40,6 +42,8 @@ namespace gprfwi {
 constexpr int kMaxT = 4;       // fused steps per launch <= x halo (4 columns = one float4)
 constexpr int kRegW = 128;     // region width  = 32 lanes x float4
 constexpr int kOwnW = 120;     // owned width   = lanes 1..30
+constexpr int kMaxGroup = 32;  // shots one CTA sweeps at most (size of the per-shot scalar table in shared memory)
+constexpr int kMetaW = 12;     // words per shot in that table
 
 template <int R, int NW, int NH = 0>
 struct RegTile {
@@ -50,9 +54,9 @@ struct RegTile {
   static constexpr int ROWBUF = XH + (NW + 1) * kRegW;
   static constexpr int TABX = ROWBUF + ROWS * kRegW;
   static constexpr int TABZ = TABX + 6 * kRegW;
-  static constexpr int MASK = TABZ + 6 * ROWS;                 // 2 words: rows of the region that hold receivers
-  static constexpr int META = MASK + 2;                        // 2 x 8 words: per-shot scalars, fetched one shot ahead
-  static constexpr int HIST = (META + 16 + 31) / 32 * 32 + GPRFWI_SMEM_PAD;
+  static constexpr int META = TABZ + 6 * ROWS;                 // kMaxGroup x kMetaW words: per-shot scalars of the CTA's group
+  static constexpr int PRIV = META + kMetaW * kMaxGroup;       // THREADS x 8 words, thread-private (adjoint: residual samples, next receiver)
+  static constexpr int HIST = (PRIV + 8 * THREADS + 31) / 32 * 32 + GPRFWI_SMEM_PAD;
   static constexpr int PSI = HIST + NH * ROWS * kRegW;
   GPR_HD static size_t smem_bytes(bool pml) { return sizeof(float) * (size_t)(PSI + (pml ? 4 * ROWS * kRegW : 0)); }
 };
@@ -65,32 +69,31 @@ __device__ __forceinline__ float FA(float a, float b) { return __fadd_rn(a, b); 
 __device__ __forceinline__ float FF(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 
 // ---- packed pairs of fp32 (sm_100: one FFMA2 / FADD2 / FMUL2 does two IEEE-rounded operations in one
-// issue slot; the kernels are issue-bound, not FP-pipe-bound).  A float4 unit of a row is held as
-// P = (c0, c2), Q = (c1, c3): see gprfwi_common.cuh.
-typedef unsigned long long u64;
+// issue slot).  A float4 unit of a row is held as P = (c0, c2), Q = (c1, c3): see gprfwi_common.cuh.
+// The pairs are plain float2 values and the operations the sm_100 intrinsics of crt/sm_100_rt.h (explicit
+// round-to-nearest per component, never contracted), so that ptxas sees the components: negations fold
+// into operand modifiers and scalar operands into the broadcast form instead of costing LOP3 / MOV pairs.
+typedef float2 u64;
 struct P2 { u64 p, q; };
-__device__ __forceinline__ u64 pk(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ float lo2(u64 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
-__device__ __forceinline__ float hi2(u64 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
-__device__ __forceinline__ u64 bc2(float v) { return pk(v, v); }
-__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ u64 neg2(u64 a) { return a ^ 0x8000000080000000ULL; }
-__device__ __forceinline__ P2 zero2() { P2 v; v.p = 0ULL; v.q = 0ULL; return v; }
-__device__ __forceinline__ P2 ldg2(const float* p)          // read-only global, 128 bit
-{
-  const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2*>(p));
-  P2 r; r.p = v.x; r.q = v.y; return r;
-}
-__device__ __forceinline__ P2 ld2(const float* p)           // shared / generic, 128 bit
-{
-  const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(p);
-  P2 r; r.p = v.x; r.q = v.y; return r;
-}
-__device__ __forceinline__ void st2(float* p, P2 v) { *reinterpret_cast<ulonglong2*>(p) = make_ulonglong2(v.p, v.q); }
-__device__ __forceinline__ void stcs2(float* p, P2 v) { __stcs(reinterpret_cast<ulonglong2*>(p), make_ulonglong2(v.p, v.q)); }
+__device__ __forceinline__ u64 pk(float lo, float hi) { return make_float2(lo, hi); }
+__device__ __forceinline__ float lo2(u64 v) { return v.x; }
+__device__ __forceinline__ float hi2(u64 v) { return v.y; }
+__device__ __forceinline__ u64 bc2(float v) { return make_float2(v, v); }
+__device__ __forceinline__ u64 zf2() { return make_float2(0.f, 0.f); }
+__device__ __forceinline__ u64 neg2(u64 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { return __fadd2_rn(a, neg2(b)); }
+__device__ __forceinline__ P2 zero2() { P2 v; v.p = zf2(); v.q = zf2(); return v; }
+__device__ __forceinline__ P2 mkP2(float4 v) { P2 r; r.p = make_float2(v.x, v.y); r.q = make_float2(v.z, v.w); return r; }
+__device__ __forceinline__ float4 f4of(P2 v) { return make_float4(v.p.x, v.p.y, v.q.x, v.q.y); }
+__device__ __forceinline__ P2 ldg2(const float* p) { return mkP2(__ldg(reinterpret_cast<const float4*>(p))); }     // read-only global, 128 bit
+// global through L2 only (data a previous launch wrote), 128 bit
+__device__ __forceinline__ P2 ldcg2(const float* p) { return mkP2(__ldcg(reinterpret_cast<const float4*>(p))); }
+__device__ __forceinline__ P2 ld2(const float* p) { return mkP2(*reinterpret_cast<const float4*>(p)); }            // shared / generic, 128 bit
+__device__ __forceinline__ void st2(float* p, P2 v) { *reinterpret_cast<float4*>(p) = f4of(v); }
+__device__ __forceinline__ void stcs2(float* p, P2 v) { __stcs(reinterpret_cast<float4*>(p), f4of(v)); }
 
 __device__ __forceinline__ void ldg4a(const float* p, float* o)
 {
@@ -152,14 +155,8 @@ struct TileCtx {
   __device__ __forceinline__ float* rowbuf_() const { return sm + L::ROWBUF; }
   __device__ __forceinline__ float* tabx_() const { return sm + L::TABX; }
   __device__ __forceinline__ float* tabz_() const { return sm + L::TABZ; }
-  __device__ __forceinline__ unsigned* mask_() const { return reinterpret_cast<unsigned*>(sm + L::MASK); }
-  // this warp's R bits of the receiver-row mask (valid after the barrier that follows the atomicOr's)
-  __device__ __forceinline__ unsigned row_flags() const
-  {
-    const unsigned long long m = (unsigned long long)mask_()[0] | ((unsigned long long)mask_()[1] << 32);
-    return (unsigned)(m >> lr0) & ((1u << R) - 1u);
-  }
   __device__ __forceinline__ int* meta_() const { return reinterpret_cast<int*>(sm + L::META); }
+  __device__ __forceinline__ float* priv_() const { return sm + L::PRIV + 8 * threadIdx.x; }
   __device__ __forceinline__ float* hist_() const { return sm + L::HIST + toff; }
   __device__ __forceinline__ float* phz_() const { return sm + L::PSI + 0 * L::ROWS * kRegW + toff; }
   __device__ __forceinline__ float* pez_() const { return sm + L::PSI + 1 * L::ROWS * kRegW + toff; }
