@@ -24,6 +24,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB_PATH
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
+    flags += os.environ.get("GPRFWI_NVCC_EXTRA", "").split()       # tuning builds, e.g. -DGPRFWI_PROBE
     tmp = LIB_PATH + f".tmp{os.getpid()}"
     cmd = [nvcc, *flags, *(["-Xptxas", "-v"] if verbose else []), "-I", os.path.join(_ROOT, "include"),
            "-I", CSRC, "-o", tmp, os.path.join(CSRC, "gprfwi.cu")]

@@ -68,8 +68,8 @@ static Shape fwd_shape()
 template <int R, int NW, int MINB>
 static Shape adj_shape()
 {
-  return {R, NW, MINB, (const void*)adj_kernel<R, NW, MINB>, RegTile<R, NW, 3>::smem_bytes(true),
-          RegTile<R, NW, 3>::smem_bytes(false)};
+  return {R, NW, MINB, (const void*)adj_kernel<R, NW, MINB>, RegTile<R, NW, kAdjRing>::smem_bytes(true),
+          RegTile<R, NW, kAdjRing>::smem_bytes(false)};
 }
 static const Shape kFwdShapes[] = {fwd_shape<3, 12, 1>(), fwd_shape<3, 8, 2>(), fwd_shape<4, 12, 1>(), fwd_shape<2, 16, 1>()};
 static const Shape kAdjShapes[] = {adj_shape<3, 12, 1>(), adj_shape<3, 8, 2>(), adj_shape<4, 12, 1>(), adj_shape<2, 16, 1>()};
@@ -92,6 +92,10 @@ struct Layout {
   size_t plane = 0, zstrip = 0, xstrip = 0;
   size_t hslot = 0;        // Hx, Hy, 4 psi strips of ONE shot
   size_t full = 0;         // hslot + Ez plane
+  // a block of S complete states (arrays ez[S] hx[S] hy[S] + strips), padded to whole planes so that every
+  // field plane of the workspace sits a whole number of planes from its first byte (the TMA tensor maps
+  // address the workspace as ONE array of planes, gprfwi_tile.cuh)
+  size_t blk(size_t S) const { return (S * full + plane - 1) / plane * plane; }
   int T = 4;               // time steps fused per launch = halo rows
   Tiling f, a;             // forward / adjoint tilings
   int fv = 0, av = 0;      // kernel shapes in use (indices into kFwdShapes / kAdjShapes)
@@ -209,6 +213,7 @@ struct Carve {
   float* tail = nullptr;      // Mtail * (K-1) * S planes: the same planes of the last Mtail segments, all shots
   float* fscratch = nullptr;  // 2 * S full states (forward ping-pong; reused by the recompute)
   float* lam = nullptr;       // 2 * Sb full states (adjoint ping-pong)
+  size_t nplanes = 0;         // planes from ca to the end of the last plane array
 };
 
 // One routine both sizes and carves the workspace, so the two can never disagree.
@@ -224,10 +229,28 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
   const size_t ntile = (size_t)L.f.tiles(), natile = (size_t)L.a.tiles();
   Carve tmp;
   Carve& o = c ? *c : tmp;
-  o.ca = (float*)take(L.plane * f);
-  o.cb = (float*)take(L.plane * f);
-  o.gca = (float*)take((size_t)L.ngroups * L.plane * f);
-  o.gcb = (float*)take((size_t)L.ngroups * L.plane * f);
+  // arrays of field planes start a whole number of planes from the workspace's first byte
+  auto take_planes = [&](size_t bytes) -> char* {
+    off = align_up(off, L.plane * f);
+    char* r = base ? base + off : nullptr;
+    off += bytes;
+    return r;
+  };
+  o.ca = (float*)take_planes(L.plane * f);
+  o.cb = (float*)take_planes(L.plane * f);
+  o.gca = (float*)take_planes((size_t)L.ngroups * L.plane * f);
+  o.gcb = (float*)take_planes((size_t)L.ngroups * L.plane * f);
+  o.fscratch = (float*)take_planes(2 * L.blk(S) * f);
+  o.lam = (float*)take_planes(2 * L.blk(L.Sb) * f);
+  if (L.full_history) {
+    o.hist = (float*)take_planes((size_t)(p->nt + 1) * S * L.plane * f);
+  } else {
+    o.ckpt = (float*)take_planes((size_t)(L.ncheck + 1) * L.blk(S) * f);
+    o.seg = (float*)take_planes(std::max<size_t>((size_t)(L.K - 1) * L.Sb * L.plane, 1) * f);
+    if (L.Mtail > 0) o.tail = (float*)take_planes((size_t)L.Mtail * (L.K - 1) * S * L.plane * f);
+  }
+  o.nplanes = (off + L.plane * f - 1) / (L.plane * f);
+  off = align_up(off, 256);
   const size_t stat0 = off;
   o.tables = (float*)take((size_t)10 * (p->nx + p->nz) * f);
   o.stat = (char*)o.tables;
@@ -239,15 +262,6 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
   o.reg_ent = (int*)take(std::max<size_t>(6 * S * R, 1) * 2 * sizeof(int));
   o.reg_mask = (int*)take(S * natile * 2 * sizeof(int));
   o.stat_bytes = off - stat0;
-  o.fscratch = (float*)take(2 * S * L.full * f);
-  o.lam = (float*)take(2 * (size_t)L.Sb * L.full * f);
-  if (L.full_history) {
-    o.hist = (float*)take((size_t)(p->nt + 1) * S * L.plane * f);
-  } else {
-    o.ckpt = (float*)take((size_t)(L.ncheck + 1) * S * L.full * f);
-    o.seg = (float*)take(std::max<size_t>((size_t)(L.K - 1) * L.Sb * L.plane, 1) * f);
-    if (L.Mtail > 0) o.tail = (float*)take((size_t)L.Mtail * (L.K - 1) * S * L.plane * f);
-  }
   return off;
 }
 
@@ -357,6 +371,9 @@ struct gprfwi_handle {
   size_t stage_bytes = 0;
   std::vector<int32_t> geo_src, geo_rec;     // the acquisition the block was built for
   const char* stat_on_device = nullptr;      // where it was uploaded to
+  // TMA views of the workspace (gprfwi_tile.cuh): box = 128 columns x owned rows / x region rows of a tile
+  CUtensorMap tm_adj_own, tm_adj_reg, tm_fwd_reg;
+  const void* tm_base = nullptr;             // workspace the maps were encoded for
   bool forward_done = false;
   int64_t launches = 0;
   // Shots are independent, so the launch sequence is issued as `nlanes` interleaved chains on
@@ -525,6 +542,49 @@ static int upload_static(gprfwi_handle* h, const int32_t* src_zx, const int32_t*
   return GPRFWI_OK;
 }
 
+// The workspace from its first byte (Ca) as a 3-D fp32 tensor [nplanes][nz][roundup4(nx)] with row pitch
+// L.pitch: every field plane the kernels touch is one z-slice of it (carve() keeps them plane-aligned).
+// cuTensorMapEncodeTiled is a driver entry point; it is fetched through the runtime, so the library links
+// against cudart only.
+static int encode_map(CUtensorMap* map, const gprfwi_handle* h, int box_rows)
+{
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn fn = nullptr;
+  if (!fn) {
+    void* sym = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    GPR_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &q));
+    if (!sym || q != cudaDriverEntryPointSuccess) return cuda_fail(cudaErrorNotSupported, "cuTensorMapEncodeTiled lookup");
+    fn = (encode_fn)sym;
+  }
+  const Layout& L = h->L;
+  const cuuint64_t dims[3] = {(cuuint64_t)((h->p.nx + 3) & ~3), (cuuint64_t)h->p.nz, (cuuint64_t)h->c.nplanes};
+  const cuuint64_t strides[2] = {(cuuint64_t)L.pitch * sizeof(float), (cuuint64_t)L.plane * sizeof(float)};
+  const cuuint32_t box[3] = {(cuuint32_t)kRegW, (cuuint32_t)box_rows, 1u};
+  const cuuint32_t estr[3] = {1u, 1u, 1u};
+  const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)h->c.ca, dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return GPRFWI_ECUDA;
+  }
+  return GPRFWI_OK;
+}
+
+static int maps_init(gprfwi_handle* h, bool same_plan)
+{
+  if (same_plan && h->tm_base == (const void*)h->c.ca) return GPRFWI_OK;
+  h->tm_base = nullptr;
+  if (int rc = encode_map(&h->tm_adj_own, h, h->L.a.oz)) return rc;
+  if (int rc = encode_map(&h->tm_adj_reg, h, kAdjShapes[h->L.av].rows())) return rc;
+  if (int rc = encode_map(&h->tm_fwd_reg, h, kFwdShapes[h->L.fv].rows())) return rc;
+  h->tm_base = (const void*)h->c.ca;
+  return GPRFWI_OK;
+}
+
 static int kernels_init(const gprfwi_params* p, const Layout& L)
 {
   const bool pml = p->npml > 0;
@@ -645,7 +705,11 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   a.out = out;
   a.ca = h->c.ca;
   a.cb = h->c.cb;
-  for (int t = 0; t <= kMaxT; ++t) a.ez_planes[t] = t <= nsub ? ez_of(n_hi - t) : nullptr;
+  auto plane_index = [&](const float* q) { return (int)((q - h->c.ca) / (long long)L.plane); };
+  a.tm_own = h->tm_adj_own;
+  a.tm_reg = h->tm_adj_reg;
+  for (int t = 0; t <= kMaxT; ++t) a.ez_pl[t] = t <= nsub ? plane_index(ez_of(n_hi - t)) : 0;
+  a.in_pl[0] = plane_index(in.ez); a.in_pl[1] = plane_index(in.hx); a.in_pl[2] = plane_index(in.hy);
   a.gca = h->c.gca + (size_t)grp0 * L.plane;        // this launch's groups start at plane pair grp0
   a.gcb = h->c.gcb + (size_t)grp0 * L.plane;
   a.trace_stride = tstride;
@@ -726,6 +790,16 @@ int gprfwi_get_plan(const gprfwi_handle* h, gprfwi_plan* plan)
 
 int64_t gprfwi_launch_count(const gprfwi_handle* h) { return h ? h->launches : 0; }
 
+#ifdef GPRFWI_PROBE
+// tuning builds only: copy the adjoint kernel's clock stamps (gprfwi_adj_kernel.cuh) to the host
+int gprfwi_probe_read(long long* out, size_t bytes)
+{
+  GPR_CUDA(cudaDeviceSynchronize());
+  GPR_CUDA(cudaMemcpyFromSymbol(out, g_probe, std::min(bytes, sizeof(g_probe))));
+  return GPRFWI_OK;
+}
+#endif
+
 void gprfwi_release(gprfwi_handle* h) { delete h; }
 
 int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_r, const float* sigma,
@@ -759,6 +833,7 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
   carve(p, L, (char*)workspace, &h->c);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   rc = upload_static(h, src_zx, rec_zx, same_plan, st);
+  if (rc == GPRFWI_OK) rc = maps_init(h, same_plan);
   if (rc != GPRFWI_OK) { if (fresh) delete h; else h->stat_on_device = nullptr; return rc; }
   *hp = h;
 
@@ -771,12 +846,12 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
     h->launches++;
   }
   // fields are zero at n = 0
-  GPR_CUDA(cudaMemsetAsync(h->c.fscratch, 0, 2 * S * L.full * f, st));
-  float* slot[2] = {h->c.fscratch, h->c.fscratch + S * L.full};
+  GPR_CUDA(cudaMemsetAsync(h->c.fscratch, 0, 2 * L.blk(S) * f, st));
+  float* slot[2] = {h->c.fscratch, h->c.fscratch + L.blk(S)};
   rc = kernels_init(p, L);
   if (rc != GPRFWI_OK) return rc;
   if (L.full_history) GPR_CUDA(cudaMemsetAsync(h->c.hist, 0, S * L.plane * f, st));
-  else GPR_CUDA(cudaMemsetAsync(h->c.ckpt, 0, S * L.full * f, st));       // checkpoint 0 = zero state
+  else GPR_CUDA(cudaMemsetAsync(h->c.ckpt, 0, L.blk(S) * f, st));       // checkpoint 0 = zero state
   // blocks of up to T steps that never cross a checkpoint boundary, issued lane by lane
   rc = lanes_init(h);
   if (rc != GPRFWI_OK) return rc;
@@ -797,9 +872,9 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
         rc = launch_fwd_block(h, h->lanes[k], n, nsub, sh0, ns, in, out, traces,
                               [&](int q) { return h->c.hist + ((size_t)q * S + sh0) * L.plane; });
       } else {
-        float* src = (n % L.K == 0) ? h->c.ckpt + (size_t)(n / L.K) * S * L.full : slot[idx & 1];
-        float* dst = (m == p->nt) ? h->c.ckpt + (size_t)L.ncheck * S * L.full
-                   : (m % L.K == 0) ? h->c.ckpt + (size_t)(m / L.K) * S * L.full : slot[(idx + 1) & 1];
+        float* src = (n % L.K == 0) ? h->c.ckpt + (size_t)(n / L.K) * L.blk(S) : slot[idx & 1];
+        float* dst = (m == p->nt) ? h->c.ckpt + (size_t)L.ncheck * L.blk(S)
+                   : (m % L.K == 0) ? h->c.ckpt + (size_t)(m / L.K) * L.blk(S) : slot[(idx + 1) & 1];
         State in = state_at(L, src, S, sh0), out = state_at(L, dst, S, sh0);
         const int c = n / L.K, c0 = L.ncheck - L.Mtail;
         if (c >= c0) {
@@ -836,15 +911,15 @@ int gprfwi_adjoint(gprfwi_handle* h, const float* residual, float* grad_eps_r, f
   const size_t S = p->nshots, f = sizeof(float);
   GPR_CUDA(cudaMemsetAsync(h->c.gca, 0, (size_t)L.ngroups * L.plane * f, st));
   GPR_CUDA(cudaMemsetAsync(h->c.gcb, 0, (size_t)L.ngroups * L.plane * f, st));
-  float* lam[2] = {h->c.lam, h->c.lam + (size_t)L.Sb * L.full};
-  float* rs[2] = {h->c.fscratch, h->c.fscratch + S * L.full};     // recompute ping-pong
+  float* lam[2] = {h->c.lam, h->c.lam + L.blk(L.Sb)};
+  float* rs[2] = {h->c.fscratch, h->c.fscratch + L.blk(S)};     // recompute ping-pong
 
   int rc = lanes_init(h);
   if (rc != GPRFWI_OK) return rc;
   for (int shot0 = 0; shot0 < (int)S; shot0 += L.Sb) {
     const int ns = std::min(L.Sb, (int)S - shot0);
     // lambda = 0 at the end time, Eq. (10)
-    GPR_CUDA(cudaMemsetAsync(h->c.lam, 0, 2 * (size_t)L.Sb * L.full * f, st));
+    GPR_CUDA(cudaMemsetAsync(h->c.lam, 0, 2 * L.blk(L.Sb) * f, st));
     // the shots of this pass go down `nl` interleaved lanes (chunks are whole CTA groups)
     const std::vector<int> lb = lane_bounds(ns, (int)h->lanes.size(), L.group);
     const int nl = (int)lb.size() - 1;
@@ -860,10 +935,10 @@ int gprfwi_adjoint(gprfwi_handle* h, const float* residual, float* grad_eps_r, f
         return [=](int m) -> float* {
           const int g0 = shot0 + l0;
           if (L.full_history) return h->c.hist + ((size_t)m * S + g0) * L.plane;
-          if (m == n0) return h->c.ckpt + (size_t)c * S * L.full + (size_t)g0 * L.plane;
+          if (m == n0) return h->c.ckpt + (size_t)c * L.blk(S) + (size_t)g0 * L.plane;
           if (m == n1) {
             const size_t slot = (m == p->nt) ? (size_t)L.ncheck : (size_t)(m / L.K);
-            return h->c.ckpt + slot * S * L.full + (size_t)g0 * L.plane;
+            return h->c.ckpt + slot * L.blk(S) + (size_t)g0 * L.plane;
           }
           if (c >= L.ncheck - L.Mtail)
             return h->c.tail + (((size_t)(c - (L.ncheck - L.Mtail)) * (L.K - 1) + (m - n0 - 1)) * S + g0) * L.plane;
@@ -878,7 +953,7 @@ int gprfwi_adjoint(gprfwi_handle* h, const float* residual, float* grad_eps_r, f
           for (int k = 0; k < nl; ++k) {
             const int l0 = lb[k], nsl = lb[k + 1] - lb[k], g0 = shot0 + l0;
             auto ez_plane = ez_plane_of(l0);
-            State in = (n == n0) ? state_at(L, h->c.ckpt + (size_t)c * S * L.full, S, g0)
+            State in = (n == n0) ? state_at(L, h->c.ckpt + (size_t)c * L.blk(S), S, g0)
                                  : state_at(L, rs[idx & 1], S, l0);
             State out = state_at(L, rs[(idx + 1) & 1], S, l0);
             in.ez = ez_plane(n);

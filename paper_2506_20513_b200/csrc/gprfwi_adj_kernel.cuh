@@ -20,10 +20,16 @@
 namespace gprfwi {
 
 struct AdjArgs {
+  // TMA views of the workspace as one 3-D array [plane][nz][roundup4(nx)] of fp32 (all field planes sit a
+  // whole number of planes from its first byte): box = 128 columns x the tile's owned rows / x all the
+  // region's rows
+  alignas(64) CUtensorMap tm_own;
+  alignas(64) CUtensorMap tm_reg;
   Geo g;
   State in, out;                      // adjoint variables, ping-pong (pointers of local shot 0)
   const float *ca, *cb;               // masked as in the forward kernel
-  const float* ez_planes[kMaxT + 1];  // [t] = forward Ez^{n_hi - t} (local shot 0), t = 0..nsub
+  int ez_pl[kMaxT + 1];               // [t] = workspace plane index of forward Ez^{n_hi - t} (local shot 0), t = 0..nsub
+  int in_pl[3];                       // workspace plane indices of in.ez, in.hx, in.hy (local shot 0)
   float *gca, *gcb;                   // [ngroups][nz][pitch]
   const float* residual;              // sample n_hi of local shot 0 (sample n_hi - t at - t*nrec)
   long long trace_stride;             // nt * nrec
@@ -38,15 +44,28 @@ struct AdjArgs {
 };
 
 #if defined(__CUDACC__)
+// Tuning aid (builds with -DGPRFWI_PROBE only): clock64 stamps of every warp of one interior CTA at fixed
+// points of each shot, read back with gprfwi_probe_read (gprfwi.cu).
+#ifdef GPRFWI_PROBE
+__device__ long long g_probe[kMaxGroup][16][12];
+#define GPR_PROBE(shot, k)                                                                          \
+  do {                                                                                              \
+    if (blockIdx.x == gridDim.x / 2 && blockIdx.y == gridDim.y / 2 && blockIdx.z == 0 && (threadIdx.x & 31) == 0) \
+      g_probe[(shot)][threadIdx.x >> 5][(k)] = clock64();                                           \
+  } while (0)
+#else
+#define GPR_PROBE(shot, k) do { } while (0)
+#endif
+
 // transpose of recording: residual sample n_hi - t enters lamE at the start of reverse step n_hi-1-t;
 // it is staged in rowbuf (zero between uses) one barrier ahead of its use.  The receivers of the
 // region are dealt out one per thread (its residual samples of the launch sit in the thread's private
 // shared-memory slot).
 template <int R, int NW>
-__device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
+__device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW, kAdjRing>& c, int s, int rk0, int rk1,
                                           int entx, int t)
 {
-  using L = RegTile<R, NW, 3>;
+  using L = RegTile<R, NW, kAdjRing>;
   if (a.n_hi - t >= a.nt) return;
   if (entx >= 0) atomicAdd(c.rowbuf_() + entx, c.priv_()[t]);          // coincident receivers sum
   if (rk1 - rk0 > L::THREADS)                                                // more receivers than threads
@@ -56,63 +75,72 @@ __device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW,
     }
 }
 
-// owned rows of forward plane Ez^{n_hi - t} -> slot t % 3 of the thread's history ring (one commit group)
+// The forward Ez planes a CTA reads form one stream: planes 0 .. nsub of its first shot (plane t =
+// Ez^{n_hi - t}), then those of its next shot, and so on.  Stream position `pos` lands in slot pos % kAdjRing
+// of the history ring; the mbarrier of a slot completes once per fetch into it, so the fetch at position pos
+// is awaited with parity (pos / kAdjRing) & 1.  Step t of the shot whose plane 0 sits at position q0 reads
+// positions q0 + t and q0 + t + 1 and has position q0 + t + kAdjRing - 1 fetched (a shot has one plane more
+// than it has steps: position q0 + kAdjRing - 2 is fetched when the shot begins), so the first plane(s) of
+// the next shot are in flight during the last step(s) of this one.  ONE thread issues the copy (TMA: box = 128 columns x the owned rows, placed at the
+// owned rows of the slot; cells outside the grid arrive as zeros); it does so right after a CTA barrier that
+// follows every thread's last read of the slot's previous contents (position pos - kAdjRing).
 template <int R, int NW>
-__device__ __forceinline__ void adj_fetch(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int t)
+__device__ __forceinline__ void adj_fetch(const AdjArgs& a, const TileCtx<R, NW, kAdjRing>& c, int s, int s_end, int q0, int pos)
 {
-  using L = RegTile<R, NW, 3>;
-  if (t <= a.nsub) {
-    const float* src = a.ez_planes[t] + s * a.g.plane + (long long)c.gj0 * a.g.pitch + c.gi;
-    float* dst = c.hist_() + (t % 3) * (L::ROWS * kRegW);
-#pragma unroll
-    for (int r = 0; r < R; ++r)
-      if ((c.own >> r) & 1u) cp_async16(dst + r * kRegW, src + (long long)r * a.g.pitch);
-  }
+  using L = RegTile<R, NW, kAdjRing>;
+  int t = pos - q0;
+  if (t > a.nsub) { t -= a.nsub + 1; ++s; }             // a plane of the next shot
+  if (s >= s_end) return;
+  const unsigned bar = smem_u32(c.sm + L::MBAR) + 8u * (unsigned)(pos % kAdjRing);
+  mbar_expect_tx(bar, (unsigned)(a.oz * kRegW * sizeof(float)));
+  tma_load_3d(smem_u32(c.sm + L::HIST + (pos % kAdjRing) * (L::ROWS * kRegW) + a.hz * kRegW), &a.tm_own, c.ri0,
+              c.rj0 + a.hz, a.ez_pl[t] + s, bar);
+}
+template <int R, int NW>
+__device__ __forceinline__ void adj_await(const TileCtx<R, NW, kAdjRing>& c, int pos)
+{
+  using L = RegTile<R, NW, kAdjRing>;
+  mbar_wait(smem_u32(c.sm + L::MBAR) + 8u * (unsigned)(pos % kAdjRing), (unsigned)(pos / kAdjRing) & 1u);
 }
 
-// A warp that touches no CPML never uses its thread-private psi slots: they serve as the landing zone for
-// the NEXT shot's adjoint state (field f: 0 lamE, 1 lamHx, 2 lamHy), fetched while this shot is stepped, so
-// that the next shot does not start with the state loads exposed.
+// A CTA that touches no CPML never uses the psi region of its shared memory: it serves as the landing zone
+// [3][ROWS][128] for the NEXT shot's adjoint state (lamE, lamHx, lamHy: three TMA boxes of the whole region
+// on mbarrier kAdjRing), fetched while this shot is stepped, so that the next shot does not start with its state
+// loads exposed.
 template <int R, int NW>
-__device__ __forceinline__ float* adj_land(const TileCtx<R, NW, 3>& c, int f)
+__device__ __forceinline__ void adj_prefetch_state(const AdjArgs& a, const TileCtx<R, NW, kAdjRing>& c, int s_next)
 {
-  return f == 0 ? c.phz_() : (f == 1 ? c.pez_() : c.phx_());
-}
-template <int R, int NW>
-__device__ __forceinline__ void adj_prefetch_state(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s_next, int f)
-{
-  const float* src = (f == 0 ? a.in.ez : (f == 1 ? a.in.hx : a.in.hy)) + s_next * a.g.plane + (long long)c.gj0 * a.g.pitch + c.gi;
-  float* dst = adj_land<R, NW>(c, f);
+  using L = RegTile<R, NW, kAdjRing>;
+  const unsigned bar = smem_u32(c.sm + L::MBAR) + 8u * kAdjRing;
+  mbar_expect_tx(bar, (unsigned)(3 * L::ROWS * kRegW * sizeof(float)));
 #pragma unroll
-  for (int r = 0; r < R; ++r)
-    if (c.colin && ((c.rin >> r) & 1u)) cp_async16(dst + r * kRegW, src + (long long)r * a.g.pitch);
+  for (int f = 0; f < 3; ++f)
+    tma_load_3d(smem_u32(c.sm + L::LAND + f * (L::ROWS * kRegW)), &a.tm_reg, c.ri0, c.rj0, a.in_pl[f] + s_next, bar);
 }
 
 // The T reverse steps of one warp for one shot; ZP / XP as in fwd_steps (the psi forms below give
 // exactly tx = q, tz = -q, sx, sz = +-Db lamH with the trivial coefficients outside the CPML).
 // Packed pairs as in the forward kernel: P = (c0, c2), Q = (c1, c3).
 template <int R, int NW, bool ZP, bool XP>
-__device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
-                                          int entx, unsigned iflags, bool prefetch,
+__device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW, kAdjRing>& c, int s, int rk0, int rk1,
+                                          int entx, unsigned iflags, bool prefetch, int q0, int s_end,
                                           P2 (&le)[R], P2 (&lhx)[R], P2 (&lhy)[R], const P2 (&ca)[R], const P2 (&cb)[R],
                                           P2 (&ga)[R], P2 (&gb)[R])
 {
-  using L = RegTile<R, NW, 3>;
+  using L = RegTile<R, NW, kAdjRing>;
   const unsigned full = 0xffffffffu;
   const u64 rdx2 = bc2(a.g.rdx), Db2 = bc2(a.g.Db), nDb2 = bc2(-a.g.Db);
 #pragma unroll 1
   for (int t = 0; t < a.nsub; ++t) {
     // ---- [A] adjoint source, gradient terms ------------------------------------------------------
-    adj_fetch<R, NW>(a, c, s, t + 2);                   // two steps ahead; planes t and t+1 have landed after the wait
-    if (prefetch) {                                     // next shot's state, one field per step, in the same commit group
-      if (t < 3) adj_prefetch_state<R, NW>(a, c, s + 1, t);
-      if (t + 1 == a.nsub)
-        for (int f = t + 1; f < 3; ++f) adj_prefetch_state<R, NW>(a, c, s + 1, f);
+    if (threadIdx.x == 0) {                             // (every thread is past the previous step's barriers)
+      adj_fetch<R, NW>(a, c, s, s_end, q0, q0 + t + kAdjRing - 1);           // kAdjRing - 1 positions ahead
+      if (t == 0 && prefetch) adj_prefetch_state<R, NW>(a, c, s + 1);
     }
-    cp_async_commit();
-    cp_async_wait<1>();
-    const float* h1 = c.hist_() + (t % 3) * (L::ROWS * kRegW);
-    const float* h0 = c.hist_() + ((t + 1) % 3) * (L::ROWS * kRegW);
+    if (t == 0) adj_await<R, NW>(c, q0);                // planes t and t + 1 (plane t was awaited a step ago)
+    adj_await<R, NW>(c, q0 + t + 1);
+    const float* h1 = c.hist_() + ((q0 + t) % kAdjRing) * (L::ROWS * kRegW);
+    const float* h0 = c.hist_() + ((q0 + t + 1) % kAdjRing) * (L::ROWS * kRegW);
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       if ((iflags >> r) & 1u) {
@@ -121,8 +149,8 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
         le[r].p = add2(le[r].p, v.p); le[r].q = add2(le[r].q, v.q);
         st2(rb, zero2());
       }
-      {                                                 // (every thread: the ring slots of cells the tile does not own
-                                                        //  are never fetched into and stay zero, so they add nothing)
+      {                                                 // (every thread: what the accumulators of cells the tile does not
+                                                        //  own collect is never flushed)
         const P2 e0 = ld2(h0 + r * kRegW), e1 = ld2(h1 + r * kRegW);      // E^n, E^{n+1}
         ga[r].p = fma2(le[r].p, e0.p, ga[r].p); ga[r].q = fma2(le[r].q, e0.q, ga[r].q);
         gb[r].p = fma2(le[r].p, fma2(neg2(ca[r].p), e0.p, e1.p), gb[r].p);
@@ -215,19 +243,25 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
       le[0].p = fma2(rdx2, sub2(sza.p, sz0.p), le[0].p);
       le[0].q = fma2(rdx2, sub2(sza.q, sz0.q), le[0].q);
     }
+    GPR_PROBE(s % a.group, 4 + t);
   }
 }
 
 template <int R, int NW, int MINB>
-__global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
+__global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const __grid_constant__ AdjArgs a)
 {
-  using L = RegTile<R, NW, 3>;
-  extern __shared__ float4 smem4[];
+  using L = RegTile<R, NW, kAdjRing>;
+  extern __shared__ __align__(128) float4 smem4[];
   const Geo& g = a.g;
-  TileCtx<R, NW, 3> c;
+  TileCtx<R, NW, kAdjRing> c;
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
   const int grp = blockIdx.z, tile = blockIdx.y * a.tiles_x + blockIdx.x;
   pdl_launch_dependents();
+  if (threadIdx.x == 0) {              // mbarriers 0 .. kAdjRing-1: history ring slots, kAdjRing: state landing zone
+#pragma unroll
+    for (int k = 0; k <= kAdjRing; ++k) mbar_init(smem_u32(c.sm + L::MBAR) + 8u * k, 1u);
+    mbar_init_fence();
+  }
   // per-shot scalars of the whole group (static input: nothing a previous launch writes), word k of 4:
   // receiver range [rk0, rk1) of the region, 64-bit mask of the region rows that hold a receiver
   const int s_beg = grp * a.group, s_end = min((grp + 1) * a.group, a.nshots);
@@ -241,7 +275,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
     reinterpret_cast<float4*>(c.rowbuf_())[k] = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-  for (int k = 0; k < 3 * R; ++k)      // the thread's own slots of the Ez-history ring (see [A])
+  for (int k = 0; k < kAdjRing * R; ++k)      // the thread's own slots of the Ez-history ring (rows the copies never fill)
     st2(c.hist_() + (k / R) * (L::ROWS * kRegW) + (k % R) * kRegW, zero2());
 
   P2 ca[R], cb[R], ga[R], gb[R];
@@ -254,7 +288,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
       cb[r] = ldg2(a.cb + o);
     }
   }
-  __syncthreads();                     // the group's scalars are visible
+  // a CTA none of whose warps touches the CPML lands the next shot's state in the (unused) psi region
+  const bool can_land = g.P > 0 && !__syncthreads_or((c.zp || c.xp) ? 1 : 0);      // (barrier: the group's scalars are visible)
   // the receiver this thread injects (receivers of the region are dealt out one per thread); fetched one
   // shot ahead into the thread's private slot so that no shot starts with a chain of dependent loads
   {
@@ -264,24 +299,31 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
   }
 
   pdl_wait();                          // everything below reads what the previous launch wrote
-  const bool can_land = g.P > 0 && !(c.zp || c.xp);     // (warp-uniform; the psi slots exist only when npml > 0)
   bool landed = false;
-  for (int s = s_beg; s < s_end; ++s) {
+  int q0 = 0, nland = 0;               // stream position of this shot's plane 0; state landings so far
+  for (int s = s_beg; s < s_end; ++s, q0 += a.nsub + 1) {
     // ---- everything this shot needs from global memory, issued together ----------------------------
+    GPR_PROBE(s - s_beg, 0);
     const int* m = c.meta_() + (s - s_beg) * 4;
     const int rk0 = m[0], rk1 = m[1];
     const unsigned iflags = (unsigned)((((unsigned long long)(unsigned)m[3] << 32) | (unsigned)m[2]) >> c.lr0) & ((1u << R) - 1u);
     const int2 ent = *reinterpret_cast<const int2*>(c.priv_() + 4);
     P2 le[R], lhx[R], lhy[R];
-    if (landed) cp_async_wait<0>();    // this shot's state was fetched into the warp's landing slots during the previous one
+    if (threadIdx.x == 0) {            // (every thread is past the last barrier of the previous shot; planes
+                                       //  0 .. kAdjRing - 3 of a later shot came during the previous shot's last steps)
+      for (int k = (s == s_beg ? 0 : kAdjRing - 2); k < kAdjRing - 1; ++k) adj_fetch<R, NW>(a, c, s, s_end, q0, q0 + k);
+    }
+    if (landed) {                      // this shot's state was fetched into the landing zone during the previous one
+      mbar_wait(smem_u32(c.sm + L::MBAR) + 8u * kAdjRing, (unsigned)(nland - 1) & 1u);
+    }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       le[r] = zero2(); lhx[r] = zero2(); lhy[r] = zero2();
       if (c.colin && ((c.rin >> r) & 1u)) {
         if (landed) {
-          le[r] = ld2(adj_land<R, NW>(c, 0) + r * kRegW);
-          lhx[r] = ld2(adj_land<R, NW>(c, 1) + r * kRegW);
-          lhy[r] = ld2(adj_land<R, NW>(c, 2) + r * kRegW);
+          le[r] = ld2(c.sm + L::LAND + 0 * (L::ROWS * kRegW) + c.toff + r * kRegW);
+          lhx[r] = ld2(c.sm + L::LAND + 1 * (L::ROWS * kRegW) + c.toff + r * kRegW);
+          lhy[r] = ld2(c.sm + L::LAND + 2 * (L::ROWS * kRegW) + c.toff + r * kRegW);
         } else {
           const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
           le[r] = ldcg2(a.in.ez + o);  // (written by the previous launch: not through the read-only path)
@@ -290,12 +332,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
         }
       }
     }
+    GPR_PROBE(s - s_beg, 1);
     const bool prefetch = can_land && s + 1 < s_end;
-    adj_fetch<R, NW>(a, c, s, 0);
-    cp_async_commit();
-    adj_fetch<R, NW>(a, c, s, 1);
-    cp_async_commit();
-    c.fetch_psi(g, a.in, s);           // lands with the history planes: step 0 waits for all but the newest group
+    c.fetch_psi(g, a.in, s);           // (one cp.async group, awaited before the barrier below)
     // this thread's residual samples of this launch, and the receiver it injects for the next shot
     float rv[kMaxT];
 #pragma unroll
@@ -311,12 +350,15 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
     *reinterpret_cast<int2*>(c.priv_() + 4) = ent_next;
     const int entx = ent.x;
     adj_stage<R, NW>(a, c, s, rk0, rk1, entx, 0);         // (the previous shot left rowbuf all zero, two barriers ago)
+    GPR_PROBE(s - s_beg, 2);
+    cp_async_wait<0>();
     __syncthreads();
+    GPR_PROBE(s - s_beg, 3);
 
-    if (c.zp && c.xp) adj_steps<R, NW, true, true>(a, c, s, rk0, rk1, entx, iflags, prefetch, le, lhx, lhy, ca, cb, ga, gb);
-    else if (c.zp) adj_steps<R, NW, true, false>(a, c, s, rk0, rk1, entx, iflags, prefetch, le, lhx, lhy, ca, cb, ga, gb);
-    else if (c.xp) adj_steps<R, NW, false, true>(a, c, s, rk0, rk1, entx, iflags, prefetch, le, lhx, lhy, ca, cb, ga, gb);
-    else adj_steps<R, NW, false, false>(a, c, s, rk0, rk1, entx, iflags, prefetch, le, lhx, lhy, ca, cb, ga, gb);
+    if (c.zp && c.xp) adj_steps<R, NW, true, true>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb);
+    else if (c.zp) adj_steps<R, NW, true, false>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb);
+    else if (c.xp) adj_steps<R, NW, false, true>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb);
+    else adj_steps<R, NW, false, false>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb);
 
     // ---- write back the owned part of the adjoint state ------------------------------------------------
 #pragma unroll
@@ -329,6 +371,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const AdjArgs a)
     }
     if (c.zp || c.xp) c.store_psi(g, a.out, s);
     landed = prefetch;
+    nland += prefetch ? 1 : 0;
+    GPR_PROBE(s - s_beg, 8);
   }
 
   // ---- once per CTA: add the register partial sums to this group's gCa / gCb planes --------------------

@@ -204,9 +204,9 @@ __device__ __forceinline__ void fwd_fetch(const FwdArgs& a, const TileCtx<R, NW,
   for (int r = 0; r < R; ++r)
     if (c.colin && ((c.rin >> r) & 1u)) {
       const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-      cp_async16(c.hist_() + 0 * L::ROWS * kRegW + r * kRegW, a.in.ez + o);
-      cp_async16(c.hist_() + 1 * L::ROWS * kRegW + r * kRegW, a.in.hx + o);
-      cp_async16(c.hist_() + 2 * L::ROWS * kRegW + r * kRegW, a.in.hy + o);
+      cp_async16(c.fland_() + 0 * L::ROWS * kRegW + r * kRegW, a.in.ez + o);
+      cp_async16(c.fland_() + 1 * L::ROWS * kRegW + r * kRegW, a.in.hx + o);
+      cp_async16(c.fland_() + 2 * L::ROWS * kRegW + r * kRegW, a.in.hy + o);
     }
   cp_async_commit();
 }
@@ -269,9 +269,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
     for (int r = 0; r < R; ++r) {
       e[r] = zero2(); hx[r] = zero2(); hy[r] = zero2();
       if (c.colin && ((c.rin >> r) & 1u)) {
-        e[r] = ld2(c.hist_() + 0 * L::ROWS * kRegW + r * kRegW);
-        hx[r] = ld2(c.hist_() + 1 * L::ROWS * kRegW + r * kRegW);
-        hy[r] = ld2(c.hist_() + 2 * L::ROWS * kRegW + r * kRegW);
+        e[r] = ld2(c.fland_() + 0 * L::ROWS * kRegW + r * kRegW);
+        hx[r] = ld2(c.fland_() + 1 * L::ROWS * kRegW + r * kRegW);
+        hy[r] = ld2(c.fland_() + 2 * L::ROWS * kRegW + r * kRegW);
       }
     }
     // this warp's R bits of the mask of region rows that hold a receiver of this shot

@@ -24,10 +24,14 @@
 //                     mask of the region rows that hold a receiver), loaded once per CTA
 //   priv [THREADS][8]  thread-private scalars (adjoint: the thread's residual samples of this launch, its receiver
 //                     entry for the next shot)
-//   hist [NH][NW*R][128] thread-private cp.async landing zone: adjoint = ring of forward Ez planes fetched two
-//                     steps ahead; forward = Ez, Hx, Hy of the NEXT shot fetched while this one is stepped
+//   mbar [8]          mbarriers of the TMA copies
+//   hist [NH][NW*R][128] landing zone, rows x 128 columns of the region like the registers: adjoint = ring of
+//                     forward Ez planes (owned rows) fetched two steps ahead by TMA; forward = Ez, Hx, Hy of the
+//                     NEXT shot fetched by cp.async while this one is stepped
 //   psi  [4][NW*R][128]  CPML psi of the region, thread-private (only when npml > 0): hz ez hx ex
 #pragma once
+#include <cuda.h>          // CUtensorMap (type only; the encoder is fetched through the runtime)
+
 #include "gprfwi_common.cuh"
 
 namespace gprfwi {
@@ -44,6 +48,10 @@ constexpr int kRegW = 128;     // region width  = 32 lanes x float4
 constexpr int kOwnW = 120;     // owned width   = lanes 1..30
 constexpr int kMaxGroup = 32;  // shots one CTA sweeps at most (size of the per-shot scalar table in shared memory)
 constexpr int kMetaW = 12;     // words per shot in that table
+#ifndef GPRFWI_ADJ_RING
+#define GPRFWI_ADJ_RING 4
+#endif
+constexpr int kAdjRing = GPRFWI_ADJ_RING;   // slots of the adjoint's ring of forward Ez planes (3: 275.6, 4: 286.3 Gcell-updates/s on config 4)
 
 template <int R, int NW, int NH = 0>
 struct RegTile {
@@ -56,8 +64,10 @@ struct RegTile {
   static constexpr int TABZ = TABX + 6 * kRegW;
   static constexpr int META = TABZ + 6 * ROWS;                 // kMaxGroup x kMetaW words: per-shot scalars of the CTA's group
   static constexpr int PRIV = META + kMetaW * kMaxGroup;       // THREADS x 8 words, thread-private (adjoint: residual samples, next receiver)
-  static constexpr int HIST = (PRIV + 8 * THREADS + 31) / 32 * 32 + GPRFWI_SMEM_PAD;
-  static constexpr int PSI = HIST + NH * ROWS * kRegW;
+  static constexpr int MBAR = (PRIV + 8 * THREADS + 1) / 2 * 2;  // 8 mbarriers (8 bytes each) for the TMA copies
+  static constexpr int HIST = (MBAR + 16 + 31) / 32 * 32;      // 128-byte aligned: TMA destination
+  static constexpr int LAND = HIST + NH * ROWS * kRegW + 32;   // 128-byte aligned: the psi region doubles as a TMA landing zone
+  static constexpr int PSI = LAND + GPRFWI_SMEM_PAD;
   GPR_HD static size_t smem_bytes(bool pml) { return sizeof(float) * (size_t)(PSI + (pml ? 4 * ROWS * kRegW : 0)); }
 };
 
@@ -133,6 +143,38 @@ __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepc
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void zero4(float* v) { v[0] = v[1] = v[2] = v[3] = 0.f; }
 
+// ---- TMA (cp.async.bulk.tensor) + mbarrier: one elected thread copies a whole [rows][128] box of a field
+// plane into shared memory; the copy engine does the addressing, the bounds handling (cells outside the
+// grid arrive as zeros) and the transfer, and no thread spends load/store-pipe issue slots on it.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_init_fence() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// box of the 3-D tensor (x = column, y = row, z = plane of the workspace) -> shared memory, completing on `bar`
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map, int x, int y, int z, unsigned bar)
+{
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+               ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar) : "memory");
+}
+
 // Per-thread view of the region: where this lane's 4 columns and this warp's R rows sit in the grid,
 // which of them carry CPML psi, and the shared-memory carve-up.
 template <int R, int NW, int NH = 0>
@@ -158,6 +200,8 @@ struct TileCtx {
   __device__ __forceinline__ int* meta_() const { return reinterpret_cast<int*>(sm + L::META); }
   __device__ __forceinline__ float* priv_() const { return sm + L::PRIV + 8 * threadIdx.x; }
   __device__ __forceinline__ float* hist_() const { return sm + L::HIST + toff; }
+  // the forward kernel's thread-private cp.async landing slots: the same region, shifted (see GPRFWI_SMEM_PAD)
+  __device__ __forceinline__ float* fland_() const { return sm + L::HIST + GPRFWI_SMEM_PAD + toff; }
   __device__ __forceinline__ float* phz_() const { return sm + L::PSI + 0 * L::ROWS * kRegW + toff; }
   __device__ __forceinline__ float* pez_() const { return sm + L::PSI + 1 * L::ROWS * kRegW + toff; }
   __device__ __forceinline__ float* phx_() const { return sm + L::PSI + 2 * L::ROWS * kRegW + toff; }
