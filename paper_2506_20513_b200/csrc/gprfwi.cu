@@ -664,6 +664,10 @@ static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, 
   a.out = out;
   a.ca = h->c.ca;
   a.cb = h->c.cb;
+  a.tm_reg = h->tm_fwd_reg;
+  a.in_pl[0] = (int)((in.ez - h->c.ca) / (long long)L.plane);
+  a.in_pl[1] = (int)((in.hx - h->c.ca) / (long long)L.plane);
+  a.in_pl[2] = (int)((in.hy - h->c.ca) / (long long)L.plane);
   // planes for Ez after steps 1 .. nsub-1 of this launch: consecutive at a fixed stride in every plan
   a.ez_mid = nsub > 1 ? ez_of(n + 1) : nullptr;
   a.ez_mid_stride = (a.ez_mid && nsub > 2) ? (long long)(ez_of(n + 2) - ez_of(n + 1)) : 0;

@@ -47,10 +47,14 @@ struct AdjArgs {
 // Tuning aid (builds with -DGPRFWI_PROBE only): clock64 stamps of every warp of one interior CTA at fixed
 // points of each shot, read back with gprfwi_probe_read (gprfwi.cu).
 #ifdef GPRFWI_PROBE
+#ifndef GPRFWI_PROBE_BX
+#define GPRFWI_PROBE_BX (gridDim.x / 2)
+#define GPRFWI_PROBE_BY (gridDim.y / 2)
+#endif
 __device__ long long g_probe[kMaxGroup][16][12];
 #define GPR_PROBE(shot, k)                                                                          \
   do {                                                                                              \
-    if (blockIdx.x == gridDim.x / 2 && blockIdx.y == gridDim.y / 2 && blockIdx.z == 0 && (threadIdx.x & 31) == 0) \
+    if (blockIdx.x == GPRFWI_PROBE_BX && blockIdx.y == GPRFWI_PROBE_BY && blockIdx.z == 0 && (threadIdx.x & 31) == 0) \
       g_probe[(shot)][threadIdx.x >> 5][(k)] = clock64();                                           \
   } while (0)
 #else

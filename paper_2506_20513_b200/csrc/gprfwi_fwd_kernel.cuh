@@ -22,6 +22,9 @@
 namespace gprfwi {
 
 struct FwdArgs {
+  // TMA view of the workspace as one 3-D array of planes (gprfwi_adj_kernel.cuh), box = 128 columns x the region's rows
+  alignas(64) CUtensorMap tm_reg;
+  int in_pl[3];               // workspace plane indices of in.ez, in.hx, in.hy (local shot 0)
   Geo g;
   State in, out;              // out.ez: Ez plane after the last step of this launch
   const float *ca, *cb;       // [nz][pitch], 0 on the PEC ring, in PEC cells and in the pitch padding
@@ -194,28 +197,24 @@ __device__ __forceinline__ int fwd_meta_word(const FwdArgs& a, int s, int tile, 
   return 0;
 }
 
-// Ez, Hx, Hy of shot s (this thread's cells) -> the thread's landing slots, one commit group
+// Ez, Hx, Hy of shot s (the whole region) -> the CTA's landing zone [3][ROWS][128], three TMA boxes issued by
+// ONE thread and completing on mbarrier 0; cells outside the grid arrive as zeros
 template <int R, int NW>
 __device__ __forceinline__ void fwd_fetch(const FwdArgs& a, const TileCtx<R, NW, 3>& c, int s)
 {
   using L = RegTile<R, NW, 3>;
-  const Geo& g = a.g;
+  const unsigned bar = smem_u32(c.sm + L::MBAR);
+  mbar_expect_tx(bar, (unsigned)(3 * L::ROWS * kRegW * sizeof(float)));
 #pragma unroll
-  for (int r = 0; r < R; ++r)
-    if (c.colin && ((c.rin >> r) & 1u)) {
-      const long long o = s * g.plane + (long long)(c.gj0 + r) * g.pitch + c.gi;
-      cp_async16(c.fland_() + 0 * L::ROWS * kRegW + r * kRegW, a.in.ez + o);
-      cp_async16(c.fland_() + 1 * L::ROWS * kRegW + r * kRegW, a.in.hx + o);
-      cp_async16(c.fland_() + 2 * L::ROWS * kRegW + r * kRegW, a.in.hy + o);
-    }
-  cp_async_commit();
+  for (int f = 0; f < 3; ++f)
+    tma_load_3d(smem_u32(c.sm + L::HIST + f * (L::ROWS * kRegW)), &a.tm_reg, c.ri0, c.rj0, a.in_pl[f] + s, bar);
 }
 
 template <int R, int NW, int MINB>
-__global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
+__global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const __grid_constant__ FwdArgs a)
 {
   using L = RegTile<R, NW, 3>;
-  extern __shared__ float4 smem4[];
+  extern __shared__ __align__(128) float4 smem4[];
   const Geo& g = a.g;
   TileCtx<R, NW, 3> c;
   c.init(reinterpret_cast<float*>(smem4), g, blockIdx.x, blockIdx.y, a.oz, a.hz);
@@ -226,6 +225,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
   // once per CTA, overlapping the previous launch's tail: CPML tables -> shared memory, Ca / Cb of the
   // region -> registers; then, once the previous launch's state is complete, the first shot's fields
   pdl_launch_dependents();
+  if (tid == 0) {
+    mbar_init(smem_u32(c.sm + L::MBAR), 1u);
+    mbar_init_fence();
+  }
   for (int k = tid; k < kMetaW * (s1 - s0); k += L::THREADS)
     c.meta_()[k] = fwd_meta_word(a, s0 + k / kMetaW, tile, ntile, k % kMetaW);
   c.template stage_tables<true>(g);
@@ -240,9 +243,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
       cb[r] = ldg2(a.cb + o);
     }
   }
+  __syncthreads();                     // mbarrier initialised, tables and the group's scalars visible
   pdl_wait();
-  fwd_fetch<R, NW>(a, c, s0);
-  __syncthreads();
+  if (tid == 0) fwd_fetch<R, NW>(a, c, s0);
   // the receiver this thread records (receivers of the tile are dealt out one per thread)
   int2 ent_next = make_int2(-1, 0);
   if (c.meta_()[0] + tid < c.meta_()[1]) ent_next = a.blk_ent[(long long)s0 * a.nrec + c.meta_()[0] + tid];
@@ -263,16 +266,13 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
     }
     // ---- this shot's fields have landed in the thread's slots: move them to registers ---------------
     P2 e[R], hx[R], hy[R];
-    c.fetch_psi(g, a.in, s);           // (the previous shot's psi went out in its store_psi)
-    cp_async_wait<1>();                // fields: landed; psi: on its way
+    c.fetch_psi(g, a.in, s);           // (one cp.async group; the previous shot's psi went out in its store_psi)
+    mbar_wait(smem_u32(c.sm + L::MBAR), (unsigned)(s - s0) & 1u);      // this shot's fields have landed
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      e[r] = zero2(); hx[r] = zero2(); hy[r] = zero2();
-      if (c.colin && ((c.rin >> r) & 1u)) {
-        e[r] = ld2(c.fland_() + 0 * L::ROWS * kRegW + r * kRegW);
-        hx[r] = ld2(c.fland_() + 1 * L::ROWS * kRegW + r * kRegW);
-        hy[r] = ld2(c.fland_() + 2 * L::ROWS * kRegW + r * kRegW);
-      }
+    for (int r = 0; r < R; ++r) {      // (cells outside the grid arrived as zeros)
+      e[r] = ld2(c.hist_() + 0 * L::ROWS * kRegW + r * kRegW);
+      hx[r] = ld2(c.hist_() + 1 * L::ROWS * kRegW + r * kRegW);
+      hy[r] = ld2(c.hist_() + 2 * L::ROWS * kRegW + r * kRegW);
     }
     // this warp's R bits of the mask of region rows that hold a receiver of this shot
     const unsigned rflags = (unsigned)((((unsigned long long)(unsigned)m[9] << 32) | (unsigned)m[8]) >> c.lr0) & ((1u << R) - 1u);
@@ -283,16 +283,16 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const FwdArgs a)
       for (int r = 0; r < R; ++r)
         if ((rflags >> r) & 1u) st2(c.rowbuf_() + (c.lr0 + r) * kRegW + c.l4, e[r]);
     }
-    // ---- next shot: fields into the (now free) landing slots; the receiver it records -----------------
-    if (s + 1 >= s1) cp_async_commit();   // (keeps the group count uniform: psi is always the second newest)
+    // ---- next shot: the receiver this thread records; its fields into the landing zone once every thread
+    // has taken this shot's out of it
     ent_next = make_int2(-1, 0);
     if (s + 1 < s1) {
-      fwd_fetch<R, NW>(a, c, s + 1);
       const int* mn = m + kMetaW;
       if (mn[0] + tid < mn[1]) ent_next = a.blk_ent[(long long)(s + 1) * a.nrec + mn[0] + tid];
     }
-    cp_async_wait<1>();                // psi landed (the next shot's fields may still be in flight)
-    __syncthreads();                   // exchange row and receiver rows published
+    cp_async_wait<0>();                // psi landed
+    __syncthreads();                   // exchange row and receiver rows published; landing zone free
+    if (tid == 0 && s + 1 < s1) fwd_fetch<R, NW>(a, c, s + 1);
 
     if (c.zp && c.xp) fwd_steps<R, NW, true, true>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
     else if (c.zp) fwd_steps<R, NW, true, false>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
