@@ -17,7 +17,14 @@ from paper_2506_20513_b200 import (GprfwiError, Simulation, gprfwi_gradient_host
 
 pytestmark = pytest.mark.gpu
 
-TOL_TRACE, TOL_GRAD = 1e-4, 1e-3
+# north_star's bars are 1e-4 (traces) and 1e-3 (gradients) over the whole array.  Asserted here: 1e-4 on both
+# (measured on B200: traces <= 4e-6, gradients <= 3e-5), and -- because a gradient spans many decades and the
+# near-source cells dominate a whole-array norm -- the same relative L2 inside each region a bug could hide in
+# (CPML strips, the cells around every tile seam, the ring-adjacent cells, the far field), plus the largest
+# absolute error against the largest value.  DESIGN.md section 6 lists the measured per-region numbers.
+TOL_TRACE, TOL_GRAD = 1e-4, 1e-4
+TOL_REGION, TOL_MAXABS = 1e-3, 1e-4
+TILE_OZ, TILE_OX = 28, 120          # owned rows / columns of a tile in the default kernel shape
 
 
 def dev():
@@ -63,7 +70,50 @@ def oracle_all(wl, residual=None, with_obs=False):
     return tr, residual, ge, gs
 
 
-def assert_parity(wl, got, ref, tag=""):
+def regions(wl):
+    """Boolean masks of the full grid where a localised error would hide under a whole-array norm."""
+    nz, nx, P = wl.nz, wl.nx, wl.npml
+    j = np.arange(nz)[:, None] * np.ones((1, nx), dtype=np.int64)
+    i = np.ones((nz, 1), dtype=np.int64) * np.arange(nx)[None, :]
+    out = {}
+    if P > 0:
+        out["cpml-top"], out["cpml-bottom"] = j < P, j >= nz - P
+        out["cpml-left"], out["cpml-right"] = i < P, i >= nx - P
+    dj = np.minimum(j % TILE_OZ, TILE_OZ - j % TILE_OZ)
+    di = np.minimum(i % TILE_OX, TILE_OX - i % TILE_OX)
+    seam_z = (dj <= 4) & (j >= TILE_OZ - 4) & (j <= (nz - 1) // TILE_OZ * TILE_OZ + 4)
+    seam_x = (di <= 4) & (i >= TILE_OX - 4) & (i <= (nx - 1) // TILE_OX * TILE_OX + 4)
+    if seam_z.any():
+        out["tile-seams-z"] = seam_z
+    if seam_x.any():
+        out["tile-seams-x"] = seam_x
+    out["ring-adjacent"] = (j == 1) | (j == nz - 2) | (i == 1) | (i == nx - 2)
+    far = np.ones((nz, nx), bool)                      # farther than a third of the grid from every source and receiver
+    rad = max(nz, nx) // 3
+    pts = np.concatenate([wl.src_zx.reshape(-1, 2), wl.rec_zx.reshape(-1, 2)])
+    for z, x in np.unique(pts, axis=0):
+        far[max(z - rad, 0):z + rad + 1, max(x - rad, 0):x + rad + 1] = False
+    far &= (j >= P) & (j < nz - P) & (i >= P) & (i < nx - P)
+    if far.any():
+        out["far-field"] = far
+    return out
+
+
+def region_report(wl, g, g_o, name):
+    """rel-L2 of a gradient inside each region and the scaled max-abs error.  Regions where the oracle's
+    gradient stays below 1e-5 of its peak are left to the max-abs bound: fp32 sums whose terms are of the
+    peak's size cannot resolve such cells relative to themselves (ring-adjacent cells deep in the CPML)."""
+    rep = {}
+    peak = float(np.abs(g_o).max())
+    for key, m in regions(wl).items():
+        if np.abs(g_o[m]).max() > 1e-5 * peak:
+            rep[key] = rel_l2(g[m], g_o[m])
+    rep["max-abs/peak"] = float(np.abs(g.astype(np.float64) - g_o).max() / max(peak, 1e-300))
+    print(f"[regions] {wl.name} {name}: " + " ".join(f"{k} {v:.1e}" for k, v in rep.items()))
+    return rep
+
+
+def assert_parity(wl, got, ref, tag="", tol_region=None, tol_maxabs=None):
     tr, ge, gs = got
     tr_o, ge_o, gs_o = ref
     et, ee, es = rel_l2(tr, tr_o), rel_l2(ge, ge_o), rel_l2(gs, gs_o)
@@ -71,6 +121,9 @@ def assert_parity(wl, got, ref, tag=""):
     assert et <= TOL_TRACE, et
     assert ee <= TOL_GRAD, ee
     assert es <= TOL_GRAD, es
+    for name, g, g_o in (("grad_eps_r", ge, ge_o), ("grad_sigma", gs, gs_o)):
+        for key, v in region_report(wl, g, g_o, name).items():
+            assert v <= ((tol_maxabs or TOL_MAXABS) if key == "max-abs/peak" else (tol_region or TOL_REGION)), (name, key, v)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -100,7 +153,9 @@ def test_config1_end_to_end_residual_on_gpu():
     assert abs(misfit - 0.5 * np.sum(res_o.astype(np.float64) ** 2)) <= 2e-3 * misfit
     ee, es = rel_l2(ge, ge_o), rel_l2(gs, gs_o)
     print(f"[parity] config1 end-to-end: grad_eps_r {ee:.2e} grad_sigma {es:.2e} misfit {misfit:.6e}")
-    assert ee <= TOL_GRAD and es <= TOL_GRAD
+    # north_star's 1e-3: the residual is 1.7 % of the traces here, so the traces' 1e-6 becomes 6e-5 in the residual
+    # and about 4e-4 in the gradient; every other test gives both sides the same residual
+    assert ee <= 1e-3 and es <= 1e-3
 
 
 @pytest.mark.parametrize("shape", [(44, 52, 8), (70, 150, 10), (97, 263, 12), (40, 40, 0), (33, 129, 5),
@@ -274,7 +329,13 @@ def test_config2_full_launch_configuration_properties():
     assert rel_l2(tr[[0, 10, 19]], tr_o) <= TOL_TRACE
     t3, _, _, _ = run_gpu(sub)
     assert np.array_equal(t3, tr[[0, 10, 19]])
-    assert np.isfinite(ge).all() and np.isfinite(gs).all()
+    ge_sum, gs_sum = np.zeros_like(ge, dtype=np.float64), np.zeros_like(gs, dtype=np.float64)
+    for k in range(wl.nshots):
+        _, a, b, _ = run_gpu(wl.subset([k]), res[k:k + 1])
+        ge_sum += a; gs_sum += b
+    ea, eb = rel_l2(ge, ge_sum), rel_l2(gs, gs_sum)
+    print(f"[additivity] config 2: 20-shot batch vs sum of 20 one-shot runs: grad_eps_r {ea:.1e} grad_sigma {eb:.1e}")
+    assert ea < 1e-5 and eb < 1e-5
 
 
 def test_config3_checkpointed_subset_against_oracle():
@@ -582,3 +643,111 @@ def test_config3_full_launch_configuration_properties():
         _, a, b, _ = run_gpu(half, res[lo:hi], budget=budget)
         ga += a; gb += b
     assert rel_l2(ge, ga) <= 1e-5 and rel_l2(gs, gb) <= 1e-5
+
+
+# ------------------------------------------------------------------------------------------------
+# parity at the sizes bench.py times, in the plans it gets (SURVEY 8(c) "parity protocol":
+# a declared subset of shots with ALL nt and the full grid).  The whole batch runs at full nt with a residual
+# that is zero except on one shot, so the batch gradient IS that shot's gradient and is compared -- together
+# with that shot's traces -- with a one-shot oracle run at full nt.
+# ------------------------------------------------------------------------------------------------
+def _one_hot_residual_case(wl, shot, budget, oracle_stride, tol_local=None):
+    one = wl.subset([shot])
+    pb = problem(one)
+    rng = np.random.default_rng(1000 + shot)
+    res1 = rng.standard_normal((1, wl.nt, wl.nrec)).astype(np.float32)
+    res1[:, 0, :] = 0.0
+    ge_o, gs_o, tr_o = oracle.gradient(pb, one.eps_r, one.sigma, res1, checkpoint_stride=oracle_stride, want_traces=True)
+    res = np.zeros((wl.nshots, wl.nt, wl.nrec), dtype=np.float32)
+    res[shot] = res1[0]
+    tr, ge, gs, plan = run_gpu(wl, res, budget=budget)
+    print(f"[plan] {wl.name} one-hot shot {shot}:", plan)
+    assert_parity(one, (tr[shot:shot + 1], ge, gs), (tr_o, ge_o, gs_o), f" full nt, batch of {wl.nshots}, residual on shot {shot}",
+                  tol_region=tol_local, tol_maxabs=tol_local)
+    return plan
+
+
+def _bench_budget():
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()                  # (earlier tests' cached blocks would shrink the plan bench.py gets)
+    free, _ = torch.cuda.mem_get_info(dev())
+    return int(free * 0.9)
+
+
+@pytest.mark.parametrize("shot", [0, 59])
+def test_config3_full_nt_in_benchmarked_plan_against_oracle(shot):
+    """Config 3 as bench.py runs it (60 shots, nt = 4000, the plan the library picks for the free HBM:
+    checkpoint-and-recompute with stored tail segments, 3 lanes), first and last shot of the pass."""
+    plan = _one_hot_residual_case(gi.config3(), shot, _bench_budget(), oracle_stride=0)
+    assert plan["full_history"] == 0 and plan["shots_per_pass"] == 60
+
+
+def test_config4_full_nt_in_benchmarked_plan_against_oracle():
+    """Config 4 as bench.py runs it (100 shots, nt = 6000; sub-batched adjoint passes, K chosen by the plan):
+    the LAST shot of the first adjoint pass (the end of a lane's last CTA group) against a one-shot oracle run
+    at full nt (the oracle uses its own stride-100 checkpointing: its full history would be 105 GB)."""
+    wl = gi.config4()
+    budget = _bench_budget()
+    p = params_of(wl)
+    _, plan0 = gprfwi_workspace_bytes(p, budget)
+    assert plan0["full_history"] == 0 and 1 < plan0["shots_per_pass"] < wl.nshots
+    plan = _one_hot_residual_case(wl, plan0["shots_per_pass"] - 1, budget, oracle_stride=100)
+    assert plan == plan0
+
+
+def test_config5_512_full_nt_and_1024_batch32_against_oracle():
+    """Config 5 at its full nt = 1000: 512^2 with B = 8 (shots 0 and 7 against the oracle), and 1024^2 with
+    B = 32 in one call (one-hot residual on shot 31)."""
+    wl = gi.config5(n=512, batch=8)
+    sub = wl.subset([0, 7])
+    tr_o, res_sub, ge_o, gs_o = oracle_all(sub)
+    res = np.zeros((wl.nshots, wl.nt, wl.nrec), dtype=np.float32)
+    res[[0, 7]] = res_sub
+    tr, ge, gs, plan = run_gpu(wl, res)
+    assert plan["shots_per_pass"] == 8
+    # SURVEY's recipe for config 5 is a WHITE-NOISE residual: injected at a receiver 11 cells from a source of
+    # this strongly lossy i.i.d. medium it leaves single receiver cells 4e-4 of the peak off (the fp32
+    # wavefield, not the accumulation: runs with 2 and 4 fused steps agree to 3e-7 there, and the physical
+    # residual below is exact to 1e-6), so the whole-array bar holds and the local ones are 1e-3 here ...
+    assert_parity(sub, (tr[[0, 7]], ge, gs), (tr_o, ge_o, gs_o), " 512^2 B=8 full nt, white-noise residual",
+                  tol_region=1e-3, tol_maxabs=1e-3)
+    # ... and strict with a band-limited residual (the shots' own traces)
+    res[[0, 7]] = tr_o.astype(np.float32)
+    ge_o2, gs_o2 = oracle.gradient(problem(sub), sub.eps_r, sub.sigma, res[[0, 7]])
+    _, ge2, gs2, _ = run_gpu(wl, res)
+    assert_parity(sub, (tr[[0, 7]], ge2, gs2), (tr_o, ge_o2, gs_o2), " 512^2 B=8 full nt, residual = traces")
+    _one_hot_residual_case(gi.config5(n=1024, batch=32), 31, _bench_budget(), oracle_stride=0, tol_local=1e-3)
+
+
+def test_split_batch_multi_call_sum_against_oracle():
+    """bench.py sweeps a batch that does not fit one call as several calls through one workspace and sums the
+    gradients (split_batch picks the split): 512^2, B = 8, nt = 400 under a budget that forces more than
+    one call, summed as bench.py sums it, against the oracle's gradient of all 8 shots."""
+    from paper_2506_20513_b200 import split_batch
+    wl = gi.config5(n=512, batch=8, nt=400)
+    p = params_of(wl)
+    lo, hi = 1 << 20, gprfwi_workspace_bytes(p, 0)[0]               # smallest workspace the 8 shots fit in one call
+    while hi - lo > (1 << 16):
+        mid = (lo + hi) // 2
+        lo, hi = (lo, mid) if gprfwi_workspace_bytes(p, mid)[0] else (mid, hi)
+    budget = lo                                                     # ... and just below it: the batch must be split
+    assert gprfwi_workspace_bytes(p, budget)[0] == 0
+    ncalls, cs, plan = split_batch(p, budget)
+    print("[split]", ncalls, "calls of", cs, "shots:", plan)
+    assert ncalls > 1 and ncalls * cs == wl.nshots
+    tr_o, res, ge_o, gs_o = oracle_all(wl)
+    p.nshots = cs
+    sim = Simulation(p, wl.src_zx[:cs], wl.rec_zx[:cs], wl.wavelet, dev(), budget_bytes=budget)
+    e = torch.as_tensor(wl.eps_r, device=dev()); s_ = torch.as_tensor(wl.sigma, device=dev())
+    ge = torch.zeros_like(e); gs = torch.zeros_like(e)
+    tr = np.zeros_like(tr_o, dtype=np.float32)
+    for ci in range(ncalls):
+        sl = slice(ci * cs, (ci + 1) * cs)
+        sim.src_zx, sim.rec_zx = wl.src_zx[sl], wl.rec_zx[sl]
+        tr[sl] = sim.forward(e, s_).cpu().numpy()
+        a, b = sim.adjoint(torch.as_tensor(res[sl], device=dev()))
+        ge += a; gs += b
+    sim.close()
+    assert_parity(wl, (tr, ge.cpu().numpy(), gs.cpu().numpy()), (tr_o, ge_o, gs_o), f" {ncalls} calls of {cs} shots",
+                  tol_region=1e-3, tol_maxabs=1e-3)           # (white-noise residual on config 5: see above)
