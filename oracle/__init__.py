@@ -145,8 +145,17 @@ def cpml_profile(n, npml, order, sigma_max, kappa_max, alpha_max, dt, half):
     return b, c, ik
 
 
-def forward(pb: Problem, eps_r, sigma, want_ez_hist=False, want_h_hist=False):
-    """Algorithm 1.  Returns dict(traces[S][nt][R], ez_hist?, hx_hist?, hy_hist?)."""
+def _mu(pb, mu_r):
+    if mu_r is None:
+        return None
+    m = np.ascontiguousarray(mu_r, dtype=np.float64)
+    assert m.shape == (pb.nz, pb.nx)
+    return m
+
+
+def forward(pb: Problem, eps_r, sigma, want_ez_hist=False, want_h_hist=False, mu_r=None):
+    """Algorithm 1.  Returns dict(traces[S][nt][R], ez_hist?, hx_hist?, hy_hist?).
+    mu_r: optional [nz][nx] relative permeability (Table 1 `miu`; None = 1)."""
     lib = _load()
     p, src, rec, wav = _pack(pb)
     cplx = np.iscomplexobj(eps_r) or np.iscomplexobj(sigma)
@@ -165,14 +174,15 @@ def forward(pb: Problem, eps_r, sigma, want_ez_hist=False, want_h_hist=False):
         hy = np.zeros((S, nt + 1, pb.nz, pb.nx - 1), dtype=dtype)
         out["hx_hist"], out["hy_hist"] = hx, hy
     fn = lib.oraclez_forward if cplx else lib.oracle_forward
+    mu = _mu(pb, mu_r)
     rc = fn(ctypes.byref(p), _ptr(e), _ptr(s), _ptr(wav), _ptr(src), _ptr(rec),
-            _ptr(out["traces"]), _ptr(ez), _ptr(hx), _ptr(hy))
+            _ptr(out["traces"]), _ptr(ez), _ptr(hx), _ptr(hy), _ptr(mu))
     if rc != 0:
         raise ValueError(f"oracle forward failed: code {rc}")
     return out
 
 
-def gradient(pb: Problem, eps_r, sigma, residual, checkpoint_stride=0, want_traces=False):
+def gradient(pb: Problem, eps_r, sigma, residual, checkpoint_stride=0, want_traces=False, mu_r=None):
     """Algorithm 2 + chain rule: (grad_eps_r, grad_sigma[, traces]) of sum(residual * traces)."""
     lib = _load()
     p, src, rec, wav = _pack(pb)
@@ -184,8 +194,9 @@ def gradient(pb: Problem, eps_r, sigma, residual, checkpoint_stride=0, want_trac
     ge = np.zeros_like(e)
     gs = np.zeros_like(e)
     tr = np.zeros((p.nshots, pb.nt, p.nrec)) if want_traces else None
+    mu = _mu(pb, mu_r)
     rc = lib.oracle_gradient(ctypes.byref(p), _ptr(e), _ptr(s), _ptr(wav), _ptr(src), _ptr(rec),
-                             _ptr(res), ctypes.c_int(checkpoint_stride), _ptr(tr), _ptr(ge), _ptr(gs))
+                             _ptr(res), ctypes.c_int(checkpoint_stride), _ptr(tr), _ptr(ge), _ptr(gs), _ptr(mu))
     if rc != 0:
         raise ValueError(f"oracle gradient failed: code {rc}")
     return (ge, gs, tr) if want_traces else (ge, gs)

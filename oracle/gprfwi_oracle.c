@@ -5,7 +5,8 @@
  * (GPR dual-parameter FWI): the 2-D TM-mode (Ez, Hx, Hy) Yee FDTD in lossy
  * media with CPML, run forward (Algorithm 1) and then as its
  * hand-derived exact discrete adjoint (Algorithm 2) to give
- * d(sum residual*trace)/d(eps_r) and /d(sigma).
+ * d(sum residual*trace)/d(eps_r) and /d(sigma).  The relative permeability mu_r is an optional
+ * per-cell model input (Table 1 `miu`; it is not inverted for).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
  * --impl reference legs may build, load or call this file.  It shares no code
@@ -205,7 +206,7 @@ static void tables_free(tables_t *t) { free(t->b_ex); }
  * Stage 1 (receivers) and 7 (save wavefield) are done by the caller around this.
  * ------------------------------------------------------------------------------------- */
 static void forward_step(state_t *s, const tables_t *t, const SCALAR *Ca, const SCALAR *Cb,
-                         double dx, double Db, int src_z, int src_x, double w_n)
+                         double dx, const double *Db, int src_z, int src_x, double w_n)
 {
   const int nz = s->nz, nx = s->nx;
   /* stages 2-3: magnetic update + magnetic PML.  Eq. (4) */
@@ -215,7 +216,7 @@ static void forward_step(state_t *s, const tables_t *t, const SCALAR *Ca, const 
       size_t k = (size_t)j * nx + i;
       SCALAR g = (s->Ez[(size_t)(j + 1) * nx + i] - s->Ez[(size_t)j * nx + i]) / dx;
       s->pHxz[k] = t->b_hz[j] * s->pHxz[k] + t->c_hz[j] * g;
-      s->Hx[k] -= Db * (g * t->ik_hz[j] + s->pHxz[k]);
+      s->Hx[k] -= Db[(size_t)j * nx + i] * (g * t->ik_hz[j] + s->pHxz[k]);
     }
   /* Eq. (5) */
 #pragma omp parallel for schedule(static)
@@ -224,7 +225,7 @@ static void forward_step(state_t *s, const tables_t *t, const SCALAR *Ca, const 
       size_t k = (size_t)j * (nx - 1) + i;
       SCALAR g = (s->Ez[(size_t)j * nx + i + 1] - s->Ez[(size_t)j * nx + i]) / dx;
       s->pHyx[k] = t->b_hx[i] * s->pHyx[k] + t->c_hx[i] * g;
-      s->Hy[k] += Db * (g * t->ik_hx[i] + s->pHyx[k]);
+      s->Hy[k] += Db[(size_t)j * nx + i] * (g * t->ik_hx[i] + s->pHyx[k]);
     }
   /* stages 4-5: electric update + electric PML.  Eq. (3) in Ca/Cb form.
    * Outer ring of Ez nodes is PEC and never updated (reading R5). */
@@ -244,6 +245,20 @@ static void forward_step(state_t *s, const tables_t *t, const SCALAR *Ca, const 
     size_t k = (size_t)src_z * nx + src_x;
     s->Ez[k] -= Cb[k] * w_n / (dx * dx);
   }
+}
+
+/* Magnetic update coefficient per cell: the paper's uH4 = 1/HA, HA = mu0 * mu_r / dt (ucget listing,
+ * PAPER.md:291-295; model input `miu`, Table 1).  The listing indexes mr, uH1 and uH4 with
+ * the same (i, j, k) as the H component they update, so the H component stored at array index (j, i) --
+ * Hx at (j+1/2, i), Hy at (j, i+1/2) -- takes mu_r[j][i], without averaging (reading R22).
+ * mu_r == NULL means mu_r = 1 everywhere (what every BASELINE.json config uses). */
+static double *db_alloc(const oracle_params *p, const double *mu_r)
+{
+  const size_t ncell = (size_t)p->nz * p->nx;
+  double *Db = (double *)malloc(ncell * sizeof(double));
+  if (!Db) return NULL;
+  for (size_t k = 0; k < ncell; ++k) Db[k] = p->dt / (MU0 * (mu_r ? mu_r[k] : 1.0));
+  return Db;
 }
 
 static int check_geometry(const oracle_params *p, const int32_t *src_zx, const int32_t *rec_zx)
@@ -273,20 +288,20 @@ static int check_geometry(const oracle_params *p, const int32_t *src_zx, const i
  * ------------------------------------------------------------------------------------- */
 int FN(forward)(const oracle_params *p, const SCALAR *eps_r, const SCALAR *sigma,
                 const double *wavelet, const int32_t *src_zx, const int32_t *rec_zx,
-                SCALAR *traces, SCALAR *ez_hist, SCALAR *hx_hist, SCALAR *hy_hist)
+                SCALAR *traces, SCALAR *ez_hist, SCALAR *hx_hist, SCALAR *hy_hist, const double *mu_r)
 {
   int rc = check_geometry(p, src_zx, rec_zx);
   if (rc) return rc;
   const int nz = p->nz, nx = p->nx, nt = p->nt, R = p->nrec;
   const size_t ncell = (size_t)nz * nx;
-  const double Db = p->dt / MU0;                 /* uH4 with mu_r = 1 */
+  double *Db = db_alloc(p, mu_r);                /* uH4 */
   tables_t tab;
-  if (tables_alloc(&tab, p)) return -4;
+  if (!Db || tables_alloc(&tab, p)) { free(Db); return -4; }
   SCALAR *Ca = (SCALAR *)malloc(ncell * sizeof(SCALAR));
   SCALAR *Cb = (SCALAR *)malloc(ncell * sizeof(SCALAR));
   state_t st;
   SCALAR *buf = state_alloc(&st, nz, nx);
-  if (!Ca || !Cb || !buf) { free(Ca); free(Cb); free(buf); tables_free(&tab); return -4; }
+  if (!Ca || !Cb || !buf) { free(Ca); free(Cb); free(buf); free(Db); tables_free(&tab); return -4; }
   FN(coefficients)((int64_t)ncell, eps_r, sigma, p->dt, Ca, Cb);
 
   for (int s = 0; s < p->nshots; ++s) {
@@ -311,7 +326,7 @@ int FN(forward)(const oracle_params *p, const SCALAR *eps_r, const SCALAR *sigma
     if (hy_hist) memcpy(hy_hist + ((size_t)s * (nt + 1) + nt) * (size_t)nz * (nx - 1), st.Hy,
                         (size_t)nz * (nx - 1) * sizeof(SCALAR));
   }
-  free(Ca); free(Cb); free(buf); tables_free(&tab);
+  free(Ca); free(Cb); free(buf); free(Db); tables_free(&tab);
   return 0;
 }
 
@@ -325,7 +340,7 @@ int FN(forward)(const oracle_params *p, const SCALAR *eps_r, const SCALAR *sigma
  * Derivation: DESIGN.md section 4.
  * ------------------------------------------------------------------------------------- */
 static void adjoint_step(state_t *lam, const tables_t *t, const double *Ca, const double *Cb,
-                         double dx, double Db, const double *En, const double *En1,
+                         double dx, const double *Db, const double *En, const double *En1,
                          double *gCa, double *gCb, double *tx, double *tz,
                          const int32_t *rec, int R, const double *res_n)
 {
@@ -371,7 +386,7 @@ static void adjoint_step(state_t *lam, const tables_t *t, const double *Ca, cons
   for (int j = 0; j <= nz - 2; ++j)
     for (int i = 0; i < nx; ++i) {
       size_t k = (size_t)j * nx + i;
-      double px = -Db * lam->Hx[k];
+      double px = -Db[(size_t)j * nx + i] * lam->Hx[k];
       double T = lam->pHxz[k] + px;
       tz[k] = px * t->ik_hz[j] + t->c_hz[j] * T;        /* sz */
       lam->pHxz[k] = t->b_hz[j] * T;
@@ -386,7 +401,7 @@ static void adjoint_step(state_t *lam, const tables_t *t, const double *Ca, cons
   for (int j = 0; j < nz; ++j)
     for (int i = 0; i <= nx - 2; ++i) {
       size_t k = (size_t)j * (nx - 1) + i;
-      double py = Db * lam->Hy[k];
+      double py = Db[(size_t)j * nx + i] * lam->Hy[k];
       double T = lam->pHyx[k] + py;
       double sx = py * t->ik_hx[i] + t->c_hx[i] * T;
       lam->pHyx[k] = t->b_hx[i] * T;
@@ -416,18 +431,18 @@ static void adjoint_step(state_t *lam, const tables_t *t, const double *Ca, cons
 int oracle_gradient(const oracle_params *p, const double *eps_r, const double *sigma,
                     const double *wavelet, const int32_t *src_zx, const int32_t *rec_zx,
                     const double *residual, int checkpoint_stride,
-                    double *traces, double *grad_eps_r, double *grad_sigma)
+                    double *traces, double *grad_eps_r, double *grad_sigma, const double *mu_r)
 {
   int rc = check_geometry(p, src_zx, rec_zx);
   if (rc) return rc;
   const int nz = p->nz, nx = p->nx, nt = p->nt, R = p->nrec;
   const size_t ncell = (size_t)nz * nx;
   const size_t nstate = state_count(nz, nx);
-  const double Db = p->dt / MU0;
   const int K = checkpoint_stride > 0 ? checkpoint_stride : nt;
   const int nseg = (nt + K - 1) / K;
+  double *Db = db_alloc(p, mu_r);                /* uH4 per cell (mu_r == NULL: 1) */
   tables_t tab;
-  if (tables_alloc(&tab, p)) return -4;
+  if (!Db || tables_alloc(&tab, p)) { free(Db); return -4; }
   double *Ca = (double *)malloc(ncell * sizeof(double));
   double *Cb = (double *)malloc(ncell * sizeof(double));
   double *gCa = (double *)calloc(ncell, sizeof(double));
@@ -441,7 +456,7 @@ int oracle_gradient(const oracle_params *p, const double *eps_r, const double *s
   double *lbuf = state_alloc(&lam, nz, nx);
   if (!Ca || !Cb || !gCa || !gCb || !tx || !tz || !seg || !ckpt || !fbuf || !lbuf) {
     free(Ca); free(Cb); free(gCa); free(gCb); free(tx); free(tz); free(seg); free(ckpt);
-    free(fbuf); free(lbuf); tables_free(&tab);
+    free(fbuf); free(lbuf); free(Db); tables_free(&tab);
     return -4;
   }
   oracle_coefficients((int64_t)ncell, eps_r, sigma, p->dt, Ca, Cb);
@@ -484,7 +499,7 @@ int oracle_gradient(const oracle_params *p, const double *eps_r, const double *s
     grad_sigma[k] = -(gCa[k] * (EPS0 * eps_r[k] / p->dt) + 0.5 * gCb[k]) / (EA * EA);
   }
   free(Ca); free(Cb); free(gCa); free(gCb); free(tx); free(tz); free(seg); free(ckpt);
-  free(fbuf); free(lbuf); tables_free(&tab);
+  free(fbuf); free(lbuf); free(Db); tables_free(&tab);
   return 0;
 }
 #endif /* !ORACLE_COMPLEX */

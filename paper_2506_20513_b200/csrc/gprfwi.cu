@@ -71,8 +71,14 @@ static Shape adj_shape()
   return {R, NW, MINB, (const void*)adj_kernel<R, NW, MINB>, RegTile<R, NW, kAdjRing>::smem_bytes(true),
           RegTile<R, NW, kAdjRing>::smem_bytes(false)};
 }
+// (the other shapes exist in tuning builds only, -DGPRFWI_TUNING: they spill and were measured slower)
+#ifdef GPRFWI_TUNING
 static const Shape kFwdShapes[] = {fwd_shape<3, 12, 1>(), fwd_shape<3, 8, 2>(), fwd_shape<4, 12, 1>(), fwd_shape<2, 16, 1>()};
 static const Shape kAdjShapes[] = {adj_shape<3, 12, 1>(), adj_shape<3, 8, 2>(), adj_shape<4, 12, 1>(), adj_shape<2, 16, 1>()};
+#else
+static const Shape kFwdShapes[] = {fwd_shape<3, 12, 1>()};
+static const Shape kAdjShapes[] = {adj_shape<3, 12, 1>()};
+#endif
 #endif
 static int shape_index(const char* env, int count)
 {

@@ -22,7 +22,7 @@ C0, MU0, EPS0 = gi.C0, gi.MU0, gi.EPS0
 # ------------------------------------------------------------------------------------------------
 # Pin 1: analytic 2-D line source  (forward scheme, source scale and sign, time alignment, CPML)
 # ------------------------------------------------------------------------------------------------
-def _analytic_trace(w, dt, rho, eps_r, sigma):
+def _analytic_trace(w, dt, rho, eps_r, sigma, mu_r=1.0):
     """Ez(rho, t_n = n dt) for a z-directed line current I(t) sampled as w[n] = I((n+1/2) dt) in a
     homogeneous medium: Ez(w) = -(w mu0 / 4) I(w) H0^(2)(k rho), k = w sqrt(mu0 eps (1 - j s/(w eps)))
     (Harrington, Time-Harmonic EM Fields, eq. 5-84), e^{+jwt} convention."""
@@ -33,13 +33,14 @@ def _analytic_trace(w, dt, rho, eps_r, sigma):
     E = np.zeros_like(W)
     o = om[1:]
     eps = EPS0 * eps_r
-    k = o * np.sqrt(MU0 * eps * (1.0 - 1j * sigma / (o * eps)))
+    mu = MU0 * mu_r
+    k = o * np.sqrt(mu * eps * (1.0 - 1j * sigma / (o * eps)))
     k = np.where(k.imag > 0, -k, k)              # decaying branch for e^{+jwt}
-    E[1:] = -(o * MU0 / 4.0) * W[1:] * np.exp(-1j * o * dt / 2.0) * hankel2(0, k * rho)
+    E[1:] = -(o * mu / 4.0) * W[1:] * np.exp(-1j * o * dt / 2.0) * hankel2(0, k * rho)
     return np.fft.irfft(E, nfft)[:nt]
 
 
-def _line_source_error(dx, eps_r, sigma, offsets_m):
+def _line_source_error(dx, eps_r, sigma, offsets_m, mu_r=None):
     f = 400e6
     dt = 2e-11 * dx / 0.01
     nt = int(round(12e-9 / dt))
@@ -57,11 +58,12 @@ def _line_source_error(dx, eps_r, sigma, offsets_m):
     pb = oracle.Problem(nz=n, nx=n, dx=dx, dt=dt, nt=nt, npml=npml, pml_order=order, pml_sigma_max=smax,
                         pml_kappa_max=kmax, pml_alpha_max=amax, src_zx=np.array([[c, c]]),
                         rec_zx=np.array([recs]), wavelet=w)
-    tr = oracle.forward(pb, np.full((n, n), eps_r), np.full((n, n), sigma))["traces"][0]
+    tr = oracle.forward(pb, np.full((n, n), eps_r), np.full((n, n), sigma),
+                        mu_r=None if mu_r is None else np.full((n, n), mu_r))["traces"][0]
     errs = []
     for r, (z, x) in enumerate(recs):
         rho = dx * np.hypot(z - c, x - c)
-        errs.append(rel_l2(tr[:, r], _analytic_trace(w, dt, rho, eps_r, sigma)))
+        errs.append(rel_l2(tr[:, r], _analytic_trace(w, dt, rho, eps_r, sigma, 1.0 if mu_r is None else mu_r)))
     return np.array(errs)
 
 
@@ -444,3 +446,88 @@ def test_lowpass_oracle_equals_numpy_convolve():
         for r in range(3):
             assert np.allclose(y[s, :, r], np.convolve(x[s, :, r], taps, mode="same"), atol=1e-13)
     assert np.allclose(ep.lowpass(np.ones((1, 100, 1)), taps)[0, 20:80, 0], 1.0, atol=1e-13)
+
+
+# ------------------------------------------------------------------------------------------------
+# mu_r model input (Table 1 `miu`; uH4 = dt / (mu0 mu_r); reading R22)
+# ------------------------------------------------------------------------------------------------
+def test_mu_r_line_source_green_function_second_order():
+    """Homogeneous mu_r = 2: the analytic line-source field has mu = mu0 mu_r in BOTH the amplitude
+    -(w mu / 4) and the wavenumber; a Db that ignored mu_r, or used it in only one of the two H updates,
+    gives O(1) errors (wrong speed / anisotropy), the correct scheme converges with order 2."""
+    offs = (0.2, 0.4)
+    e1 = _line_source_error(0.01, 2.0, 2e-3, offs, mu_r=2.0)
+    e2 = _line_source_error(0.005, 2.0, 2e-3, offs, mu_r=2.0)
+    assert np.all(e1 < 4e-2), e1
+    ratio = e1 / e2
+    assert np.all(ratio > 3.0) and np.all(ratio < 5.0), (e1, e2, ratio)
+
+
+def _random_mu(wl, seed):
+    return np.random.default_rng(seed).uniform(1.0, 3.0, (wl.nz, wl.nx))
+
+
+def test_mu_r_energy_conserved_with_heterogeneous_permeability():
+    """Lossless PEC box, heterogeneous eps_r AND mu_r: the discrete energy with mu0 mu_r[j][i] weighting the
+    H component stored at array index (j, i) is conserved to round-off once the source is off.  A mu_r taken
+    from a neighbouring index, applied to one H component only, or left out of the CPML-free update breaks
+    this at O(1)."""
+    wl = gi.small_random(nz=40, nx=46, nt=600, npml=0, nshots=1, nrec=1, lossy=False, seed=8)
+    mu = _random_mu(wl, 3)
+    w = wl.wavelet.astype(np.float64).copy()
+    nsrc_on = 380
+    w[nsrc_on:] = 0.0
+    out = oracle.forward(problem(wl, wavelet=w), wl.eps_r, wl.sigma, want_h_hist=True, mu_r=mu)
+    ez, hx, hy = out["ez_hist"][0], out["hx_hist"][0], out["hy_hist"][0]
+    eps = EPS0 * wl.eps_r.astype(np.float64)
+    dx2 = wl.dx ** 2
+    ns = np.arange(nsrc_on + 1, wl.nt)
+    W = np.array([0.5 * np.sum(eps * ez[n] ** 2) * dx2
+                  + 0.5 * MU0 * (np.sum(mu[:-1, :] * hx[n + 1] * hx[n]) + np.sum(mu[:, :-1] * hy[n + 1] * hy[n])) * dx2
+                  for n in ns])
+    assert W[0] > 0
+    assert np.max(np.abs(W / W[0] - 1.0)) < 1e-12
+    # ... and the same sum with mu_r left out of the weights is NOT constant (the test can fail)
+    W1 = np.array([0.5 * np.sum(eps * ez[n] ** 2) * dx2
+                   + 0.5 * MU0 * (np.sum(hx[n + 1] * hx[n]) + np.sum(hy[n + 1] * hy[n])) * dx2 for n in ns])
+    assert np.max(np.abs(W1 / W1[0] - 1.0)) > 1e-3
+
+
+def test_mu_r_reciprocity_and_adjoint_identity():
+    """Heterogeneous lossy model with CPML and heterogeneous mu_r: swapping source and receiver leaves the
+    trace unchanged (1e-12), and <J dm, y> = <dm, J^T y> with J dm from the complex-step forward (1e-10):
+    the transpose of the H update carries the same per-cell Db on the same component."""
+    wl = gi.small_random(nz=60, nx=70, nt=400, npml=10, nshots=1, nrec=1, seed=12)
+    mu = _random_mu(wl, 4)
+    a, b = (14, 17), (41, 55)
+    tr = []
+    for s_, r_ in ((a, b), (b, a)):
+        pb = problem(wl, src_zx=np.array([s_]), rec_zx=np.array([[r_]]))
+        tr.append(oracle.forward(pb, wl.eps_r, wl.sigma, mu_r=mu)["traces"][0, :, 0])
+    assert np.linalg.norm(tr[0]) > 0 and rel_l2(tr[0], tr[1]) < 1e-12
+    assert rel_l2(tr[0], oracle.forward(problem(wl, src_zx=np.array([a]), rec_zx=np.array([[b]])), wl.eps_r,
+                                        wl.sigma)["traces"][0, :, 0]) > 1e-2       # mu_r does change the answer
+    wl = gi.small_random(nz=44, nx=52, nt=160, npml=8, nshots=2, nrec=6, seed=22)
+    mu = _random_mu(wl, 5)
+    pb = problem(wl)
+    rng = np.random.default_rng(6)
+    de = rng.standard_normal((wl.nz, wl.nx)); ds = rng.standard_normal((wl.nz, wl.nx)) * 1e-2
+    y = rng.standard_normal((wl.nshots, wl.nt, wl.nrec))
+    h = 1e-30
+    Jdm = oracle.forward(pb, wl.eps_r + 1j * h * de, wl.sigma + 1j * h * ds, mu_r=mu)["traces"].imag / h
+    ge, gs = oracle.gradient(pb, wl.eps_r, wl.sigma, y, mu_r=mu)
+    lhs, rhs = float(np.sum(Jdm * y)), float(np.sum(ge * de) + np.sum(gs * ds))
+    assert abs(lhs) > 0 and abs(lhs - rhs) / abs(lhs) < 1e-10
+    ge_k, gs_k = oracle.gradient(pb, wl.eps_r, wl.sigma, y, checkpoint_stride=37, mu_r=mu)
+    assert rel_l2(ge_k, ge) < 1e-13 and rel_l2(gs_k, gs) < 1e-13
+
+
+def test_mu_r_of_one_is_the_default():
+    wl = gi.small_random(nz=44, nx=52, nt=120, npml=8, nshots=2, nrec=5, seed=23)
+    pb = problem(wl)
+    y = gi.random_residual(wl, 1.0)
+    one = np.ones((wl.nz, wl.nx))
+    assert np.array_equal(oracle.forward(pb, wl.eps_r, wl.sigma)["traces"],
+                          oracle.forward(pb, wl.eps_r, wl.sigma, mu_r=one)["traces"])
+    for a_, b_ in zip(oracle.gradient(pb, wl.eps_r, wl.sigma, y), oracle.gradient(pb, wl.eps_r, wl.sigma, y, mu_r=one)):
+        assert np.array_equal(a_, b_)
