@@ -88,7 +88,10 @@ size_t gprfwi_workspace_bytes(const gprfwi_params* p, size_t budget_bytes, gprfw
  * nt steps of {record receivers, H update + H CPML (Eqs. 4-5), E update + E CPML (Eq. 3 in the
  * Ca/Cb form of PAPER.md:415-424), source injection, save wavefield}.
  *   h        out: *h receives a new handle (release with gprfwi_release).  If *h is non-NULL on
- *            entry it is reused (it must come from an earlier call with identical params).
+ *            entry it is reused (it must come from an earlier call with identical params).  A reused
+ *            handle that meets the same workspace, plan and acquisition again does not rebuild or
+ *            re-upload the receiver / CPML tables it keeps in the workspace: between calls on a live
+ *            handle the caller must leave the workspace alone.
  *   eps_r, sigma   device [nz][pitch]; must stay unmodified until the last gprfwi_adjoint
  *   wavelet  device [nt] or [nshots][nt]
  *   src_zx   host   [nshots][2]        (z, x) cell indices, copied
@@ -102,6 +105,17 @@ int gprfwi_forward(gprfwi_handle** h, const gprfwi_params* p,
                    const int32_t* src_zx, const int32_t* rec_zx,
                    void* workspace, size_t workspace_bytes,
                    float* traces, void* cuda_stream);
+
+/* gprfwi_forward with a relative-permeability model (Table 1 `miu`; the paper's uH4 = 1/HA,
+ * HA = m0*mr/dt).  mu_r: device [nz][pitch] fp32, > 0, read during this call only, or
+ * NULL (= 1 everywhere, identical to gprfwi_forward).  Reading R22: the H component stored at
+ * array index (j, i) -- Hx at (j+1/2, i), Hy at (j, i+1/2) -- takes mu_r[j][i], no averaging.  mu_r is a
+ * model input only: gprfwi_adjoint (which uses the same model through the handle) still returns the
+ * gradients with respect to eps_r and sigma.  Everything else as gprfwi_forward. */
+int gprfwi_forward_mu(gprfwi_handle** h, const gprfwi_params* p,
+                      const float* eps_r, const float* sigma, const float* mu_r,
+                      const float* wavelet, const int32_t* src_zx, const int32_t* rec_zx,
+                      void* workspace, size_t workspace_bytes, float* traces, void* cuda_stream);
 
 /* Adjoint sweep + gradient, Algorithm 2: reverse time loop of {transpose of the
  * E update + E CPML, transpose of the H update + H CPML, adjoint source = residual sample n at the

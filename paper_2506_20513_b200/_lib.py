@@ -15,7 +15,7 @@ GPRFWI_OK = 0
 STATUS_NAMES = {0: "OK", -1: "EINVAL", -2: "ECFL", -3: "EGEOM", -4: "ENOMEM", -5: "ESTATE", -6: "ECUDA"}
 
 EXPORTS = (
-    "gprfwi_workspace_bytes", "gprfwi_forward", "gprfwi_adjoint", "gprfwi_gradient_host",
+    "gprfwi_workspace_bytes", "gprfwi_forward", "gprfwi_forward_mu", "gprfwi_adjoint", "gprfwi_gradient_host",
     "gprfwi_workspace_bytes_host", "gprfwi_residual", "gprfwi_launch_count", "gprfwi_get_plan",
     "gprfwi_release", "gprfwi_strerror", "gprfwi_version", "gprfwi_update", "gprfwi_update_workspace_bytes", "gprfwi_lowpass",
 )
@@ -75,6 +75,9 @@ def _declare(lib):
     lib.gprfwi_forward.restype = ctypes.c_int
     lib.gprfwi_forward.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(Params), fp, fp, fp, i32p, i32p,
                                    vp, sz, fp, vp]
+    lib.gprfwi_forward_mu.restype = ctypes.c_int
+    lib.gprfwi_forward_mu.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(Params), fp, fp, fp, fp, i32p, i32p,
+                                      vp, sz, fp, vp]
     lib.gprfwi_adjoint.restype = ctypes.c_int
     lib.gprfwi_adjoint.argtypes = [vp, fp, fp, fp, vp]
     lib.gprfwi_gradient_host.restype = ctypes.c_int

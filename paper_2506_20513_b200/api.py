@@ -85,8 +85,9 @@ def split_batch(p: Params, budget_bytes: int = 0, min_shots_per_pass: int = 3):
 
 
 def gprfwi_forward(p: Params, eps_r, sigma, wavelet, src_zx, rec_zx, workspace, traces, handle=None,
-                   stream=None):
-    """Enqueue Algorithm 1 on `stream`; returns the (new or reused) handle (an int)."""
+                   stream=None, mu_r=None):
+    """Enqueue Algorithm 1 on `stream`; returns the (new or reused) handle (an int).
+    mu_r: optional relative-permeability model (gprfwi_forward_mu; None = 1 everywhere)."""
     lib = _lib.load()
     src = _i32(src_zx, (p.nshots, 2), "src_zx")
     rec = _i32(np.asarray(rec_zx).reshape(p.nshots, p.nrec, 2), (p.nshots, p.nrec, 2), "rec_zx")
@@ -94,8 +95,9 @@ def gprfwi_forward(p: Params, eps_r, sigma, wavelet, src_zx, rec_zx, workspace, 
         raise TypeError("workspace must be a CUDA uint8 tensor")
     h = ctypes.c_void_p(handle)
     nw = (p.nshots if p.wavelet_per_shot else 1) * p.nt
-    code = lib.gprfwi_forward(
+    code = lib.gprfwi_forward_mu(
         ctypes.byref(h), ctypes.byref(p), _dev(eps_r, "eps_r", p.nz * p.pitch), _dev(sigma, "sigma", p.nz * p.pitch),
+        None if mu_r is None else _dev(mu_r, "mu_r", p.nz * p.pitch),
         _dev(wavelet, "wavelet", nw), src.ctypes.data, rec.ctypes.data, workspace.data_ptr(),
         workspace.numel(), _dev(traces, "traces", p.nshots * p.nt * p.nrec) if p.nrec else None,
         _stream_ptr(stream))
@@ -215,10 +217,10 @@ class Simulation:
         self.handle = None
         self._models = None
 
-    def forward(self, eps_r: torch.Tensor, sigma: torch.Tensor, stream=None) -> torch.Tensor:
-        self._models = (eps_r, sigma)       # must stay alive and unmodified until the adjoint
+    def forward(self, eps_r: torch.Tensor, sigma: torch.Tensor, stream=None, mu_r=None) -> torch.Tensor:
+        self._models = (eps_r, sigma, mu_r)  # must stay alive and unmodified until the adjoint
         self.handle = gprfwi_forward(self.p, eps_r, sigma, self.wavelet, self.src_zx, self.rec_zx,
-                                     self.workspace, self.traces, self.handle, stream)
+                                     self.workspace, self.traces, self.handle, stream, mu_r)
         return self.traces
 
     def adjoint(self, residual: torch.Tensor, stream=None):

@@ -52,24 +52,25 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 // Entry 0 of each table is the default; GPRFWI_FWD_SHAPE / GPRFWI_ADJ_SHAPE pick another (tuning).
 struct Shape {
   int R, NW, minb;
-  const void* func;
-  size_t smem_pml, smem_plain;
+  const void *func, *func_mu;                  // the kernel; its variant for problems with a mu_r model
+  size_t smem_pml, smem_plain, smem_mu;        // bytes with / without psi slots; extra bytes with a mu_r model
   int rows() const { return R * NW; }
   int threads() const { return NW * 32; }
-  size_t smem(bool pml) const { return pml ? smem_pml : smem_plain; }
+  size_t smem(bool pml, bool mu = false) const { return (pml ? smem_pml : smem_plain) + (mu ? smem_mu : 0); }
 };
 #if defined(__CUDACC__)
 template <int R, int NW, int MINB>
 static Shape fwd_shape()
 {
-  return {R, NW, MINB, (const void*)fwd_kernel<R, NW, MINB>, RegTile<R, NW, 3>::smem_bytes(true),
-          RegTile<R, NW, 3>::smem_bytes(false)};
+  return {R, NW, MINB, (const void*)fwd_kernel<R, NW, MINB, false>, (const void*)fwd_kernel<R, NW, MINB, true>, RegTile<R, NW, 3>::smem_bytes(true),
+          RegTile<R, NW, 3>::smem_bytes(false), RegTile<R, NW, 3>::smem_bytes(false, true) - RegTile<R, NW, 3>::smem_bytes(false)};
 }
 template <int R, int NW, int MINB>
 static Shape adj_shape()
 {
-  return {R, NW, MINB, (const void*)adj_kernel<R, NW, MINB>, RegTile<R, NW, kAdjRing>::smem_bytes(true),
-          RegTile<R, NW, kAdjRing>::smem_bytes(false)};
+  return {R, NW, MINB, (const void*)adj_kernel<R, NW, MINB, false>, (const void*)adj_kernel<R, NW, MINB, true>, RegTile<R, NW, kAdjRing>::smem_bytes(true),
+          RegTile<R, NW, kAdjRing>::smem_bytes(false),
+          RegTile<R, NW, kAdjRing>::smem_bytes(false, true) - RegTile<R, NW, kAdjRing>::smem_bytes(false)};
 }
 // (the other shapes exist in tuning builds only, -DGPRFWI_TUNING: they spill and were measured slower)
 #ifdef GPRFWI_TUNING
@@ -206,7 +207,7 @@ static void set_groups(const gprfwi_params* p, Layout& L)
 
 // device pointers carved out of the caller's workspace
 struct Carve {
-  float *ca = nullptr, *cb = nullptr, *gca = nullptr, *gcb = nullptr;
+  float *ca = nullptr, *cb = nullptr, *dbc = nullptr, *gca = nullptr, *gcb = nullptr;   // dbc: per-cell Db (mu_r model)
   // static block (one contiguous range, uploaded with one copy): CPML tables, source cells, receiver tables
   char* stat = nullptr;
   size_t stat_bytes = 0;
@@ -244,6 +245,7 @@ static size_t carve(const gprfwi_params* p, const Layout& L, char* base, Carve* 
   };
   o.ca = (float*)take_planes(L.plane * f);
   o.cb = (float*)take_planes(L.plane * f);
+  o.dbc = (float*)take_planes(L.plane * f);
   o.gca = (float*)take_planes((size_t)L.ngroups * L.plane * f);
   o.gcb = (float*)take_planes((size_t)L.ngroups * L.plane * f);
   o.fscratch = (float*)take_planes(2 * L.blk(S) * f);
@@ -369,6 +371,7 @@ struct gprfwi_handle {
   Carve c;
   Geo geo;
   const float *eps_r = nullptr, *sigma = nullptr, *wavelet = nullptr;
+  bool mu = false;           // the last forward had a mu_r model: the kernels read the per-cell Db plane
   void* workspace = nullptr;
   // Host copy of the static block (CPML tables, source cells, receiver tables) in PINNED memory, laid out
   // like Carve::stat so that one asynchronous copy uploads it; rebuilt only when the geometry, the plan or
@@ -593,22 +596,26 @@ static int maps_init(gprfwi_handle* h, bool same_plan)
 
 static int kernels_init(const gprfwi_params* p, const Layout& L)
 {
-  const bool pml = p->npml > 0;
+  const bool pml = p->npml > 0;      // (the largest request either variant makes)
   GPR_CUDA(cudaFuncSetAttribute(kFwdShapes[L.fv].func, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)kFwdShapes[L.fv].smem(pml)));
   GPR_CUDA(cudaFuncSetAttribute(kAdjShapes[L.av].func, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)kAdjShapes[L.av].smem(pml)));
+  GPR_CUDA(cudaFuncSetAttribute(kFwdShapes[L.fv].func_mu, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)kFwdShapes[L.fv].smem(pml, true)));
+  GPR_CUDA(cudaFuncSetAttribute(kAdjShapes[L.av].func_mu, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)kAdjShapes[L.av].smem(pml, true)));
   return GPRFWI_OK;
 }
 
 // every tile-kernel launch allows programmatic dependent launch (the kernels call griddepcontrol.wait
 // before they read the previous launch's output)
-static int launch_pdl(const Shape& sh, dim3 grid, void* arg, bool pml, cudaStream_t st)
+static int launch_pdl(const Shape& sh, dim3 grid, void* arg, bool pml, bool mu, cudaStream_t st)
 {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = grid;
   cfg.blockDim = dim3(sh.threads());
-  cfg.dynamicSmemBytes = sh.smem(pml);
+  cfg.dynamicSmemBytes = sh.smem(pml, mu);
   cfg.stream = st;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -616,7 +623,7 @@ static int launch_pdl(const Shape& sh, dim3 grid, void* arg, bool pml, cudaStrea
   cfg.attrs = at;
   cfg.numAttrs = 1;
   void* args[] = {arg};
-  GPR_CUDA(cudaLaunchKernelExC(&cfg, sh.func, args));
+  GPR_CUDA(cudaLaunchKernelExC(&cfg, mu ? sh.func_mu : sh.func, args));
   return GPRFWI_OK;
 }
 
@@ -670,6 +677,7 @@ static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, 
   a.out = out;
   a.ca = h->c.ca;
   a.cb = h->c.cb;
+  a.dbc = h->mu ? h->c.dbc : nullptr;
   a.tm_reg = h->tm_fwd_reg;
   a.in_pl[0] = (int)((in.ez - h->c.ca) / (long long)L.plane);
   a.in_pl[1] = (int)((in.hx - h->c.ca) / (long long)L.plane);
@@ -695,7 +703,7 @@ static int launch_fwd_block(gprfwi_handle* h, cudaStream_t st, int n, int nsub, 
   a.oz = L.f.oz;
   const Shape& sh = kFwdShapes[L.fv];
   dim3 grid(L.f.tiles_x, L.f.tiles_y, (ns + L.fgroup - 1) / L.fgroup);
-  if (int rc = launch_pdl(sh, grid, &a, p.npml > 0, st)) return rc;
+  if (int rc = launch_pdl(sh, grid, &a, p.npml > 0, h->mu, st)) return rc;
   h->launches++;
   return GPRFWI_OK;
 }
@@ -715,6 +723,7 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   a.out = out;
   a.ca = h->c.ca;
   a.cb = h->c.cb;
+  a.dbc = h->mu ? h->c.dbc : nullptr;
   auto plane_index = [&](const float* q) { return (int)((q - h->c.ca) / (long long)L.plane); };
   a.tm_own = h->tm_adj_own;
   a.tm_reg = h->tm_adj_reg;
@@ -740,7 +749,7 @@ static int launch_adj_block(gprfwi_handle* h, cudaStream_t st, int n_hi, int nsu
   a.shot_base = shot0;
   const Shape& sh = kAdjShapes[L.av];
   dim3 grid(L.a.tiles_x, L.a.tiles_y, ngrp);
-  if (int rc = launch_pdl(sh, grid, &a, p.npml > 0, st)) return rc;
+  if (int rc = launch_pdl(sh, grid, &a, p.npml > 0, h->mu, st)) return rc;
   h->launches++;
   return GPRFWI_OK;
 }
@@ -816,6 +825,14 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
                    const float* wavelet, const int32_t* src_zx, const int32_t* rec_zx, void* workspace,
                    size_t workspace_bytes, float* traces, void* cuda_stream)
 {
+  return gprfwi_forward_mu(hp, p, eps_r, sigma, nullptr, wavelet, src_zx, rec_zx, workspace, workspace_bytes, traces,
+                           cuda_stream);
+}
+
+int gprfwi_forward_mu(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_r, const float* sigma,
+                      const float* mu_r, const float* wavelet, const int32_t* src_zx, const int32_t* rec_zx,
+                      void* workspace, size_t workspace_bytes, float* traces, void* cuda_stream)
+{
   int rc = validate(p);
   if (rc != GPRFWI_OK) return rc;
   if (!hp || !eps_r || !sigma || !wavelet || !src_zx || !workspace || (p->nrec > 0 && (!rec_zx || !traces)))
@@ -838,6 +855,7 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
   h->p = *p;
   h->L = L;
   h->eps_r = eps_r; h->sigma = sigma; h->wavelet = wavelet; h->workspace = workspace;
+  h->mu = mu_r != nullptr;
   h->forward_done = false;
   h->launches = 0;
   carve(p, L, (char*)workspace, &h->c);
@@ -851,8 +869,8 @@ int gprfwi_forward(gprfwi_handle** hp, const gprfwi_params* p, const float* eps_
   // kernel a: Ca/Cb once per call, shared by all shots
   {
     dim3 grid((L.pitch + 127) / 128, p->nz), block(128);
-    GPR_LAUNCH(coef_kernel, grid, block, st, eps_r, sigma, p->pitch, p->nz, p->nx, L.pitch,
-                                        (float)(1.0 / (double)p->dt), h->c.ca, h->c.cb);
+    GPR_LAUNCH(coef_kernel, grid, block, st, eps_r, sigma, mu_r, p->pitch, p->nz, p->nx, L.pitch,
+                                        (float)(1.0 / (double)p->dt), h->geo.Db, h->c.ca, h->c.cb, h->c.dbc);
     h->launches++;
   }
   // fields are zero at n = 0

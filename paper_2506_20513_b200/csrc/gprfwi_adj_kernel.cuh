@@ -28,6 +28,7 @@ struct AdjArgs {
   Geo g;
   State in, out;                      // adjoint variables, ping-pong (pointers of local shot 0)
   const float *ca, *cb;               // masked as in the forward kernel
+  const float* dbc;                   // per-cell Db as in the forward kernel, or NULL: mu_r = 1
   int ez_pl[kMaxT + 1];               // [t] = workspace plane index of forward Ez^{n_hi - t} (local shot 0), t = 0..nsub
   int in_pl[3];                       // workspace plane indices of in.ez, in.hx, in.hy (local shot 0)
   float *gca, *gcb;                   // [ngroups][nz][pitch]
@@ -125,7 +126,7 @@ __device__ __forceinline__ void adj_prefetch_state(const AdjArgs& a, const TileC
 // The T reverse steps of one warp for one shot; ZP / XP as in fwd_steps (the psi forms below give
 // exactly tx = q, tz = -q, sx, sz = +-Db lamH with the trivial coefficients outside the CPML).
 // Packed pairs as in the forward kernel: P = (c0, c2), Q = (c1, c3).
-template <int R, int NW, bool ZP, bool XP>
+template <int R, int NW, bool ZP, bool XP, bool MU>
 __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW, kAdjRing>& c, int s, int rk0, int rk1,
                                           int entx, unsigned iflags, bool prefetch, int q0, int s_end,
                                           P2 (&le)[R], P2 (&lhx)[R], P2 (&lhy)[R], const P2 (&ca)[R], const P2 (&cb)[R],
@@ -211,8 +212,14 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       P2 sx, sz;
-      sz.p = mul2(nDb2, lhx[r].p); sz.q = mul2(nDb2, lhx[r].q);
-      sx.p = mul2(Db2, lhy[r].p); sx.q = mul2(Db2, lhy[r].q);
+      if (MU) {                                         // per-cell Db (mu_r model, reading R22)
+        const P2 db = ld2(c.dbc_(a.g) + r * kRegW);
+        sz.p = mul2(neg2(db.p), lhx[r].p); sz.q = mul2(neg2(db.q), lhx[r].q);
+        sx.p = mul2(db.p, lhy[r].p); sx.q = mul2(db.q, lhy[r].q);
+      } else {
+        sz.p = mul2(nDb2, lhx[r].p); sz.q = mul2(nDb2, lhx[r].q);
+        sx.p = mul2(Db2, lhy[r].p); sx.q = mul2(Db2, lhy[r].q);
+      }
       if (ZP) {
         P2 p = ld2(c.phz_() + r * kRegW);
         const u64 b = bc2(c.tabz_()[0 * L::ROWS + c.lr0 + r]), cc = bc2(c.tabz_()[1 * L::ROWS + c.lr0 + r]),
@@ -251,7 +258,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
   }
 }
 
-template <int R, int NW, int MINB>
+template <int R, int NW, int MINB, bool MU>
 __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const __grid_constant__ AdjArgs a)
 {
   using L = RegTile<R, NW, kAdjRing>;
@@ -276,6 +283,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const __grid_constan
   }
   c.template stage_tables<false>(g);
   c.zero_psi(g);
+  if (MU) c.load_dbc(g, a.dbc);
   for (int k = threadIdx.x; k < L::ROWS * kRegW / 4; k += L::THREADS)
     reinterpret_cast<float4*>(c.rowbuf_())[k] = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
@@ -359,10 +367,13 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const __grid_constan
     __syncthreads();
     GPR_PROBE(s - s_beg, 3);
 
-    if (c.zp && c.xp) adj_steps<R, NW, true, true>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb);
-    else if (c.zp) adj_steps<R, NW, true, false>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb);
-    else if (c.xp) adj_steps<R, NW, false, true>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb);
-    else adj_steps<R, NW, false, false>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb);
+#define GPR_ADJ_STEPS(ZP_, XP_) \
+  adj_steps<R, NW, ZP_, XP_, MU>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb)
+    if (c.zp && c.xp) GPR_ADJ_STEPS(true, true);
+    else if (c.zp) GPR_ADJ_STEPS(true, false);
+    else if (c.xp) GPR_ADJ_STEPS(false, true);
+    else GPR_ADJ_STEPS(false, false);
+#undef GPR_ADJ_STEPS
 
     // ---- write back the owned part of the adjoint state ------------------------------------------------
 #pragma unroll

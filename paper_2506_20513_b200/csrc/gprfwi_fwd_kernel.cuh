@@ -28,6 +28,7 @@ struct FwdArgs {
   Geo g;
   State in, out;              // out.ez: Ez plane after the last step of this launch
   const float *ca, *cb;       // [nz][pitch], 0 on the PEC ring, in PEC cells and in the pitch padding
+  const float* dbc;           // [nz][pitch] Db = dt / (mu0 mu_r) per cell, or NULL: mu_r = 1 (Geo::Db, Geo::kap)
   float* ez_mid;              // plane for Ez after step 1 of this launch (local shot 0) or NULL: not kept;
   long long ez_mid_stride;    //   the planes after steps 2 .. nsub-1 follow at this stride (floats)
   const float* wavelet;       // sample n of local shot 0
@@ -49,7 +50,9 @@ struct FwdArgs {
 // different variants.  Every field row of the thread is two packed pairs P = (c0, c2), Q = (c1, c3):
 // differences to the right / left neighbour are Q - P resp. P - Q for half the cells and need one
 // repacked pair (with the lane shuffle) for the other half.
-template <int R, int NW, bool ZP, bool XP>
+// MU: the problem has a mu_r model (reading R22) -- Db and Db/dx come per cell from the thread's shared-memory
+// slot instead of the two scalars; with mu_r = 1 every product below rounds like the scalar form.
+template <int R, int NW, bool ZP, bool XP, bool MU>
 __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW, 3>& c, int s, int rk0, int rk1,
                                           int2 ent, unsigned rflags, int src_r, int src_c, const float (&wv)[kMaxT],
                                           P2 (&e)[R], P2 (&hx)[R], P2 (&hy)[R], const P2 (&ca)[R], const P2 (&cb)[R])
@@ -57,7 +60,7 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
   using L = RegTile<R, NW, 3>;
   const Geo& g = a.g;
   const unsigned full = 0xffffffffu;
-  const u64 rdx2 = bc2(g.rdx), Db2 = bc2(g.Db), nDb2 = bc2(-g.Db), kap2 = bc2(g.kap), nkap2 = bc2(-g.kap);
+  const u64 rdx2 = bc2(g.rdx), Db2 = bc2(g.Db), kap2 = bc2(g.kap);
   const long long hoff = s * g.plane + (long long)c.gj0 * g.pitch + c.gi;     // this thread's row 0 in a plane of shot s
   float* const trp = a.traces + (s * a.trace_stride + ent.y);                 // this thread's receiver, sample n
 #pragma unroll 1
@@ -81,27 +84,32 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
       const P2 eb = (r + 1 < R) ? e[r + 1] : ld2(c.xe_() + (c.w + 1) * kRegW + c.l4);     // Ez of the row below
       // Ez to the right of (c1, c3) is (c2, c0 of the next lane); to the right of (c0, c2) it is Q itself
       const u64 enq = pk(hi2(e[r].p), __shfl_down_sync(full, lo2(e[r].p), 1));
+      P2 db, kp;                                        // Db and Db/dx of the thread's cells
+      if (MU) { db = ld2(c.dbc_(g) + r * kRegW); kp.p = mul2(db.p, rdx2); kp.q = mul2(db.q, rdx2); }
+      else { db.p = db.q = Db2; kp.p = kp.q = kap2; }
       if (ZP) {
         P2 p = ld2(c.phz_() + r * kRegW);
         const u64 b = bc2(c.tabz_()[0 * L::ROWS + c.lr0 + r]), cr = bc2(c.tabz_()[1 * L::ROWS + c.lr0 + r]),
-                  nkk = bc2(-c.tabz_()[2 * L::ROWS + c.lr0 + r]);
+                  kk = bc2(c.tabz_()[2 * L::ROWS + c.lr0 + r]);          // Db/(dx kappa); with MU: 1/kappa
+        const u64 kkp = MU ? mul2(kp.p, kk) : kk, kkq = MU ? mul2(kp.q, kk) : kk;
         const u64 dp = sub2(eb.p, e[r].p), dq = sub2(eb.q, e[r].q);
         p.p = fma2(b, p.p, mul2(cr, dp)); p.q = fma2(b, p.q, mul2(cr, dq));
-        hx[r].p = fma2(nDb2, p.p, fma2(nkk, dp, hx[r].p)); hx[r].q = fma2(nDb2, p.q, fma2(nkk, dq, hx[r].q));
+        hx[r].p = fma2(neg2(db.p), p.p, fma2(neg2(kkp), dp, hx[r].p)); hx[r].q = fma2(neg2(db.q), p.q, fma2(neg2(kkq), dq, hx[r].q));
         st2(c.phz_() + r * kRegW, p);
       } else {
-        hx[r].p = fma2(nkap2, sub2(eb.p, e[r].p), hx[r].p);
-        hx[r].q = fma2(nkap2, sub2(eb.q, e[r].q), hx[r].q);
+        hx[r].p = fma2(neg2(kp.p), sub2(eb.p, e[r].p), hx[r].p);
+        hx[r].q = fma2(neg2(kp.q), sub2(eb.q, e[r].q), hx[r].q);
       }
       if (XP) {
         P2 p = ld2(c.phx_() + r * kRegW);
         const u64 dp = sub2(e[r].q, e[r].p), dq = sub2(enq, e[r].q);
+        const u64 xkp = MU ? mul2(kp.p, xk.p) : xk.p, xkq = MU ? mul2(kp.q, xk.q) : xk.q;
         p.p = fma2(xb.p, p.p, mul2(xc.p, dp)); p.q = fma2(xb.q, p.q, mul2(xc.q, dq));
-        hy[r].p = fma2(Db2, p.p, fma2(xk.p, dp, hy[r].p)); hy[r].q = fma2(Db2, p.q, fma2(xk.q, dq, hy[r].q));
+        hy[r].p = fma2(db.p, p.p, fma2(xkp, dp, hy[r].p)); hy[r].q = fma2(db.q, p.q, fma2(xkq, dq, hy[r].q));
         st2(c.phx_() + r * kRegW, p);
       } else {
-        hy[r].p = fma2(kap2, sub2(e[r].q, e[r].p), hy[r].p);
-        hy[r].q = fma2(kap2, sub2(enq, e[r].q), hy[r].q);
+        hy[r].p = fma2(kp.p, sub2(e[r].q, e[r].p), hy[r].p);
+        hy[r].q = fma2(kp.q, sub2(enq, e[r].q), hy[r].q);
       }
     }
     st2(c.xh_() + (c.w + 1) * kRegW + c.l4, hx[R - 1]);
@@ -210,7 +218,7 @@ __device__ __forceinline__ void fwd_fetch(const FwdArgs& a, const TileCtx<R, NW,
     tma_load_3d(smem_u32(c.sm + L::HIST + f * (L::ROWS * kRegW)), &a.tm_reg, c.ri0, c.rj0, a.in_pl[f] + s, bar);
 }
 
-template <int R, int NW, int MINB>
+template <int R, int NW, int MINB, bool MU>
 __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const __grid_constant__ FwdArgs a)
 {
   using L = RegTile<R, NW, 3>;
@@ -231,8 +239,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const __grid_constan
   }
   for (int k = tid; k < kMetaW * (s1 - s0); k += L::THREADS)
     c.meta_()[k] = fwd_meta_word(a, s0 + k / kMetaW, tile, ntile, k % kMetaW);
-  c.template stage_tables<true>(g);
+  c.template stage_tables<true>(g, MU);
   c.zero_psi(g);
+  if (MU) c.load_dbc(g, a.dbc);
   P2 ca[R], cb[R];
 #pragma unroll
   for (int r = 0; r < R; ++r) {
@@ -294,10 +303,13 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const __grid_constan
     __syncthreads();                   // exchange row and receiver rows published; landing zone free
     if (tid == 0 && s + 1 < s1) fwd_fetch<R, NW>(a, c, s + 1);
 
-    if (c.zp && c.xp) fwd_steps<R, NW, true, true>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
-    else if (c.zp) fwd_steps<R, NW, true, false>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
-    else if (c.xp) fwd_steps<R, NW, false, true>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
-    else fwd_steps<R, NW, false, false>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb);
+#define GPR_FWD_STEPS(ZP_, XP_) \
+  fwd_steps<R, NW, ZP_, XP_, MU>(a, c, s, rk0, rk1, ent, rflags, src_r, src_c, wv, e, hx, hy, ca, cb)
+    if (c.zp && c.xp) GPR_FWD_STEPS(true, true);
+    else if (c.zp) GPR_FWD_STEPS(true, false);
+    else if (c.xp) GPR_FWD_STEPS(false, true);
+    else GPR_FWD_STEPS(false, false);
+#undef GPR_FWD_STEPS
 
     // ---- write back what this tile owns (out.ez was written by the last E phase) --------------------
 #pragma unroll

@@ -32,8 +32,11 @@ GPR_HD void grad_cell(float er, float sg, float rdt, float gca, float gcb_cb, fl
 }
 
 #if defined(__CUDACC__)
-__global__ void coef_kernel(const float* __restrict__ eps_r, const float* __restrict__ sigma, int upitch,
-                            int nz, int nx, int pitch, float rdt, float* __restrict__ ca, float* __restrict__ cb)
+// mu_r (optional, [nz][upitch]): per-cell Db = (dt/mu0) / mu_r in the internal column order (the paper's uH4,
+// PAPER.md:291-295; reading R22), 0 outside the grid; with mu_r = 1 it equals the scalar Db bit for bit
+__global__ void coef_kernel(const float* __restrict__ eps_r, const float* __restrict__ sigma,
+                            const float* __restrict__ mu_r, int upitch, int nz, int nx, int pitch, float rdt,
+                            float Db, float* __restrict__ ca, float* __restrict__ cb, float* __restrict__ dbc)
 {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y;
@@ -45,6 +48,7 @@ __global__ void coef_kernel(const float* __restrict__ eps_r, const float* __rest
     coef_cell(eps_r[(long long)j * upitch + i], sigma[(long long)j * upitch + i], rdt, a, b);
   ca[(long long)j * pitch + col_pos(i)] = a;          // internal column order: gprfwi_common.cuh
   cb[(long long)j * pitch + col_pos(i)] = b;
+  if (mu_r) dbc[(long long)j * pitch + col_pos(i)] = i < nx ? __fdiv_rn(Db, mu_r[(long long)j * upitch + i]) : 0.f;
 }
 
 __global__ void grad_finalize_kernel(const float* __restrict__ eps_r, const float* __restrict__ sigma, int upitch,

@@ -68,7 +68,11 @@ struct RegTile {
   static constexpr int HIST = (MBAR + 16 + 31) / 32 * 32;      // 128-byte aligned: TMA destination
   static constexpr int LAND = HIST + NH * ROWS * kRegW + 32;   // 128-byte aligned: the psi region doubles as a TMA landing zone
   static constexpr int PSI = LAND + GPRFWI_SMEM_PAD;
-  GPR_HD static size_t smem_bytes(bool pml) { return sizeof(float) * (size_t)(PSI + (pml ? 4 * ROWS * kRegW : 0)); }
+  // (a problem with a mu_r model appends one more [ROWS][128] array: the per-cell Db of the region, thread-private)
+  GPR_HD static size_t smem_bytes(bool pml, bool mu = false)
+  {
+    return sizeof(float) * (size_t)(PSI + (pml ? 4 * ROWS * kRegW : 0) + (mu ? ROWS * kRegW : 0));
+  }
 };
 
 #if defined(__CUDACC__)
@@ -206,6 +210,17 @@ struct TileCtx {
   __device__ __forceinline__ float* pez_() const { return sm + L::PSI + 1 * L::ROWS * kRegW + toff; }
   __device__ __forceinline__ float* phx_() const { return sm + L::PSI + 2 * L::ROWS * kRegW + toff; }
   __device__ __forceinline__ float* pex_() const { return sm + L::PSI + 3 * L::ROWS * kRegW + toff; }
+  // per-cell Db = dt / (mu0 mu_r) of the thread's cells (only when the problem has a mu_r model)
+  __device__ __forceinline__ float* dbc_(const Geo& g) const { return sm + L::PSI + (g.P > 0 ? 4 : 0) * L::ROWS * kRegW + toff; }
+  __device__ __forceinline__ void load_dbc(const Geo& g, const float* dbc) const
+  {
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      P2 v = zero2();
+      if (colin && ((rin >> r) & 1u)) v = ldg2(dbc + (long long)(gj0 + r) * g.pitch + gi);
+      st2(dbc_(g) + r * kRegW, v);
+    }
+  }
 
   __device__ __forceinline__ void init(float* sm_, const Geo& g, int tile_x, int tile_y, int oz, int hz)
   {
@@ -234,11 +249,12 @@ struct TileCtx {
 
   // CPML tables of the region's rows and columns -> shared memory (outside the grid: b = c = 0, 1/kappa = 1).
   // FWD: (b, c/dx, Db/(dx kappa)) at H nodes and (b, c/dx, 1/kappa) at E nodes; else (b, c, 1/kappa) at both.
+  // (FWD with a mu_r model: Db is per cell, so the H sets keep the bare 1/kappa and the kernel multiplies)
   template <bool FWD>
-  __device__ __forceinline__ void stage_tables(const Geo& g) const
+  __device__ __forceinline__ void stage_tables(const Geo& g, bool mu = false) const
   {
-    const int r1 = FWD ? 3 : 1, r2h = FWD ? 4 : 2;
-    const float k0 = FWD ? g.kap : 1.f;
+    const int r1 = FWD ? 3 : 1, r2h = (FWD && !mu) ? 4 : 2;
+    const float k0 = (FWD && !mu) ? g.kap : 1.f;
     if (w == 0) {
 #pragma unroll
       for (int c = 0; c < 4; ++c) {

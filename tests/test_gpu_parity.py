@@ -751,3 +751,34 @@ def test_split_batch_multi_call_sum_against_oracle():
     sim.close()
     assert_parity(wl, (tr, ge.cpu().numpy(), gs.cpu().numpy()), (tr_o, ge_o, gs_o), f" {ncalls} calls of {cs} shots",
                   tol_region=1e-3, tol_maxabs=1e-3)           # (white-noise residual on config 5: see above)
+
+
+def test_mu_r_model_against_oracle_and_unit_permeability_bit_identical():
+    """SURVEY 8(f)-3, reading R22: a heterogeneous relative permeability (Table 1 `miu`) through
+    gprfwi_forward_mu against the oracle (ragged grid, CPML, several tiles, stored history and
+    checkpoint-and-recompute), and mu_r = 1 everywhere bit-identical to the call without a mu_r model."""
+    wl = gi.small_random(nz=97, nx=263, nt=180, npml=12, nshots=3, nrec=7, seed=97263)
+    rng = np.random.default_rng(11)
+    mu = rng.uniform(1.0, 3.0, (wl.nz, wl.nx)).astype(np.float32)
+    pb = problem(wl)
+    tr_o = oracle.forward(pb, wl.eps_r, wl.sigma, mu_r=mu)["traces"]
+    res = gi.random_residual(wl, float(np.sqrt(np.mean(tr_o ** 2))))
+    ge_o, gs_o = oracle.gradient(pb, wl.eps_r, wl.sigma, res, mu_r=mu)
+    assert rel_l2(tr_o, oracle.forward(pb, wl.eps_r, wl.sigma)["traces"]) > 1e-2        # mu_r matters here
+    pitch = wl.nx + 5
+    e = torch.as_tensor(padded(wl.eps_r, pitch), device=dev()); s_ = torch.as_tensor(padded(wl.sigma, pitch), device=dev())
+    ones = torch.ones((wl.nz, pitch), device=dev())
+    m = torch.as_tensor(padded(mu, pitch), device=dev()); m[:, wl.nx:] = 1.0
+    out = {}
+    for K in (0, 16):
+        sim = Simulation(params_of(wl, pitch=pitch, checkpoint_stride=K), wl.src_zx, wl.rec_zx, wl.wavelet, dev())
+        sim.workspace.fill_(0xFF)
+        for tag, model in (("none", None), ("ones", ones), ("mu", m)):
+            tr = sim.forward(e, s_, mu_r=model).cpu().numpy().copy()
+            a, b = sim.adjoint(torch.as_tensor(res, device=dev()))
+            out[tag, K] = (tr, a.cpu().numpy()[:, :wl.nx].copy(), b.cpu().numpy()[:, :wl.nx].copy())
+        sim.close()
+        for x, y in zip(out["none", K], out["ones", K]):
+            assert np.array_equal(x, y)
+        assert_parity(wl, out["mu", K], (tr_o, ge_o, gs_o), f" mu_r model, K = {K}")
+    assert np.array_equal(out["mu", 0][0], out["mu", 16][0])
