@@ -490,6 +490,19 @@ static int build_geometry(gprfwi_handle* h, const int32_t* src_zx, const int32_t
         h_reg_mask[((size_t)s * natile + t) * 2 + (row >> 5)] |= 1u << (row & 31);
         ++nent;
       }
+      // receivers of this region that share their cell: flag them (summed atomically by the kernel)
+      {
+        const size_t lo = (size_t)h_reg_start[(size_t)s * natile + t];
+        if (nent - lo > 1) {
+          std::vector<int> cells;
+          for (size_t k = lo; k < nent; ++k) cells.push_back(h_reg_ent[2 * k]);
+          std::sort(cells.begin(), cells.end());
+          for (size_t k = lo; k < nent; ++k) {
+            const auto r2 = std::equal_range(cells.begin(), cells.end(), h_reg_ent[2 * k]);
+            if (r2.second - r2.first > 1) h_reg_ent[2 * k] |= kEntShared;
+          }
+        }
+      }
       h_reg_start[(size_t)s * natile + t + 1] = (int)nent;
     }
   }

@@ -66,18 +66,31 @@ __device__ long long g_probe[kMaxGroup][16][12];
 // it is staged in rowbuf (zero between uses) one barrier ahead of its use.  The receivers of the
 // region are dealt out one per thread (its residual samples of the launch sit in the thread's private
 // shared-memory slot).
+// Rare paths, kept out of line so that they do not sit in the step loop's instruction stream (the loops'
+// code size matters: DESIGN.md section 9): receivers beyond the first THREADS of a region, and receivers
+// that share their cell with another one of the region (the shared-memory float add is a CAS loop).
+__device__ __noinline__ void adj_stage_overflow(const AdjArgs& a, float* rowbuf, int threads, int s, int rk0, int rk1, int t)
+{
+  for (int k = rk0 + threads + threadIdx.x; k < rk1; k += threads) {
+    const int2 e2 = a.reg_ent[k];
+    atomicAdd(rowbuf + (e2.x & kEntMask), a.residual[s * a.trace_stride - (long long)t * a.nrec + e2.y]);
+  }
+}
+__device__ __noinline__ void adj_stage_shared_cell(float* cell, float v) { atomicAdd(cell, v); }
+
 template <int R, int NW>
 __device__ __forceinline__ void adj_stage(const AdjArgs& a, const TileCtx<R, NW, kAdjRing>& c, int s, int rk0, int rk1,
                                           int entx, int t)
 {
   using L = RegTile<R, NW, kAdjRing>;
   if (a.n_hi - t >= a.nt) return;
-  if (entx >= 0) atomicAdd(c.rowbuf_() + entx, c.priv_()[t]);          // coincident receivers sum
-  if (rk1 - rk0 > L::THREADS)                                                // more receivers than threads
-    for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {
-      const int2 e2 = a.reg_ent[k];
-      atomicAdd(c.rowbuf_() + e2.x, a.residual[s * a.trace_stride - (long long)t * a.nrec + e2.y]);
-    }
+  if (entx >= 0) {
+    // a cell that holds one receiver of the region has one writer (rowbuf is zero between uses);
+    // coincident receivers (entry flagged by the host) sum atomically
+    if (entx & kEntShared) adj_stage_shared_cell(c.rowbuf_() + (entx & kEntMask), c.priv_()[t]);
+    else c.rowbuf_()[entx] = c.priv_()[t];
+  }
+  if (rk1 - rk0 > L::THREADS) adj_stage_overflow(a, c.rowbuf_(), L::THREADS, s, rk0, rk1, t);   // more receivers than threads
 }
 
 // The forward Ez planes a CTA reads form one stream: planes 0 .. nsub of its first shot (plane t =

@@ -46,6 +46,15 @@ struct FwdArgs {
 };
 
 #if defined(__CUDACC__)
+// rare path, out of line (code size of the step loop): receivers of a tile beyond its first THREADS
+__device__ __noinline__ void fwd_record_overflow(const FwdArgs& a, const float* rowbuf, int threads, int s, int rk0, int rk1, int t)
+{
+  for (int k = rk0 + threads + threadIdx.x; k < rk1; k += threads) {
+    const int2 en2 = a.blk_ent[(long long)s * a.nrec + k];
+    a.traces[s * a.trace_stride + (long long)t * a.nrec + en2.y] = rowbuf[en2.x];
+  }
+}
+
 // The T-step loop of one warp.  All variants hit the same barriers, so the warps of one CTA may run
 // different variants.  Every field row of the thread is two packed pairs P = (c0, c2), Q = (c1, c3):
 // differences to the right / left neighbour are Q - P resp. P - Q for half the cells and need one
@@ -67,11 +76,7 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
   for (int t = 0; t < a.nsub; ++t) {
     // ---- stage 1: trace sample n + t from the published receiver rows ----------------------------
     if (ent.x >= 0) trp[(long long)t * a.nrec] = c.rowbuf_()[ent.x];
-    if (rk1 - rk0 > L::THREADS)                                                   // more receivers than threads
-      for (int k = rk0 + L::THREADS + threadIdx.x; k < rk1; k += L::THREADS) {
-        const int2 en2 = a.blk_ent[(long long)s * a.nrec + k];
-        a.traces[s * a.trace_stride + (long long)t * a.nrec + en2.y] = c.rowbuf_()[en2.x];
-      }
+    if (rk1 - rk0 > L::THREADS) fwd_record_overflow(a, c.rowbuf_(), L::THREADS, s, rk0, rk1, t);   // more receivers than threads
 
     // ---- stages 2-3: H update + H CPML -------------------------------------------------------------
     // x tables of this lane's columns (XP only; every lane of an XP warp runs the psi form -- lanes off

@@ -48,6 +48,10 @@ constexpr int kRegW = 128;     // region width  = 32 lanes x float4
 constexpr int kOwnW = 120;     // owned width   = lanes 1..30
 constexpr int kMaxGroup = 32;  // shots one CTA sweeps at most (size of the per-shot scalar table in shared memory)
 constexpr int kMetaW = 12;     // words per shot in that table
+// adjoint receiver entries: row*128 + column inside the region, plus a flag when another receiver of the
+// region sits on the same cell (then the residual samples are summed atomically)
+constexpr int kEntShared = 1 << 30;
+constexpr int kEntMask = kEntShared - 1;
 #ifndef GPRFWI_ADJ_RING
 #define GPRFWI_ADJ_RING 4
 #endif
