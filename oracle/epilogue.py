@@ -89,3 +89,63 @@ def lowpass(x, taps):
         if lo < hi:                                   # (taps may be longer than the series)
             out[:, lo:hi] += h * x[:, lo + sh:hi + sh]
     return out
+
+
+def lowpass_design(dt, f_cut, ntaps=0):
+    """Taps of the multiscale stage filter (PAPER.md:529-531 gives no design; reading R21): Hamming-windowed
+    sinc with corner f_cut, scaled to unit gain at DC; ntaps <= 0 picks 4 / (f_cut dt) rounded up to odd.
+    h[k] = sinc(2 f_cut dt (k - M)) (0.54 - 0.46 cos(2 pi k / (ntaps - 1))), M = (ntaps - 1)/2, h /= sum(h).
+    Pin: equals scipy.signal.firwin(ntaps, f_cut, window="hamming", fs=1/dt) (tests/test_oracle_pins.py)."""
+    if ntaps <= 0:
+        ntaps = int(4.0 / (f_cut * dt)) | 1
+    m = (ntaps - 1) / 2.0
+    k = np.arange(ntaps, dtype=np.float64)
+    h = np.sinc(2.0 * f_cut * dt * (k - m))
+    if ntaps > 1:
+        h = h * (0.54 - 0.46 * np.cos(2.0 * np.pi * k / (ntaps - 1)))
+    return h / h.sum()
+
+
+# ------------------------------------------------------------------------------------------------
+# Coarser grid for the early multiscale stages (PAPER.md:531: "early-stage use of coarse grids and
+# low-frequency data"; the paper gives no transfer operators -- reading R23): node-aligned 2:1 coarsening,
+# coarse node (J, I) = fine node (2J, 2I); n_c = (n + 1) // 2 nodes per axis.
+# ------------------------------------------------------------------------------------------------
+def _w121(n, nc):
+    """[nc][n] full-weighting matrix along one axis: (1/4, 1/2, 1/4) around fine node 2J, the weight of a
+    neighbour outside the grid folded onto the centre (so rows sum to 1 and constants are kept)."""
+    w = np.zeros((nc, n))
+    for J in range(nc):
+        c = 2 * J
+        w[J, c] += 0.5
+        for nb in (c - 1, c + 1):
+            w[J, nb if 0 <= nb < n else c] += 0.25
+    return w
+
+
+def restrict(fine):
+    """Full-weighting restriction of a node-centred model [nz][nx] -> [(nz+1)//2][(nx+1)//2]: the tensor
+    product of (1/4, 1/2, 1/4) stencils centred on the fine nodes (2J, 2I)."""
+    fine = np.asarray(fine, dtype=np.float64)
+    nz, nx = fine.shape
+    return _w121(nz, (nz + 1) // 2) @ fine @ _w121(nx, (nx + 1) // 2).T
+
+
+def _interp(n, nc):
+    """[n][nc] linear interpolation along one axis: even fine nodes copy coarse node j/2, odd ones average
+    their two coarse neighbours (the last node of an even-sized axis copies the last coarse node)."""
+    p = np.zeros((n, nc))
+    for j in range(n):
+        if j % 2 == 0:
+            p[j, j // 2] = 1.0
+        else:
+            lo, hi = j // 2, min(j // 2 + 1, nc - 1)
+            p[j, lo] += 0.5
+            p[j, hi] += 0.5
+    return p
+
+
+def prolong(coarse, nz, nx):
+    """Bilinear prolongation [nzc][nxc] -> [nz][nx] (the transfer back of a coarse-stage model update)."""
+    coarse = np.asarray(coarse, dtype=np.float64)
+    return _interp(nz, coarse.shape[0]) @ coarse @ _interp(nx, coarse.shape[1]).T

@@ -46,7 +46,7 @@ def read_table():
         return list(csv.DictReader(f))
 
 
-def read_raw(path: str, kernel_regex: str):
+def read_raw(path: str, kernel_regex: str, grid: str | None = None):
     """-> list of dict(read, write, seconds) per captured launch whose kernel name matches."""
     with open(path, newline="") as f:
         rows = [r for r in csv.reader(f) if r]
@@ -61,6 +61,8 @@ def read_raw(path: str, kernel_regex: str):
     out = []
     for r in data:
         if len(r) < len(head) or not re.search(kernel_regex, r[col["Kernel Name"]]):
+            continue
+        if grid is not None and r[col["Grid Size"]].replace(" ", "") != grid.replace(" ", ""):
             continue
         out.append({"read": val(r, "dram__bytes_read.sum"), "write": val(r, "dram__bytes_write.sum"),
                     "seconds": val(r, "gpu__time_duration.sum"), "grid": r[col["Grid Size"]],
@@ -77,8 +79,9 @@ def main():
     ap.add_argument("--cell-steps", type=float, required=True, help="cell-steps one captured launch advances")
     ap.add_argument("--source", required=True, help="the tracked profiles/ file the capture is summarised in")
     ap.add_argument("--sha", default=None, help="csrc hash of the captured build (default: the tree's)")
+    ap.add_argument("--grid", default=None, help='only launches with this grid, e.g. "(18, 38, 1)"')
     a = ap.parse_args()
-    launches = read_raw(a.raw_csv, a.kernel)
+    launches = read_raw(a.raw_csv, a.kernel, a.grid)
     if not launches:
         raise SystemExit("no launch of that kernel in the capture")
     per = statistics.mean((l["read"] + l["write"]) for l in launches) / a.cell_steps

@@ -531,3 +531,47 @@ def test_mu_r_of_one_is_the_default():
                           oracle.forward(pb, wl.eps_r, wl.sigma, mu_r=one)["traces"])
     for a_, b_ in zip(oracle.gradient(pb, wl.eps_r, wl.sigma, y), oracle.gradient(pb, wl.eps_r, wl.sigma, y, mu_r=one)):
         assert np.array_equal(a_, b_)
+
+
+# ------------------------------------------------------------------------------------------------
+# multiscale stage filter design and grid transfer operators (readings R21, R23)
+# ------------------------------------------------------------------------------------------------
+def test_lowpass_design_equals_scipy_firwin():
+    """The stage filter's taps against a library routine: scipy.signal.firwin with a Hamming window."""
+    from scipy.signal import firwin
+    from oracle import epilogue as ep
+    for dt, f_cut, ntaps in ((2e-11, 150e6, 0), (1e-10, 80e6, 0), (2e-11, 400e6, 33), (1e-11, 1e9, 1)):
+        h = ep.lowpass_design(dt, f_cut, ntaps)
+        assert len(h) % 2 == 1 and (ntaps <= 0 or len(h) == ntaps)
+        assert abs(h.sum() - 1.0) < 1e-14 and np.allclose(h, h[::-1], atol=1e-16)
+        assert np.allclose(h, firwin(len(h), f_cut, window="hamming", fs=1.0 / dt), rtol=1e-12, atol=1e-15)
+    assert len(ep.lowpass_design(2e-11, 150e6)) == (int(4.0 / (150e6 * 2e-11)) | 1)
+
+
+def test_grid_transfer_operators():
+    """restrict / prolong (R23): constants and (away from the edges) linear fields are reproduced exactly;
+    prolong(restrict(f)) differs from a smooth f by O(h^2) (error / 4 when the grid is refined by 2);
+    shapes follow n_c = (n + 1) // 2 on odd and even axes; restrict of a single fine node is the 1-2-1 stencil."""
+    from oracle import epilogue as ep
+    for nz, nx in ((41, 57), (40, 56), (33, 34)):
+        c = ep.restrict(np.full((nz, nx), 3.25))
+        assert c.shape == ((nz + 1) // 2, (nx + 1) // 2) and np.allclose(c, 3.25, rtol=0, atol=1e-14)
+        assert np.allclose(ep.prolong(c, nz, nx), 3.25, rtol=0, atol=1e-14)
+        z, x = np.meshgrid(np.arange(nz, dtype=float), np.arange(nx, dtype=float), indexing="ij")
+        lin = 2.0 + 0.3 * z - 0.7 * x
+        r = ep.restrict(lin)
+        assert np.allclose(r[1:-1, 1:-1], lin[2:-2:2, 2:-2:2][:r.shape[0] - 2, :r.shape[1] - 2], atol=1e-12)
+        back = ep.prolong(lin[::2, ::2], nz, nx)            # injection then bilinear: exact for linear fields
+        assert np.allclose(back[:2 * (r.shape[0] - 1) + 1, :2 * (r.shape[1] - 1) + 1],
+                           lin[:2 * (r.shape[0] - 1) + 1, :2 * (r.shape[1] - 1) + 1], atol=1e-12)
+    d = np.zeros((9, 9)); d[4, 4] = 1.0
+    assert np.allclose(ep.restrict(d)[1:4, 1:4], np.outer([0, 0.5, 0], [0, 0.5, 0]) + 0, atol=1e-15)
+    d[4, 4] = 0.0; d[3, 4] = 1.0                              # an odd fine node feeds its two coarse neighbours
+    assert np.allclose(ep.restrict(d)[:, 2], [0, 0.125, 0.125, 0, 0], atol=1e-15)
+    errs = []
+    for n in (33, 65, 129):
+        t = np.linspace(0.0, 1.0, n)
+        f = np.sin(2 * np.pi * t)[:, None] * np.cos(3 * np.pi * t)[None, :] + t[:, None] ** 2
+        e = ep.prolong(ep.restrict(f), n, n) - f
+        errs.append(np.abs(e[4:-4, 4:-4]).max())
+    assert 3.3 < errs[0] / errs[1] < 4.7 and 3.3 < errs[1] / errs[2] < 4.7, errs
