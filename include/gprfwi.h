@@ -190,10 +190,29 @@ int gprfwi_update(int32_t nz, int32_t nx, int32_t pitch, const gprfwi_update_par
  * traces or wavelets before a low-frequency stage.
  *   in, out  device [nseries][nt][nrec] (nrec = 1 for wavelets), out != in
  *   taps     device [ntaps], ntaps odd; out[n] = sum_k taps[k] in[n + k - (ntaps-1)/2], zero outside [0, nt)
- * The filter design (cut-off, window) is the caller's: any symmetric taps give zero phase.
+ * The filter design (cut-off, window) is the caller's (gprfwi_lowpass_design gives the one of reading R21):
+ * any symmetric taps give zero phase.
  * Errors: EINVAL (null pointer, in == out, nt/nrec/nseries < 1, ntaps even or < 1), ECUDA. */
 int gprfwi_lowpass(const float* in, float* out, int32_t nseries, int32_t nt, int32_t nrec,
                    const float* taps, int32_t ntaps, void* cuda_stream);
+
+/* Taps of the stage filter for gprfwi_lowpass (the paper gives no design; DESIGN.md reading
+ * R21): Hamming-windowed sinc with corner f_cut (Hz) at sampling interval dt (s), unit gain at DC, computed on
+ * the HOST.  ntaps <= 0 picks 4/(f_cut dt) rounded up to odd.  taps: host [ntaps] or NULL (size query).
+ * Returns the number of taps (> 0), or GPRFWI_EINVAL (non-positive dt / f_cut, even ntaps). */
+int32_t gprfwi_lowpass_design(float dt, float f_cut, int32_t ntaps, float* taps);
+
+/* Coarse grid of the early multiscale stages (reading R23): node-aligned 2:1
+ * coarsening, coarse node (J, I) = fine node (2J, 2I), (nz+1)/2 x (nx+1)/2 coarse nodes.
+ * gprfwi_restrict: coarse = full weighting of fine (tensor product of (1/4, 1/2, 1/4); a neighbour outside
+ * the grid folds onto the centre).  gprfwi_prolong_add: fine += scale * bilinear interpolation of coarse
+ * (how a coarse stage's model update returns to the fine model).
+ *   fine    device [nz][pitch];  coarse  device [(nz+1)/2][pitch_coarse], pitch_coarse >= (nx+1)/2
+ * Both enqueue on the stream.  Errors: EINVAL (null / aliased pointers, nz or nx < 3, pitches too small), ECUDA. */
+int gprfwi_restrict(const float* fine, int32_t nz, int32_t nx, int32_t pitch, float* coarse, int32_t pitch_coarse,
+                    void* cuda_stream);
+int gprfwi_prolong_add(const float* coarse, int32_t pitch_coarse, float scale, float* fine, int32_t nz, int32_t nx,
+                       int32_t pitch, void* cuda_stream);
 
 /* Number of kernel launches enqueued by the last forward / adjoint on this handle. */
 int64_t gprfwi_launch_count(const gprfwi_handle* h);

@@ -18,6 +18,7 @@ EXPORTS = (
     "gprfwi_workspace_bytes", "gprfwi_forward", "gprfwi_forward_mu", "gprfwi_adjoint", "gprfwi_gradient_host",
     "gprfwi_workspace_bytes_host", "gprfwi_residual", "gprfwi_launch_count", "gprfwi_get_plan",
     "gprfwi_release", "gprfwi_strerror", "gprfwi_version", "gprfwi_update", "gprfwi_update_workspace_bytes", "gprfwi_lowpass",
+    "gprfwi_lowpass_design", "gprfwi_restrict", "gprfwi_prolong_add",
 )
 
 
@@ -100,6 +101,13 @@ def _declare(lib):
                                   fp, fp, fp, fp, fp, fp, fp, fp, vp, sz, vp]
     lib.gprfwi_lowpass.restype = ctypes.c_int
     lib.gprfwi_lowpass.argtypes = [fp, fp, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, fp, ctypes.c_int32, vp]
+    lib.gprfwi_lowpass_design.restype = ctypes.c_int32
+    lib.gprfwi_lowpass_design.argtypes = [ctypes.c_float, ctypes.c_float, ctypes.c_int32, fp]
+    lib.gprfwi_restrict.restype = ctypes.c_int
+    lib.gprfwi_restrict.argtypes = [fp, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, fp, ctypes.c_int32, vp]
+    lib.gprfwi_prolong_add.restype = ctypes.c_int
+    lib.gprfwi_prolong_add.argtypes = [fp, ctypes.c_int32, ctypes.c_float, fp, ctypes.c_int32, ctypes.c_int32,
+                                       ctypes.c_int32, vp]
     lib.gprfwi_version.restype = ctypes.c_int
     return lib
 

@@ -190,13 +190,34 @@ def gprfwi_lowpass(x: torch.Tensor, out: torch.Tensor, taps: torch.Tensor, strea
     return out
 
 
-def lowpass_taps(dt: float, f_cut: float, ntaps: int = 0) -> np.ndarray:
-    """Hamming-windowed sinc, unit DC gain (harness-side filter design; the ABI takes any taps)."""
-    if ntaps <= 0:
-        ntaps = int(4.0 / (f_cut * dt)) | 1
-    k = np.arange(ntaps) - (ntaps - 1) / 2
-    h = np.sinc(2.0 * f_cut * dt * k) * np.hamming(ntaps)
-    return (h / h.sum()).astype(np.float32)
+def gprfwi_lowpass_design(dt: float, f_cut: float, ntaps: int = 0) -> np.ndarray:
+    """Taps of the stage filter (host call into the library; reading R21) as a float32 NumPy array."""
+    lib = _lib.load()
+    n = int(lib.gprfwi_lowpass_design(float(dt), float(f_cut), int(ntaps), None))
+    check(min(n, 0))
+    taps = np.empty(n, dtype=np.float32)
+    check(min(int(lib.gprfwi_lowpass_design(float(dt), float(f_cut), n, taps.ctypes.data)), 0))
+    return taps
+
+
+def gprfwi_restrict(fine: torch.Tensor, coarse: torch.Tensor = None, stream=None) -> torch.Tensor:
+    """Full-weighting 2:1 restriction of a model plane [nz][nx] -> [(nz+1)//2][(nx+1)//2] (reading R23)."""
+    nz, nx = fine.shape
+    if coarse is None:
+        coarse = torch.empty(((nz + 1) // 2, (nx + 1) // 2), dtype=torch.float32, device=fine.device)
+    check(_lib.load().gprfwi_restrict(_dev(fine, "fine"), nz, nx, fine.stride(0), _dev(coarse, "coarse"),
+                                      coarse.stride(0), _stream_ptr(stream)))
+    return coarse
+
+
+def gprfwi_prolong_add(coarse: torch.Tensor, fine: torch.Tensor, scale: float = 1.0, stream=None) -> torch.Tensor:
+    """fine += scale * bilinear prolongation of coarse (reading R23)."""
+    nz, nx = fine.shape
+    if tuple(coarse.shape) != ((nz + 1) // 2, (nx + 1) // 2):
+        raise ValueError("coarse must have shape ((nz+1)//2, (nx+1)//2)")
+    check(_lib.load().gprfwi_prolong_add(_dev(coarse, "coarse"), coarse.stride(0), float(scale), _dev(fine, "fine"),
+                                         nz, nx, fine.stride(0), _stream_ptr(stream)))
+    return fine
 
 
 class Simulation:
@@ -285,6 +306,48 @@ class Stage:
     lr_sigma: float
     f_cut: float | None = None
     ntaps: int = 0
+    coarsen: bool = False      # run this stage on the 2:1 coarse grid (reading R23)
+
+
+def coarse_problem(p: Params, src_zx, rec_zx):
+    """The 2:1 coarse counterpart of a problem (reading R23): same dt and nt, dx doubled, CPML thickness halved
+    (rounded up) with sigma_max halved (it scales like 1/dx), sources and receivers on the nearest coarse node
+    inside the PEC ring.  Host-side bookkeeping only."""
+    nzc, nxc = (p.nz + 1) // 2, (p.nx + 1) // 2
+    pc = make_params(nz=nzc, nx=nxc, dx=2.0 * p.dx, dt=p.dt, nt=p.nt, npml=(p.npml + 1) // 2, pml_order=p.pml_order,
+                     pml_sigma_max=0.5 * p.pml_sigma_max, pml_kappa_max=p.pml_kappa_max,
+                     pml_alpha_max=p.pml_alpha_max, nshots=p.nshots, nrec=p.nrec,
+                     wavelet_per_shot=p.wavelet_per_shot)
+
+    def coarse_idx(a):
+        a = (np.asarray(a, dtype=np.int64) + 1) // 2
+        a[..., 0] = np.clip(a[..., 0], 1, nzc - 2)
+        a[..., 1] = np.clip(a[..., 1], 1, nxc - 2)
+        return a.astype(np.int32)
+
+    return pc, coarse_idx(src_zx), coarse_idx(np.asarray(rec_zx).reshape(p.nshots, p.nrec, 2))
+
+
+def _invert_coarse(sim, eps_r, sigma, d_obs, wavelet, st, cb, update_kw):
+    """One stage on the coarse grid: restrict the models, invert there, prolong the model UPDATES back."""
+    pc, src_c, rec_c = coarse_problem(sim.p, sim.src_zx, sim.rec_zx)
+    simc = Simulation(pc, src_c, rec_c, np.zeros(wavelet.numel(), dtype=np.float32), sim.device)
+    simc.wavelet = wavelet
+    try:
+        e0, s0 = gprfwi_restrict(eps_r), gprfwi_restrict(sigma)
+        ec, sc = e0.clone(), s0.clone()
+        kw = dict(update_kw)
+        if "mask_rows" in kw:
+            kw["mask_rows"] = (kw["mask_rows"] + 1) // 2
+        hist = invert(simc, ec, sc, d_obs, iterations=st.iterations, lr_eps_r=st.lr_eps_r, lr_sigma=st.lr_sigma,
+                      callback=cb, **kw)
+        gprfwi_prolong_add(ec.sub_(e0), eps_r)
+        gprfwi_prolong_add(sc.sub_(s0), sigma)
+        eps_r.clamp_(min=kw.get("eps_r_min", 1.0))
+        sigma.clamp_(min=kw.get("sigma_min", 0.0))
+    finally:
+        simc.close()
+    return hist
 
 
 def invert_staged(sim: "Simulation", eps_r: torch.Tensor, sigma: torch.Tensor, d_obs: torch.Tensor, stages,
@@ -300,12 +363,15 @@ def invert_staged(sim: "Simulation", eps_r: torch.Tensor, sigma: torch.Tensor, d
         for k, st in enumerate(stages):
             w, d = full, d_obs
             if st.f_cut is not None:
-                taps = torch.as_tensor(lowpass_taps(sim.p.dt, st.f_cut, st.ntaps), device=dev)
+                taps = torch.as_tensor(gprfwi_lowpass_design(sim.p.dt, st.f_cut, st.ntaps), device=dev)
                 w2 = full.reshape(-1, sim.p.nt)
                 w = gprfwi_lowpass(w2, torch.empty_like(w2), taps).reshape(full.shape)
                 d = gprfwi_lowpass(d_obs, torch.empty_like(d_obs), taps)
             sim.wavelet = w
             cb = None if callback is None else (lambda it, mf, k=k: callback(k, it, mf))
+            if st.coarsen:
+                out.append(_invert_coarse(sim, eps_r, sigma, d, w, st, cb, update_kw))
+                continue
             out.append(invert(sim, eps_r, sigma, d, iterations=st.iterations, lr_eps_r=st.lr_eps_r,
                               lr_sigma=st.lr_sigma, callback=cb, **update_kw))
     finally:

@@ -1198,4 +1198,47 @@ int gprfwi_lowpass(const float* in, float* out, int32_t nseries, int32_t nt, int
   return GPRFWI_OK;
 }
 
+int32_t gprfwi_lowpass_design(float dt, float f_cut, int32_t ntaps, float* taps)
+{
+  if (!(dt > 0.f) || !(f_cut > 0.f)) return GPRFWI_EINVAL;
+  if (ntaps <= 0) ntaps = (int32_t)(4.0 / ((double)f_cut * (double)dt)) | 1;
+  if ((ntaps & 1) == 0) return GPRFWI_EINVAL;
+  if (!taps) return ntaps;
+  // Hamming-windowed sinc, unit DC gain (reading R21), in float64, stored as fp32
+  const double m = 0.5 * (ntaps - 1), fc = 2.0 * (double)f_cut * (double)dt;
+  std::vector<double> h((size_t)ntaps);
+  double sum = 0.0;
+  for (int k = 0; k < ntaps; ++k) {
+    const double x = kPi * fc * (k - m);
+    const double snc = x == 0.0 ? 1.0 : std::sin(x) / x;
+    const double win = ntaps > 1 ? 0.54 - 0.46 * std::cos(2.0 * kPi * k / (ntaps - 1)) : 1.0;
+    h[(size_t)k] = snc * win;
+    sum += h[(size_t)k];
+  }
+  for (int k = 0; k < ntaps; ++k) taps[k] = (float)(h[(size_t)k] / sum);
+  return ntaps;
+}
+
+int gprfwi_restrict(const float* fine, int32_t nz, int32_t nx, int32_t pitch, float* coarse, int32_t pitch_coarse,
+                    void* cuda_stream)
+{
+  if (!fine || !coarse || fine == coarse || nz < 3 || nx < 3 || pitch < nx || pitch_coarse < (nx + 1) / 2) return GPRFWI_EINVAL;
+  const int nzc = (nz + 1) / 2, nxc = (nx + 1) / 2;
+  dim3 grid((nxc + 127) / 128, nzc), block(128);
+  GPR_LAUNCH(restrict_kernel, grid, block, (cudaStream_t)cuda_stream, fine, nz, nx, pitch, coarse, nzc, nxc, pitch_coarse);
+  GPR_CUDA(cudaGetLastError());
+  return GPRFWI_OK;
+}
+
+int gprfwi_prolong_add(const float* coarse, int32_t pitch_coarse, float scale, float* fine, int32_t nz, int32_t nx,
+                       int32_t pitch, void* cuda_stream)
+{
+  if (!fine || !coarse || fine == coarse || nz < 3 || nx < 3 || pitch < nx || pitch_coarse < (nx + 1) / 2) return GPRFWI_EINVAL;
+  const int nzc = (nz + 1) / 2, nxc = (nx + 1) / 2;
+  dim3 grid((nx + 127) / 128, nz), block(128);
+  GPR_LAUNCH(prolong_add_kernel, grid, block, (cudaStream_t)cuda_stream, coarse, nzc, nxc, pitch_coarse, scale, fine, nz, nx, pitch);
+  GPR_CUDA(cudaGetLastError());
+  return GPRFWI_OK;
+}
+
 }  // extern "C"

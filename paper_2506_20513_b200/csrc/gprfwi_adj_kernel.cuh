@@ -17,6 +17,12 @@
 #pragma once
 #include "gprfwi_tile.cuh"
 
+#if defined(GPRFWI_PROBE) && GPRFWI_PROBE == 1
+#define GPR_APROBE(shot, k) GPR_PROBE(shot, k)
+#else
+#define GPR_APROBE(shot, k) do { } while (0)
+#endif
+
 namespace gprfwi {
 
 struct AdjArgs {
@@ -45,27 +51,6 @@ struct AdjArgs {
 };
 
 #if defined(__CUDACC__)
-// Tuning aid (builds with -DGPRFWI_PROBE only): clock64 stamps of every warp of one interior CTA at fixed
-// points of each shot, read back with gprfwi_probe_read (gprfwi.cu).
-#ifdef GPRFWI_PROBE
-#ifndef GPRFWI_PROBE_BX
-#define GPRFWI_PROBE_BX (gridDim.x / 2)
-#define GPRFWI_PROBE_BY (gridDim.y / 2)
-#endif
-__device__ long long g_probe[kMaxGroup][16][12];
-#define GPR_PROBE(shot, k)                                                                          \
-  do {                                                                                              \
-    if (blockIdx.x == GPRFWI_PROBE_BX && blockIdx.y == GPRFWI_PROBE_BY && blockIdx.z == 0 && (threadIdx.x & 31) == 0) \
-      g_probe[(shot)][threadIdx.x >> 5][(k)] = clock64();                                           \
-  } while (0)
-#else
-#define GPR_PROBE(shot, k) do { } while (0)
-#endif
-
-// transpose of recording: residual sample n_hi - t enters lamE at the start of reverse step n_hi-1-t;
-// it is staged in rowbuf (zero between uses) one barrier ahead of its use.  The receivers of the
-// region are dealt out one per thread (its residual samples of the launch sit in the thread's private
-// shared-memory slot).
 // Rare paths, kept out of line so that they do not sit in the step loop's instruction stream (the loops'
 // code size matters: DESIGN.md section 9): receivers beyond the first THREADS of a region, and receivers
 // that share their cell with another one of the region (the shared-memory float add is a CAS loop).
@@ -267,7 +252,7 @@ __device__ __forceinline__ void adj_steps(const AdjArgs& a, const TileCtx<R, NW,
       le[0].p = fma2(rdx2, sub2(sza.p, sz0.p), le[0].p);
       le[0].q = fma2(rdx2, sub2(sza.q, sz0.q), le[0].q);
     }
-    GPR_PROBE(s % a.group, 4 + t);
+    GPR_APROBE(s % a.group, 4 + t);
   }
 }
 
@@ -328,7 +313,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const __grid_constan
   int q0 = 0, nland = 0;               // stream position of this shot's plane 0; state landings so far
   for (int s = s_beg; s < s_end; ++s, q0 += a.nsub + 1) {
     // ---- everything this shot needs from global memory, issued together ----------------------------
-    GPR_PROBE(s - s_beg, 0);
+    GPR_APROBE(s - s_beg, 0);
     const int* m = c.meta_() + (s - s_beg) * 4;
     const int rk0 = m[0], rk1 = m[1];
     const unsigned iflags = (unsigned)((((unsigned long long)(unsigned)m[3] << 32) | (unsigned)m[2]) >> c.lr0) & ((1u << R) - 1u);
@@ -357,7 +342,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const __grid_constan
         }
       }
     }
-    GPR_PROBE(s - s_beg, 1);
+    GPR_APROBE(s - s_beg, 1);
     const bool prefetch = can_land && s + 1 < s_end;
     c.fetch_psi(g, a.in, s);           // (one cp.async group, awaited before the barrier below)
     // this thread's residual samples of this launch, and the receiver it injects for the next shot
@@ -375,10 +360,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const __grid_constan
     *reinterpret_cast<int2*>(c.priv_() + 4) = ent_next;
     const int entx = ent.x;
     adj_stage<R, NW>(a, c, s, rk0, rk1, entx, 0);         // (the previous shot left rowbuf all zero, two barriers ago)
-    GPR_PROBE(s - s_beg, 2);
+    GPR_APROBE(s - s_beg, 2);
     cp_async_wait<0>();
     __syncthreads();
-    GPR_PROBE(s - s_beg, 3);
+    GPR_APROBE(s - s_beg, 3);
 
 #define GPR_ADJ_STEPS(ZP_, XP_) \
   adj_steps<R, NW, ZP_, XP_, MU>(a, c, s, rk0, rk1, entx, iflags, prefetch, q0, s_end, le, lhx, lhy, ca, cb, ga, gb)
@@ -400,7 +385,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) adj_kernel(const __grid_constan
     if (c.zp || c.xp) c.store_psi(g, a.out, s);
     landed = prefetch;
     nland += prefetch ? 1 : 0;
-    GPR_PROBE(s - s_beg, 8);
+    GPR_APROBE(s - s_beg, 8);
   }
 
   // ---- once per CTA: add the register partial sums to this group's gCa / gCb planes --------------------

@@ -19,6 +19,12 @@
 #pragma once
 #include "gprfwi_tile.cuh"
 
+#if defined(GPRFWI_PROBE) && GPRFWI_PROBE == 2
+#define GPR_FPROBE(shot, k) GPR_PROBE(shot, k)
+#else
+#define GPR_FPROBE(shot, k) do { } while (0)
+#endif
+
 namespace gprfwi {
 
 struct FwdArgs {
@@ -192,6 +198,7 @@ __device__ __forceinline__ void fwd_steps(const FwdArgs& a, const TileCtx<R, NW,
     }
     st2(c.xe_() + c.w * kRegW + c.l4, e[0]);
     __syncthreads();
+    GPR_FPROBE(s % a.group, 4 + t);
   }
 }
 
@@ -266,6 +273,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const __grid_constan
 
 #pragma unroll 1
   for (int s = s0; s < s1; ++s) {
+    GPR_FPROBE(s - s0, 0);
     const int* m = c.meta_() + (s - s0) * kMetaW;
     const int rk0 = m[0], rk1 = m[1];
     float wv[kMaxT];
@@ -288,6 +296,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const __grid_constan
       hx[r] = ld2(c.hist_() + 1 * L::ROWS * kRegW + r * kRegW);
       hy[r] = ld2(c.hist_() + 2 * L::ROWS * kRegW + r * kRegW);
     }
+    GPR_FPROBE(s - s0, 1);
     // this warp's R bits of the mask of region rows that hold a receiver of this shot
     const unsigned rflags = (unsigned)((((unsigned long long)(unsigned)m[9] << 32) | (unsigned)m[8]) >> c.lr0) & ((1u << R) - 1u);
     // publish: row 0 for the warp above, the receiver rows for the first trace sample
@@ -305,7 +314,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const __grid_constan
       if (mn[0] + tid < mn[1]) ent_next = a.blk_ent[(long long)(s + 1) * a.nrec + mn[0] + tid];
     }
     cp_async_wait<0>();                // psi landed
+    GPR_FPROBE(s - s0, 2);
     __syncthreads();                   // exchange row and receiver rows published; landing zone free
+    GPR_FPROBE(s - s0, 3);
     if (tid == 0 && s + 1 < s1) fwd_fetch<R, NW>(a, c, s + 1);
 
 #define GPR_FWD_STEPS(ZP_, XP_) \
@@ -325,6 +336,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fwd_kernel(const __grid_constan
       st2(a.out.hy + o, hy[r]);
     }
     if (c.zp || c.xp) c.store_psi(g, a.out, s);
+    GPR_FPROBE(s - s0, 8);
   }
 }
 #endif

@@ -340,6 +340,27 @@ struct TileCtx {
     }
   }
 };
+// Tuning aid (builds with -DGPRFWI_PROBE only): clock64 stamps of every warp of one interior CTA at fixed
+// points of each shot, read back with gprfwi_probe_read (gprfwi.cu).  GPRFWI_PROBE=1: adjoint kernel, 2: forward.
+#ifdef GPRFWI_PROBE
+#ifndef GPRFWI_PROBE_BX
+#define GPRFWI_PROBE_BX (gridDim.x / 2)
+#define GPRFWI_PROBE_BY (gridDim.y / 2)
+#endif
+__device__ long long g_probe[kMaxGroup][16][12];
+#define GPR_PROBE(shot, k)                                                                          \
+  do {                                                                                              \
+    if (blockIdx.x == GPRFWI_PROBE_BX && blockIdx.y == GPRFWI_PROBE_BY && blockIdx.z == 0 && (threadIdx.x & 31) == 0) \
+      g_probe[(shot)][threadIdx.x >> 5][(k)] = clock64();                                           \
+  } while (0)
+#else
+#define GPR_PROBE(shot, k) do { } while (0)
+#endif
+
+// transpose of recording: residual sample n_hi - t enters lamE at the start of reverse step n_hi-1-t;
+// it is staged in rowbuf (zero between uses) one barrier ahead of its use.  The receivers of the
+// region are dealt out one per thread (its residual samples of the launch sit in the thread's private
+// shared-memory slot).
 #endif
 
 }  // namespace gprfwi

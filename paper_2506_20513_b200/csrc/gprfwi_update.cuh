@@ -119,6 +119,44 @@ __global__ void lowpass_kernel(const float* __restrict__ in, float* __restrict__
     out[base + k] = acc;
   }
 }
+
+// ---- coarse grid of the early multiscale stages (reading R23): node-aligned 2:1
+// coarsening, coarse node (J, I) = fine node (2J, 2I).
+// Full-weighting restriction: tensor product of (1/4, 1/2, 1/4) around the fine node, a neighbour outside
+// the grid folded onto the centre.
+__global__ void restrict_kernel(const float* __restrict__ fine, int nz, int nx, int pitch, float* __restrict__ coarse,
+                                int nzc, int nxc, int pitchc)
+{
+  const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y;
+  if (I >= nxc || J >= nzc) return;
+  const int jc = 2 * J, ic = 2 * I;
+  float acc = 0.f;
+#pragma unroll
+  for (int dj = -1; dj <= 1; ++dj) {
+    const int j = (jc + dj >= 0 && jc + dj < nz) ? jc + dj : jc;
+    const float wj = dj == 0 ? 0.5f : 0.25f;
+    float row = 0.f;
+#pragma unroll
+    for (int di = -1; di <= 1; ++di) {
+      const int i = (ic + di >= 0 && ic + di < nx) ? ic + di : ic;
+      row += (di == 0 ? 0.5f : 0.25f) * fine[(long long)j * pitch + i];
+    }
+    acc += wj * row;
+  }
+  coarse[(long long)J * pitchc + I] = acc;
+}
+// fine += scale * bilinear prolongation of coarse (even fine nodes copy, odd ones average their coarse neighbours)
+__global__ void prolong_add_kernel(const float* __restrict__ coarse, int nzc, int nxc, int pitchc, float scale,
+                                   float* __restrict__ fine, int nz, int nx, int pitch)
+{
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= nx || j >= nz) return;
+  const int j0 = j >> 1, j1 = (j & 1) ? min(j0 + 1, nzc - 1) : j0;
+  const int i0 = i >> 1, i1 = (i & 1) ? min(i0 + 1, nxc - 1) : i0;
+  const float v = 0.25f * (coarse[(long long)j0 * pitchc + i0] + coarse[(long long)j0 * pitchc + i1] +
+                           coarse[(long long)j1 * pitchc + i0] + coarse[(long long)j1 * pitchc + i1]);
+  fine[(long long)j * pitch + i] += scale * v;
+}
 #endif
 
 }  // namespace gprfwi

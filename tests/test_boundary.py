@@ -140,3 +140,20 @@ def test_split_batch_prefers_plans_with_several_shots_per_pass():
     assert split_batch(mk(512, 8), budget)[:2] == (1, 8)                  # fits with full history: no split
     with pytest.raises(ValueError):
         split_batch(mk(8192, 4), int(1e9))                                # one shot does not fit 1 GB
+
+
+def test_lowpass_design_host_call_matches_oracle():
+    """gprfwi_lowpass_design runs on the host (no GPU needed): its taps against the oracle's NumPy statement
+    (itself pinned against scipy.signal.firwin), the size query, and the error returns."""
+    import numpy as np
+    from oracle import epilogue as ep
+    lib = _lib.load()
+    for dt, f_cut, ntaps in ((2e-11, 150e6, 0), (1e-10, 80e6, 0), (2e-11, 400e6, 33)):
+        n = lib.gprfwi_lowpass_design(dt, f_cut, ntaps, None)
+        ref = ep.lowpass_design(np.float32(dt), np.float32(f_cut), ntaps)
+        assert n == len(ref)
+        taps = np.zeros(n, dtype=np.float32)
+        assert lib.gprfwi_lowpass_design(dt, f_cut, ntaps, taps.ctypes.data) == n
+        assert np.allclose(taps, ref, rtol=2e-7, atol=1e-9)
+    assert lib.gprfwi_lowpass_design(2e-11, 150e6, 32, None) == -1            # even tap count
+    assert lib.gprfwi_lowpass_design(0.0, 150e6, 0, None) == -1

@@ -527,10 +527,11 @@ def test_inversion_loop_reduces_misfit_and_recovers_anomaly():
 def test_lowpass_matches_oracle():
     """Multiscale stage filter: zero-phase FIR along time of traces and of a wavelet."""
     from oracle import epilogue as ep
-    from paper_2506_20513_b200 import gprfwi_lowpass, lowpass_taps
+    from paper_2506_20513_b200 import gprfwi_lowpass, gprfwi_lowpass_design
     rng = np.random.default_rng(4)
     x = rng.standard_normal((3, 517, 11)).astype(np.float32)
-    taps = lowpass_taps(2e-11, 150e6)
+    taps = gprfwi_lowpass_design(2e-11, 150e6)
+    assert np.allclose(taps, ep.lowpass_design(2e-11, 150e6), rtol=2e-7, atol=1e-9)      # library design vs the oracle's
     assert len(taps) % 2 == 1
     d_x = torch.as_tensor(x, device=dev()); d_t = torch.as_tensor(taps, device=dev())
     y = gprfwi_lowpass(d_x, torch.empty_like(d_x), d_t).cpu().numpy()
@@ -569,7 +570,7 @@ def test_staged_inversion_driver():
     with that stage's (filtered) wavelet and data; sigma does not move while its rate is 0; the
     filtered stage leaves the full-band wavelet in place afterwards; each stage lowers its misfit."""
     from oracle import epilogue as ep
-    from paper_2506_20513_b200 import Stage, invert_staged, lowpass_taps
+    from paper_2506_20513_b200 import Stage, invert_staged
     wl = gi.crosshole(nt=600)
     pb = problem(wl)
     d_obs64 = oracle.forward(pb, wl.eps_r_obs, wl.sigma_obs)["traces"]
@@ -592,7 +593,7 @@ def test_staged_inversion_driver():
     assert np.array_equal(snap[0][1], wl.sigma) and not np.array_equal(snap[0][0], wl.eps_r)
     assert not np.array_equal(snap[1][1], wl.sigma)
     assert hist[0][-1] < hist[0][0] and hist[1][-1] < hist[1][0]
-    taps = lowpass_taps(wl.dt, 80e6)
+    taps = ep.lowpass_design(wl.dt, 80e6)          # the oracle's own statement of the stage filter
     w_lp = ep.lowpass(wl.wavelet[None, :, None], taps)[0, :, 0]
     d_lp = ep.lowpass(d_obs.cpu().numpy(), taps)
     r0 = oracle.forward(problem(wl, wavelet=w_lp), wl.eps_r, wl.sigma)["traces"] - d_lp
@@ -782,3 +783,49 @@ def test_mu_r_model_against_oracle_and_unit_permeability_bit_identical():
             assert np.array_equal(x, y)
         assert_parity(wl, out["mu", K], (tr_o, ge_o, gs_o), f" mu_r model, K = {K}")
     assert np.array_equal(out["mu", 0][0], out["mu", 16][0])
+
+
+def test_grid_transfer_kernels_and_coarse_stage():
+    """SURVEY 8(f)-2 remainder (reading R23): gprfwi_restrict / gprfwi_prolong_add against the
+    NumPy oracle on odd and even grids with a row pitch, and a coarse-grid stage of invert_staged: its first
+    misfit equals the oracle's misfit of the COARSE problem (restricted models, doubled dx, halved CPML,
+    geometry on the nearest coarse nodes, low-passed wavelet and data), the fine models move by the
+    prolongation of the coarse update, and the stage lowers its misfit."""
+    from oracle import epilogue as ep
+    from paper_2506_20513_b200 import (Stage, invert_staged, coarse_problem, gprfwi_restrict, gprfwi_prolong_add)
+    rng = np.random.default_rng(31)
+    for nz, nx in ((41, 57), (40, 130), (97, 263)):
+        f = rng.standard_normal((nz, nx)).astype(np.float32)
+        d_f = torch.zeros((nz, nx + 3), device=dev()); d_f[:, :nx] = torch.as_tensor(f, device=dev())
+        d_c = gprfwi_restrict(d_f[:, :nx])
+        assert rel_l2(d_c.cpu().numpy(), ep.restrict(f)) <= 1e-6
+        base = rng.standard_normal((nz, nx)).astype(np.float32)
+        d_b = torch.as_tensor(base.copy(), device=dev())
+        gprfwi_prolong_add(d_c, d_b, scale=-0.5)
+        assert rel_l2(d_b.cpu().numpy(), base - 0.5 * ep.prolong(d_c.cpu().numpy(), nz, nx)) <= 1e-6
+        assert torch.all(d_f[:, nx:] == 0)
+    wl = gi.crosshole(nt=600)
+    pb = problem(wl)
+    d_obs64 = oracle.forward(pb, wl.eps_r_obs, wl.sigma_obs)["traces"]
+    d_obs = torch.as_tensor(d_obs64.astype(np.float32), device=dev())
+    sim = Simulation(params_of(wl), wl.src_zx, wl.rec_zx, wl.wavelet, dev())
+    eps = torch.as_tensor(wl.eps_r.copy(), device=dev()); sig = torch.as_tensor(wl.sigma.copy(), device=dev())
+    hist = invert_staged(sim, eps, sig, d_obs, [Stage(4, 0.05, 0.0, f_cut=60e6, coarsen=True)], mask_rows=0,
+                         tv_iters=3, tv_lambda=0.002, tv_alpha=0.0)
+    pc, src_c, rec_c = coarse_problem(sim.p, wl.src_zx, wl.rec_zx)
+    sim.close()
+    print("[coarse stage]", " ".join(f"{h:.3e}" for h in hist[0]))
+    assert (pc.nz, pc.nx, pc.npml) == ((wl.nz + 1) // 2, (wl.nx + 1) // 2, (wl.npml + 1) // 2)
+    taps = ep.lowpass_design(wl.dt, 60e6)
+    w_lp = ep.lowpass(wl.wavelet[None, :, None], taps)[0, :, 0]
+    d_lp = ep.lowpass(d_obs.cpu().numpy(), taps)
+    pbc = oracle.Problem(nz=pc.nz, nx=pc.nx, dx=2.0 * wl.dx, dt=wl.dt, nt=wl.nt, npml=pc.npml, pml_order=wl.pml_order,
+                         pml_sigma_max=0.5 * wl.pml_sigma_max, pml_kappa_max=wl.pml_kappa_max,
+                         pml_alpha_max=wl.pml_alpha_max, src_zx=src_c, rec_zx=rec_c, wavelet=w_lp)
+    r0 = oracle.forward(pbc, ep.restrict(wl.eps_r), ep.restrict(wl.sigma))["traces"] - d_lp
+    assert abs(hist[0][0] - 0.5 * np.sum(r0 * r0)) <= 1e-3 * hist[0][0]
+    assert hist[0][-1] < hist[0][0]
+    de = eps.cpu().numpy() - wl.eps_r
+    assert np.abs(de).max() > 0 and torch.equal(sig.cpu(), torch.as_tensor(wl.sigma))      # lr_sigma = 0
+    # the update is a bilinear field: it is reproduced by prolonging its own values at the even nodes
+    assert rel_l2(ep.prolong(de[::2, ::2], wl.nz, wl.nx), de) <= 1e-5
