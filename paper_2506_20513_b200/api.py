@@ -33,6 +33,13 @@ def _dev(t: torch.Tensor, name: str, n: int | None = None) -> int:
     return t.data_ptr()
 
 
+def _plane(t: torch.Tensor, name: str) -> int:
+    """A 2-D fp32 CUDA plane whose rows are contiguous (the row stride is passed on as the pitch)."""
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float32 or t.dim() != 2 or t.stride(1) != 1:
+        raise TypeError(f"{name} must be a 2-D float32 CUDA tensor with contiguous rows")
+    return t.data_ptr()
+
+
 def _i32(a, shape, name):
     a = np.ascontiguousarray(a, dtype=np.int32)
     if a.shape != shape:
@@ -205,7 +212,7 @@ def gprfwi_restrict(fine: torch.Tensor, coarse: torch.Tensor = None, stream=None
     nz, nx = fine.shape
     if coarse is None:
         coarse = torch.empty(((nz + 1) // 2, (nx + 1) // 2), dtype=torch.float32, device=fine.device)
-    check(_lib.load().gprfwi_restrict(_dev(fine, "fine"), nz, nx, fine.stride(0), _dev(coarse, "coarse"),
+    check(_lib.load().gprfwi_restrict(_plane(fine, "fine"), nz, nx, fine.stride(0), _plane(coarse, "coarse"),
                                       coarse.stride(0), _stream_ptr(stream)))
     return coarse
 
@@ -215,7 +222,7 @@ def gprfwi_prolong_add(coarse: torch.Tensor, fine: torch.Tensor, scale: float = 
     nz, nx = fine.shape
     if tuple(coarse.shape) != ((nz + 1) // 2, (nx + 1) // 2):
         raise ValueError("coarse must have shape ((nz+1)//2, (nx+1)//2)")
-    check(_lib.load().gprfwi_prolong_add(_dev(coarse, "coarse"), coarse.stride(0), float(scale), _dev(fine, "fine"),
+    check(_lib.load().gprfwi_prolong_add(_plane(coarse, "coarse"), coarse.stride(0), float(scale), _plane(fine, "fine"),
                                          nz, nx, fine.stride(0), _stream_ptr(stream)))
     return fine
 
