@@ -70,12 +70,12 @@ def peaks():
 
 
 def kernel_source_sha() -> str:
-    """Hash of the CUDA sources: the key the ncu traffic table (profiles/dram_traffic.csv) is stored under
+    """Hash of the kernel sources (csrc/*.cuh): the key the ncu traffic table (profiles/dram_traffic.csv) is stored under
     (the GPU box has no .git, so a commit id cannot be read at run time)."""
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2506_20513_b200", "csrc")
     for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh")):
+        if f.endswith(".cuh"):            # the device code (kernels); host-only edits do not count
             with open(os.path.join(d, f), "rb") as fh:
                 h.update(f.encode()); h.update(fh.read())
     return h.hexdigest()[:16]

@@ -889,7 +889,7 @@ int gprfwi_forward_mu(gprfwi_handle** hp, const gprfwi_params* p, const float* e
   // fields are zero at n = 0
   GPR_CUDA(cudaMemsetAsync(h->c.fscratch, 0, 2 * L.blk(S) * f, st));
   float* slot[2] = {h->c.fscratch, h->c.fscratch + L.blk(S)};
-  rc = kernels_init(p, L);
+  if (!same_plan) rc = kernels_init(p, L);       // (function attributes: once per handle and plan)
   if (rc != GPRFWI_OK) return rc;
   if (L.full_history) GPR_CUDA(cudaMemsetAsync(h->c.hist, 0, S * L.plane * f, st));
   else GPR_CUDA(cudaMemsetAsync(h->c.ckpt, 0, L.blk(S) * f, st));       // checkpoint 0 = zero state

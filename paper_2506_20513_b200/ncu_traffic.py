@@ -32,7 +32,7 @@ def kernel_source_sha() -> str:
     h = hashlib.sha256()
     d = os.path.join(_HERE, "csrc")
     for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh")):
+        if f.endswith(".cuh"):            # the device code (kernels); host-only edits do not count
             with open(os.path.join(d, f), "rb") as fh:
                 h.update(f.encode()); h.update(fh.read())
     return h.hexdigest()[:16]
