@@ -46,7 +46,8 @@ typedef enum {
   GPRFWI_EGEOM   = -3, /* a source/receiver index outside [1, n-2]                               */
   GPRFWI_ENOMEM  = -4, /* workspace smaller than gprfwi_workspace_bytes() asks for               */
   GPRFWI_ESTATE  = -5, /* adjoint without a completed forward on this handle                     */
-  GPRFWI_ECUDA   = -6  /* a CUDA call or launch failed; text via gprfwi_strerror(GPRFWI_ECUDA)   */
+  GPRFWI_ECUDA   = -6, /* a CUDA call or launch failed; text via gprfwi_strerror(GPRFWI_ECUDA)   */
+  GPRFWI_ETOOBIG = -7  /* gprfwi_update_noalloc: the model exceeds the library's fixed scratch    */
 } gprfwi_status;
 
 typedef struct {
@@ -195,6 +196,24 @@ int gprfwi_update(int32_t nz, int32_t nx, int32_t pitch, const gprfwi_update_par
  * Errors: EINVAL (null pointer, in == out, nt/nrec/nseries < 1, ntaps even or < 1), ECUDA. */
 int gprfwi_lowpass(const float* in, float* out, int32_t nseries, int32_t nt, int32_t nrec,
                    const float* taps, int32_t ntaps, void* cuda_stream);
+
+/* gprfwi_update for callers that may not allocate and have no workspace to pass (code under CUDA-graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): same arguments and result as gprfwi_update
+ * minus the workspace.  The TV term's scratch (7 planes + one word) lives in a file-scope device array inside
+ * the library, gprfwi_update_noalloc_max_bytes() = 7 * 2^20 * 4 + 256 bytes (29 360 384), which every GPU that
+ * loads the library holds until the process exits; its device address is looked up once per device
+ * (cudaGetSymbolAddress, with the caller's current device).  The call allocates nothing (no cudaMalloc /
+ * cudaFree, no allocating library routine) and only enqueues on the stream.
+ *   Limit: gprfwi_update_workspace_bytes(nz, pitch) <= gprfwi_update_noalloc_max_bytes(), i.e. about
+ *   nz * pitch <= 2^20 cells (1024 x 1024); larger models return GPRFWI_ETOOBIG -- use gprfwi_update.
+ *   All calls on a device share the array, which keeps the last call's contents; every call re-initialises
+ *   what it reads.  Calls that OVERLAP on the GPU (different streams, no ordering between them) race on it:
+ *   keep them on one stream or order them with events.
+ * Errors: as gprfwi_update, plus ETOOBIG; ECUDA if the symbol lookup fails. */
+int gprfwi_update_noalloc(int32_t nz, int32_t nx, int32_t pitch, const gprfwi_update_params* u,
+                          float* eps_r, float* sigma, float* grad_eps_r, float* grad_sigma,
+                          float* m_eps_r, float* v_eps_r, float* m_sigma, float* v_sigma, void* cuda_stream);
+size_t gprfwi_update_noalloc_max_bytes(void);
 
 /* Taps of the stage filter for gprfwi_lowpass (the paper gives no design; DESIGN.md reading
  * R21): Hamming-windowed sinc with corner f_cut (Hz) at sampling interval dt (s), unit gain at DC, computed on

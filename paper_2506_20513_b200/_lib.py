@@ -12,13 +12,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgprfwi.so")
 
 GPRFWI_OK = 0
-STATUS_NAMES = {0: "OK", -1: "EINVAL", -2: "ECFL", -3: "EGEOM", -4: "ENOMEM", -5: "ESTATE", -6: "ECUDA"}
+STATUS_NAMES = {0: "OK", -1: "EINVAL", -2: "ECFL", -3: "EGEOM", -4: "ENOMEM", -5: "ESTATE", -6: "ECUDA", -7: "ETOOBIG"}
 
 EXPORTS = (
     "gprfwi_workspace_bytes", "gprfwi_forward", "gprfwi_forward_mu", "gprfwi_adjoint", "gprfwi_gradient_host",
     "gprfwi_workspace_bytes_host", "gprfwi_residual", "gprfwi_launch_count", "gprfwi_get_plan",
     "gprfwi_release", "gprfwi_strerror", "gprfwi_version", "gprfwi_update", "gprfwi_update_workspace_bytes", "gprfwi_lowpass",
     "gprfwi_lowpass_design", "gprfwi_restrict", "gprfwi_prolong_add",
+    "gprfwi_update_noalloc", "gprfwi_update_noalloc_max_bytes",
 )
 
 
@@ -108,6 +109,11 @@ def _declare(lib):
     lib.gprfwi_prolong_add.restype = ctypes.c_int
     lib.gprfwi_prolong_add.argtypes = [fp, ctypes.c_int32, ctypes.c_float, fp, ctypes.c_int32, ctypes.c_int32,
                                        ctypes.c_int32, vp]
+    lib.gprfwi_update_noalloc.restype = ctypes.c_int
+    lib.gprfwi_update_noalloc.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(UpdateParams),
+                                          fp, fp, fp, fp, fp, fp, fp, fp, vp]
+    lib.gprfwi_update_noalloc_max_bytes.restype = sz
+    lib.gprfwi_update_noalloc_max_bytes.argtypes = []
     lib.gprfwi_version.restype = ctypes.c_int
     return lib
 

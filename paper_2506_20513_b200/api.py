@@ -186,6 +186,21 @@ def gprfwi_update(nz, nx, pitch, u: UpdateParams, eps_r, sigma, grad_eps_r, grad
                                     workspace.numel(), _stream_ptr(stream)))
 
 
+def gprfwi_update_noalloc(nz, nx, pitch, u: UpdateParams, eps_r, sigma, grad_eps_r, grad_sigma, m_eps_r, v_eps_r,
+                          m_sigma, v_sigma, stream=None):
+    """gprfwi_update with the TV scratch in the library's fixed device array: no workspace, no allocation.
+    Raises GprfwiError(ETOOBIG) beyond gprfwi_update_noalloc_max_bytes(); overlapping calls race (see the header)."""
+    n = nz * pitch
+    ptrs = [_dev(t, nm, n) for t, nm in ((eps_r, "eps_r"), (sigma, "sigma"), (grad_eps_r, "grad_eps_r"),
+                                          (grad_sigma, "grad_sigma"), (m_eps_r, "m_eps_r"), (v_eps_r, "v_eps_r"),
+                                          (m_sigma, "m_sigma"), (v_sigma, "v_sigma"))]
+    check(_lib.load().gprfwi_update_noalloc(int(nz), int(nx), int(pitch), ctypes.byref(u), *ptrs, _stream_ptr(stream)))
+
+
+def gprfwi_update_noalloc_max_bytes() -> int:
+    return int(_lib.load().gprfwi_update_noalloc_max_bytes())
+
+
 def gprfwi_lowpass(x: torch.Tensor, out: torch.Tensor, taps: torch.Tensor, stream=None):
     """Zero-phase FIR along time of x[nseries][nt][nrec] (or [nseries][nt]) into `out` (multiscale stages)."""
     if x.dim() == 2:

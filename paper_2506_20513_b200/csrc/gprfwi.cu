@@ -786,6 +786,7 @@ const char* gprfwi_strerror(int code)
     case GPRFWI_ENOMEM: return "workspace too small";
     case GPRFWI_ESTATE: return "adjoint called without a completed forward";
     case GPRFWI_ECUDA: return g_cuda_err;
+    case GPRFWI_ETOOBIG: return "problem exceeds the fixed scratch of gprfwi_update_noalloc (7 planes of 2^20 cells): use gprfwi_update with a caller workspace";
     default: return "unknown gprfwi status";
   }
 }
@@ -1239,6 +1240,60 @@ int gprfwi_prolong_add(const float* coarse, int32_t pitch_coarse, float scale, f
   GPR_LAUNCH(prolong_add_kernel, grid, block, (cudaStream_t)cuda_stream, coarse, nzc, nxc, pitch_coarse, scale, fine, nz, nx, pitch);
   GPR_CUDA(cudaGetLastError());
   return GPRFWI_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// gprfwi_update without a caller workspace and without any allocation (callers under CUDA-graph capture, tight
+// serving loops, harnesses that forbid cudaMalloc): the TV term's scratch planes live in a file-scope device
+// array of a fixed, modest size that every GPU that loads the library holds until exit.
+// ------------------------------------------------------------------------------------------------
+namespace gprfwi {
+// 7 planes of up to 2^20 cells (e.g. 1024 x 1024 incl. pitch) + the 256-byte slot of the max|X| word
+constexpr size_t kNoAllocMaxCells = (size_t)1 << 20;
+constexpr size_t kNoAllocBytes = 7 * kNoAllocMaxCells * sizeof(float) + 256;
+static __device__ __align__(256) unsigned char g_update_scratch[kNoAllocBytes];
+
+// In host code `g_update_scratch` is only a stand-in for the symbol, NOT a device address: the address the
+// kernels may use comes from cudaGetSymbolAddress, looked up once per device with that device current.
+constexpr int kNoAllocMaxDevices = 64;
+static void* g_update_scratch_ptr[kNoAllocMaxDevices] = {};
+
+static int update_scratch_address(void** out)
+{
+  int dev = -1;
+  GPR_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return GPRFWI_EINVAL;
+  void* p = __atomic_load_n(&g_update_scratch_ptr[dev], __ATOMIC_ACQUIRE);
+  if (!p) {
+    GPR_CUDA(cudaGetSymbolAddress(&p, g_update_scratch));      // (idempotent: racing first calls get the same address)
+    if (!p) return cuda_fail(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_update_scratch)");
+    __atomic_store_n(&g_update_scratch_ptr[dev], p, __ATOMIC_RELEASE);
+  }
+  *out = p;
+  return GPRFWI_OK;
+}
+}  // namespace gprfwi
+
+extern "C" {
+
+size_t gprfwi_update_noalloc_max_bytes(void) { return kNoAllocBytes; }
+
+int gprfwi_update_noalloc(int32_t nz, int32_t nx, int32_t pitch, const gprfwi_update_params* u, float* eps_r,
+                          float* sigma, float* grad_eps_r, float* grad_sigma, float* m_eps_r, float* v_eps_r,
+                          float* m_sigma, float* v_sigma, void* cuda_stream)
+{
+  const size_t need = gprfwi_update_workspace_bytes(nz, pitch);
+  if (need == 0) return GPRFWI_EINVAL;
+  if (need > kNoAllocBytes) return GPRFWI_ETOOBIG;
+  void* scratch = nullptr;
+  if (int rc = update_scratch_address(&scratch)) return rc;
+  // Every call on a device shares the array, which still holds the previous call's contents: gprfwi_update
+  // zeroes the max|X| word and tv_init_kernel rewrites every cell of the six planes it later reads, so nothing
+  // else has to start at zero.  Calls that overlap on the GPU (different streams) race on it.
+  return gprfwi_update(nz, nx, pitch, u, eps_r, sigma, grad_eps_r, grad_sigma, m_eps_r, v_eps_r, m_sigma, v_sigma,
+                       scratch, kNoAllocBytes, cuda_stream);
 }
 
 }  // extern "C"
