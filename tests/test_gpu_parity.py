@@ -721,6 +721,31 @@ def test_config5_512_full_nt_and_1024_batch32_against_oracle():
     _one_hot_residual_case(gi.config5(n=1024, batch=32), 31, _bench_budget(), oracle_stride=0, tol_local=1e-3)
 
 
+def test_config5_8192_grid_short_run_and_batch128_against_oracle():
+    """The two corners of config 5's sweep that bench.py times and no other test touches: the 8192 x 8192 grid
+    (20 520 tiles, plane offsets beyond 2^26 cells) for 16 steps with one source near the bottom-right corner and
+    six receivers within reach of the wave -- everything the wave has not reached must stay exactly zero --, and
+    512^2 with B = 128 shots in ONE call at the full nt = 1000 (one-hot residual on the last shot)."""
+    import dataclasses
+    wl = gi.config5(n=8192, batch=1, nt=16)
+    off = np.array([(2, 0), (0, 3), (-3, -1), (4, 4), (-2, 2), (1, -4)])
+    src = np.array([(8150, 8160)])
+    wl = gi.with_geometry(wl, src, src[:, None, :] + off[None, :, :], name="config5-8192-short")
+    wl = dataclasses.replace(wl, wavelet=np.sin(0.6 * np.arange(16)).astype(np.float32))
+    pb = problem(wl)
+    tr_o = oracle.forward(pb, wl.eps_r, wl.sigma)["traces"]
+    res = gi.random_residual(wl, float(np.sqrt(np.mean(tr_o ** 2))))
+    ge_o, gs_o = oracle.gradient(pb, wl.eps_r, wl.sigma, res, checkpoint_stride=4)      # (5 planes of 0.5 GB, not 17)
+    tr, ge, gs, plan = run_gpu(wl, res)
+    assert_parity(wl, (tr, ge, gs), (tr_o, ge_o, gs_o), " 8192^2, 16 steps")
+    far = np.ones((wl.nz, wl.nx), bool)
+    far[8150 - 40:8150 + 41, 8160 - 40:] = False
+    assert np.all(ge[far] == 0.0) and np.all(gs[far] == 0.0) and np.all(ge_o[far] == 0.0)
+    del tr, ge, gs, ge_o, gs_o, far
+    plan = _one_hot_residual_case(gi.config5(n=512, batch=128), 127, _bench_budget(), oracle_stride=0, tol_local=1e-3)
+    assert plan["shots_per_pass"] == 128 and plan["full_history"] == 1
+
+
 def test_split_batch_multi_call_sum_against_oracle():
     """bench.py sweeps a batch that does not fit one call as several calls through one workspace and sums the
     gradients (split_batch picks the split): 512^2, B = 8, nt = 400 under a budget that forces more than
