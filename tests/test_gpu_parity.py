@@ -746,6 +746,42 @@ def test_config5_8192_grid_short_run_and_batch128_against_oracle():
     assert plan["shots_per_pass"] == 128 and plan["full_history"] == 1
 
 
+def test_iteration_is_cuda_graph_capturable_after_one_warm_call():
+    """The boundary's "calls only enqueue" contract, checked the hard way: after one warm call on a handle (which
+    allocates the handle's pinned staging block and streams), forward -> residual -> adjoint on the same handle
+    is captured into a CUDA graph -- programmatic dependent launches, the forked launch lanes and the memsets
+    included -- and the replay, after the models were changed IN PLACE, is bit-identical to an eager run."""
+    wl = gi.small_random(nz=70, nx=150, nt=60, npml=10, nshots=3, nrec=6, seed=515)
+    sim = Simulation(params_of(wl), wl.src_zx, wl.rec_zx, wl.wavelet, dev())
+    eps = torch.as_tensor(wl.eps_r.copy(), device=dev()); sig = torch.as_tensor(wl.sigma.copy(), device=dev())
+    d_obs = torch.as_tensor(gi.random_residual(wl, 1.0), device=dev()); res = torch.empty_like(d_obs)
+
+    def iteration():
+        gprfwi_residual(sim.forward(eps, sig), d_obs, res)
+        sim.adjoint(res)
+
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        iteration()                                    # warm call: everything that allocates happens here
+        torch.cuda.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            iteration()
+    torch.cuda.synchronize()
+    eps.mul_(1.1); sig.add_(1e-3)                      # new models, same buffers
+    for t in (sim.traces, sim.grad_eps_r, sim.grad_sigma):
+        t.fill_(float("nan"))
+    graph.replay()
+    torch.cuda.synchronize()
+    got = [t.clone() for t in (sim.traces, sim.grad_eps_r, sim.grad_sigma)]
+    iteration()
+    torch.cuda.synchronize()
+    for a, b in zip(got, (sim.traces, sim.grad_eps_r, sim.grad_sigma)):
+        assert torch.isfinite(a).all() and torch.equal(a, b)
+    sim.close()
+
+
 def test_split_batch_multi_call_sum_against_oracle():
     """bench.py sweeps a batch that does not fit one call as several calls through one workspace and sums the
     gradients (split_batch picks the split): 512^2, B = 8, nt = 400 under a budget that forces more than
