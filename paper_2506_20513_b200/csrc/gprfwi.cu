@@ -607,17 +607,19 @@ static int maps_init(gprfwi_handle* h, bool same_plan)
   return GPRFWI_OK;
 }
 
-static int kernels_init(const gprfwi_params* p, const Layout& L)
+// The limit on dynamic shared memory is an attribute of the KERNEL (per device), not of a handle: it is set to
+// the largest request any problem can make (CPML psi slots, and for the mu_r variants the per-cell Db slots), so
+// that live handles with and without a CPML never lower it under one another.
+static int kernels_init(const gprfwi_params*, const Layout& L)
 {
-  const bool pml = p->npml > 0;      // (the largest request either variant makes)
   GPR_CUDA(cudaFuncSetAttribute(kFwdShapes[L.fv].func, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)kFwdShapes[L.fv].smem(pml)));
+                                (int)kFwdShapes[L.fv].smem(true)));
   GPR_CUDA(cudaFuncSetAttribute(kAdjShapes[L.av].func, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)kAdjShapes[L.av].smem(pml)));
+                                (int)kAdjShapes[L.av].smem(true)));
   GPR_CUDA(cudaFuncSetAttribute(kFwdShapes[L.fv].func_mu, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)kFwdShapes[L.fv].smem(pml, true)));
+                                (int)kFwdShapes[L.fv].smem(true, true)));
   GPR_CUDA(cudaFuncSetAttribute(kAdjShapes[L.av].func_mu, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)kAdjShapes[L.av].smem(pml, true)));
+                                (int)kAdjShapes[L.av].smem(true, true)));
   return GPRFWI_OK;
 }
 

@@ -502,6 +502,24 @@ def test_handle_reuse_with_new_geometry():
     sim.close()
 
 
+def test_two_live_handles_with_and_without_cpml_interleaved():
+    """Two handles alive at once, one with a CPML and one PEC box (whose kernels ask for less dynamic shared
+    memory), called alternately: the kernels' shared-memory limit is a per-kernel attribute, so neither handle
+    may lower it under the other; results must equal those of fresh handles bit for bit."""
+    a = gi.small_random(nz=64, nx=130, nt=60, npml=8, nshots=2, nrec=5, seed=91)
+    b = gi.small_random(nz=40, nx=40, nt=60, npml=0, nshots=2, nrec=5, seed=92)
+    ra, rb = gi.random_residual(a, 1.0, seed=3), gi.random_residual(b, 1.0, seed=4)
+    ref = {"a": run_gpu(a, ra), "b": run_gpu(b, rb)}
+    sims = {k: Simulation(params_of(w), w.src_zx, w.rec_zx, w.wavelet, dev()) for k, w in (("a", a), ("b", b))}
+    models = {k: (torch.as_tensor(w.eps_r, device=dev()), torch.as_tensor(w.sigma, device=dev())) for k, w in (("a", a), ("b", b))}
+    for k, res in (("a", ra), ("b", rb), ("a", ra), ("b", rb), ("a", ra)):
+        tr = sims[k].forward(*models[k]).cpu().numpy().copy()
+        ge, gs = [t.cpu().numpy().copy() for t in sims[k].adjoint(torch.as_tensor(res, device=dev()))]
+        assert np.array_equal(tr, ref[k][0]) and np.array_equal(ge, ref[k][1]) and np.array_equal(gs, ref[k][2]), k
+    for sm in sims.values():
+        sm.close()
+
+
 def test_inversion_loop_reduces_misfit_and_recovers_anomaly():
     """the whole iteration (forward, residual, adjoint, TV + Adam update) as C-ABI calls.
     Config 1: start from the layered background, observed data from the model with the disc; the
