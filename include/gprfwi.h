@@ -209,6 +209,8 @@ int gprfwi_lowpass(const float* in, float* out, int32_t nseries, int32_t nt, int
  *   All calls on a device share the array, which keeps the last call's contents; every call re-initialises
  *   what it reads.  Calls that OVERLAP on the GPU (different streams, no ordering between them) race on it:
  *   keep them on one stream or order them with events.
+ *   The FIRST call on a device performs the address lookup (a runtime query, not a stream operation): callers
+ *   that will run under CUDA-graph capture make one call on that device before they begin capturing.
  * Errors: as gprfwi_update, plus ETOOBIG; ECUDA if the symbol lookup fails. */
 int gprfwi_update_noalloc(int32_t nz, int32_t nx, int32_t pitch, const gprfwi_update_params* u,
                           float* eps_r, float* sigma, float* grad_eps_r, float* grad_sigma,
